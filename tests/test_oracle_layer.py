@@ -1,0 +1,236 @@
+"""Pins for oracle/layer.py (CPU only): brute force, degenerate layers, adjoint identities."""
+import numpy as np
+import pytest
+
+from oracle import layer, nvfp4
+from paper_2607_05711_b200 import synth
+
+
+def _tiny_layer(seed, M, K, N, r_s, r):
+    d = synth.layer_inputs(seed, M, K, N, max(r, 1))
+    R, L1, L2 = layer.prepare_weight(d["W"], r_s)
+    A, B = d["A"][:, :r], d["B"][:r, :]
+    D_f = np.concatenate([L1, A], axis=1).astype(np.float32)
+    U_f = np.concatenate([L2, B], axis=0).astype(np.float32)
+    return d["X"], d["dY"], R, D_f, U_f, d["W"]
+
+
+# ---------------------------------------------------------------- Eq. 1 / O-13
+def test_prepare_weight_split():
+    rng = synth.make_rng(11)
+    W = synth.normal(rng, (96, 64), 0.02)
+    # plant a rank-2 high-magnitude component (the "outliers" of PAPER.md:80)
+    u = rng.standard_normal((96, 2)).astype(np.float32)
+    v = rng.standard_normal((2, 64)).astype(np.float32)
+    W = synth.to_bf16_f32(W + 0.5 * (u @ v) / 8)
+    R, L1, L2 = layer.prepare_weight(W, 4)
+    assert L1.shape == (64, 4) and L2.shape == (4, 96) and R.shape == W.shape
+    rec = R.astype(np.float64) + (L1.astype(np.float64) @ L2.astype(np.float64)).T
+    # R absorbs the bf16 rounding of L1, L2: reconstruction is exact up to one bf16 rounding of R
+    assert np.max(np.abs(rec - W)) <= np.max(np.abs(R)) * 2.0 ** -8
+    # Eckart-Young: the residual's spectral norm is the 5th singular value of W (up to rounding)
+    s = np.linalg.svd(W.astype(np.float64), compute_uv=False)
+    sR = np.linalg.svd(R.astype(np.float64), compute_uv=False)
+    assert abs(sR[0] - s[4]) < 0.02 * s[4] + 1e-3
+    # stabilizer makes the residual easier to quantize than W (stand-in for Fig. 8 / Table 5)
+    rel = lambda a: np.linalg.norm(nvfp4.dequantize(nvfp4.quantize_blockwise(a, 16)) - a)
+    assert rel(R) < rel(W)
+    # r_s = 0 -> R = W
+    R0, L10, L20 = layer.prepare_weight(W, 0)
+    assert np.array_equal(R0, W) and L10.shape == (64, 0) and L20.shape == (0, 96)
+
+
+# ------------------------------------------------------- P-7: brute force loops
+def _brute_forward(X, R, D_f, U_f):
+    """Pure-Python restatement of F from the scalar definitions (no numpy matmul,
+    no shared quantizer internals beyond the per-element grids)."""
+    M, K = X.shape
+    N = R.shape[0]
+    r_t = D_f.shape[1]
+    qX = nvfp4.quantize_blockwise(X, 1)
+    qR = nvfp4.quantize_blockwise(R, 16)
+    gx, gr = float(qX["g_dec"]), float(qR["g_dec"])
+    Y = np.zeros((M, N))
+    H = np.zeros((M, r_t), np.float32)
+    for m in range(M):
+        for j in range(r_t):
+            s = 0.0
+            for k in range(K):
+                s += float(X[m, k]) * float(D_f[k, j])
+            H[m, j] = nvfp4.bf16_round_from_f64(np.array([s]))[0]
+    for m in range(M):
+        for n in range(N):
+            s = 0.0
+            for k in range(K):
+                xv = float(nvfp4.e2m1_decode(qX["codes"][m, k])) * float(nvfp4.e4m3_decode(qX["sf"][m, k // 16])) * gx
+                rv = float(nvfp4.e2m1_decode(qR["codes"][n, k])) * float(nvfp4.e4m3_decode(qR["sf"][n // 16, k // 16])) * gr
+                s += xv * rv
+            for j in range(r_t):
+                s += float(H[m, j]) * float(U_f[j, n])
+            Y[m, n] = s
+    return Y, H
+
+
+def test_forward_bruteforce_tiny():
+    X, G, R, D_f, U_f, _ = _tiny_layer(21, 3, 32, 16, 2, 2)
+    Yb, Hb = _brute_forward(X, R, D_f, U_f)
+    out = layer.forward(X, layer.quantize_weight(R), D_f, U_f, prescale=False, out_bf16=False)
+    assert np.array_equal(out["H"], Hb)
+    assert np.allclose(out["Y"], Yb, rtol=1e-12, atol=1e-15)
+
+
+def test_dgrad_wgrad_bruteforce_tiny():
+    X, G, R, D_f, U_f, _ = _tiny_layer(22, 3, 32, 16, 2, 2)
+    M, K = X.shape
+    N = R.shape[0]
+    r_s, r_t = 2, 4
+    qR = layer.quantize_weight(R)
+    qG = nvfp4.quantize_blockwise(G, 1)
+    dqG, dqR = nvfp4.dequantize(qG), nvfp4.dequantize(qR)
+    out = layer.dgrad(G, qR, D_f, U_f, prescale=False, out_bf16=False)
+    P = out["P"]
+    for m in range(M):
+        for j in range(r_t):
+            s = sum(float(G[m, n]) * float(U_f[j, n]) for n in range(N))
+            assert P[m, j] == nvfp4.bf16_round_from_f64(np.array([s]))[0]
+        for k in range(K):
+            s = sum(dqG[m, n] * dqR[n, k] for n in range(N))
+            s += sum(float(P[m, j]) * float(D_f[k, j]) for j in range(r_t))
+            assert abs(out["dX"][m, k] - s) <= 1e-12 * max(1.0, abs(s))
+    fw = layer.forward(X, qR, D_f, U_f)
+    w = layer.wgrad(X, G, fw["H"], P, r_s)
+    for j in range(r_t - r_s):
+        for n in range(N):
+            s = sum(float(fw["H"][m, r_s + j]) * float(G[m, n]) for m in range(M))
+            assert abs(w["dB"][j, n] - s) <= 1e-6 * max(1e-6, abs(s))
+        for k in range(K):
+            s = sum(float(X[m, k]) * float(P[m, r_s + j]) for m in range(M))
+            assert abs(w["dA"][k, j] - s) <= 1e-6 * max(1e-6, abs(s))
+    assert w["dA"].shape == (K, 2) and w["dB"].shape == (2, N)
+
+
+# ------------------------------------------------------ P-5: degenerate layers
+def test_no_lowrank_reduces_to_matmul_of_dequantized():
+    X, G, R, D_f, U_f, _ = _tiny_layer(23, 20, 64, 48, 0, 0)
+    assert D_f.shape[1] == 0
+    qR = layer.quantize_weight(R)
+    for prescale in (False, True):
+        out = layer.forward(X, qR, D_f, U_f, prescale=prescale, out_bf16=False)
+        ref = nvfp4.dequantize(out["qX"]) @ nvfp4.dequantize(qR).T
+        rtol = 2e-7 if prescale else 1e-12      # alpha is ONE float32 product in the prescaled variant
+        assert np.allclose(out["Y"], ref, rtol=rtol, atol=0)
+        outb = layer.dgrad(G, qR, D_f, U_f, prescale=prescale, out_bf16=False)
+        refb = nvfp4.dequantize(outb["qG"]) @ nvfp4.dequantize(qR)
+        assert np.allclose(outb["dX"], refb, rtol=rtol, atol=0)
+
+
+def test_zero_adapter_cases():
+    X, G, R, D_f, U_f, _ = _tiny_layer(24, 16, 64, 32, 4, 4)
+    qR = layer.quantize_weight(R)
+    r_s = 4
+    base = layer.forward(X, qR, D_f, U_f, out_bf16=False)
+    # B = 0: branch 3 contributes exactly 0 to Y and dX; dA = 0, dB != 0
+    U0 = U_f.copy(); U0[r_s:] = 0
+    f0 = layer.forward(X, qR, D_f, U0, out_bf16=False)
+    no_lora = layer.forward(X, qR, D_f[:, :r_s], U_f[:r_s], out_bf16=False)
+    assert np.array_equal(f0["Y"], no_lora["Y"])
+    assert not np.array_equal(f0["Y"], base["Y"])
+    b0 = layer.dgrad(G, qR, D_f, U0, out_bf16=False)
+    bn = layer.dgrad(G, qR, D_f[:, :r_s], U_f[:r_s], out_bf16=False)
+    assert np.array_equal(b0["dX"], bn["dX"])
+    w0 = layer.wgrad(X, G, f0["H"], b0["P"], r_s)
+    assert np.count_nonzero(w0["dA"]) == 0 and np.count_nonzero(w0["dB"]) > 0
+    # A = 0: dB = 0
+    D0 = D_f.copy(); D0[:, r_s:] = 0
+    fA = layer.forward(X, qR, D0, U_f)
+    bA = layer.dgrad(G, qR, D0, U_f)
+    wA = layer.wgrad(X, G, fA["H"], bA["P"], r_s)
+    assert np.count_nonzero(wA["dB"]) == 0 and np.count_nonzero(wA["dA"]) > 0
+    # L1 = 0: stabilizer vanishes
+    D1 = D_f.copy(); D1[:, :r_s] = 0
+    f1 = layer.forward(X, qR, D1, U_f, out_bf16=False)
+    f1n = layer.forward(X, qR, D_f[:, r_s:], U_f[r_s:], out_bf16=False)
+    assert np.allclose(f1["Y"], f1n["Y"], rtol=1e-13, atol=1e-18)
+
+
+# ------------------------------------------- P-6: exact-linearity special case
+def _grid_exact(rng, rows, cols, block_rows, emin, emax):
+    """Values from the E2M1 grid times one power of two per block, every block
+    holding a +-6, so that Q is the identity given amax_t = 2688 * 2^-J."""
+    codes = rng.integers(0, 16, (rows, cols)).astype(np.uint8)
+    br = block_rows
+    cb = codes.reshape(rows // br, br, cols // 16, 16)
+    cb[:, 0, :, 0] = 7
+    expo = rng.integers(emin, emax + 1, (rows // br, cols // 16))
+    scale = np.repeat(np.repeat(np.exp2(expo), br, 0), 16, 1)
+    return (nvfp4.e2m1_decode(codes) * scale).astype(np.float32)
+
+
+def test_adjoint_identity_exact_linear_case():
+    rng = np.random.default_rng(31)
+    M, K, N, r_s, r = 8, 64, 48, 2, 3
+    R = _grid_exact(rng, N, K, 16, -5, 1)
+    amax = 2688.0 / 64.0
+    qR = nvfp4.quantize_blockwise(R, 16, amax_t=amax)
+    assert np.array_equal(nvfp4.dequantize(qR), R.astype(np.float64))         # Q is the identity here
+    # low-rank factors with few significant bits so that bf16(H), bf16(P) are exact
+    D_f = (rng.integers(-2, 3, (K, r_s + r)) * 2.0 ** -3).astype(np.float32)
+    U_f = (rng.integers(-2, 3, (r_s + r, N)) * 2.0 ** -3).astype(np.float32)
+    Xs = (rng.integers(-3, 4, (M, K)) * 0.5).astype(np.float32)               # small-integer X for exact H
+    Xs[:, ::16] = 6.0
+    qXs = nvfp4.quantize_blockwise(Xs, 1, amax_t=amax)
+    assert np.array_equal(nvfp4.dequantize(qXs), Xs.astype(np.float64))
+    Gs = (rng.integers(-3, 4, (M, N)) * 0.5).astype(np.float32); Gs[:, ::16] = 6.0
+    f = layer.forward(Xs, qR, D_f, U_f, x_amax=amax, out_bf16=False)
+    b = layer.dgrad(Gs, qR, D_f, U_f, g_amax=amax, out_bf16=False)
+    assert np.array_equal(f["H"].astype(np.float64), Xs.astype(np.float64) @ D_f.astype(np.float64))
+    # with Q the identity the layer is Y = X W_eff: <Y, G> == <X, dX> for all three branches
+    W_eff = R.astype(np.float64).T + D_f.astype(np.float64) @ U_f.astype(np.float64)      # K x N
+    assert np.allclose(f["Y"], Xs.astype(np.float64) @ W_eff, rtol=1e-13)
+    assert np.allclose(b["dX"], Gs.astype(np.float64) @ W_eff.T, rtol=1e-13)
+    lhs = np.sum(f["Y"] * Gs.astype(np.float64))
+    rhs = np.sum(Xs.astype(np.float64) * b["dX"])
+    assert abs(lhs - rhs) <= 1e-12 * abs(lhs)
+    # Eq. 4: <dA, A'> + <dB, B'> is the directional derivative of <Y, G> along (A', B')
+    w = layer.wgrad(Xs, Gs, f["H"], b["P"], r_s)
+    Ad = rng.standard_normal((K, r)); Bd = rng.standard_normal((r, N))
+    A0, B0 = D_f[:, r_s:].astype(np.float64), U_f[r_s:].astype(np.float64)
+    Xd, Gd = Xs.astype(np.float64), Gs.astype(np.float64)
+    dirder = np.sum((Xd @ (Ad @ B0 + A0 @ Bd)) * Gd)
+    got = np.sum(w["dA"].astype(np.float64) * Ad) + np.sum(w["dB"].astype(np.float64) * Bd)
+    assert abs(got - dirder) <= 1e-6 * abs(dirder) + 1e-9
+    # guard that the check can fail: a slipped wgrad (H and P exchanged in role) breaks it
+    slipped = np.sum((Xd.T @ f["H"][:, r_s:].astype(np.float64)) * Ad)
+    assert abs(slipped + np.sum(w["dB"].astype(np.float64) * Bd) - dirder) > 1e-3 * abs(dirder)
+
+
+# ------------------------------------- O-10': the prescaled variant is the same layer
+def test_prescaled_variant_close_to_plain():
+    X, G, R, D_f, U_f, _ = _tiny_layer(25, 64, 256, 128, 8, 8)
+    qR = layer.quantize_weight(R)
+    a = layer.forward(X, qR, D_f, U_f, prescale=False, out_bf16=False)
+    p = layer.forward(X, qR, D_f, U_f, prescale=True, out_bf16=False)
+    assert np.array_equal(a["H"], p["H"])
+    # the two differ only by one bf16 rounding of the rank-r_t intermediate
+    lr = a["H"].astype(np.float64) @ U_f.astype(np.float64)
+    diff = np.linalg.norm(a["Y"] - p["Y"])
+    assert 0 < diff <= 2.0 ** -7 * np.linalg.norm(lr)
+    # Hs * alpha reproduces H to bf16 precision
+    assert np.allclose(p["Hs"].astype(np.float64) * p["alpha"], a["H"], rtol=2.0 ** -7)
+    # staged comparison hook: feeding Hs back in reproduces the same Y
+    p2 = layer.forward(X, qR, D_f, U_f, prescale=True, H_given=p["Hs"], out_bf16=False)
+    assert np.array_equal(p2["Y"], p["Y"])
+    ab = layer.dgrad(G, qR, D_f, U_f, prescale=False, out_bf16=False)
+    pb = layer.dgrad(G, qR, D_f, U_f, prescale=True, out_bf16=False)
+    lrb = ab["P"].astype(np.float64) @ D_f.astype(np.float64).T
+    assert np.linalg.norm(ab["dX"] - pb["dX"]) <= 2.0 ** -7 * np.linalg.norm(lrb)
+
+
+def test_qrt_is_permuted_qr_in_dgrad():
+    """dgrad with Q(R)^T must equal dgrad with a separately quantized R^T (16x16 blocks)."""
+    X, G, R, D_f, U_f, _ = _tiny_layer(26, 16, 64, 32, 0, 0)
+    qR = layer.quantize_weight(R)
+    qRt = layer.quantize_weight(np.ascontiguousarray(R.T))
+    out = layer.dgrad(G, qR, D_f, U_f, out_bf16=False)
+    ref = nvfp4.dequantize(out["qG"]) @ nvfp4.dequantize(qRt).T
+    assert np.allclose(out["dX"], ref, rtol=1e-10, atol=1e-14 * np.abs(ref).max())   # summation order only

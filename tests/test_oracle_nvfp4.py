@@ -1,0 +1,259 @@
+"""Pins for oracle/nvfp4.py (CPU only).  Each test names the pin of DESIGN.md it is."""
+import os
+import shutil
+import subprocess
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import nvfp4
+from paper_2607_05711_b200 import synth
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+GOLD = os.path.join(HERE, "golden")
+
+
+# ---------------------------------------------------------------- bf16 helpers
+def test_bf16_round_matches_torch():
+    rng = np.random.default_rng(0)
+    x = np.concatenate([rng.standard_normal(20000).astype(np.float32) * 10.0 ** rng.integers(-8, 8, 20000),
+                        np.array([1.00390625, 1.01171875, 0.0, -0.0, 3e-39, 65280.0], np.float32)])
+    ref = torch.from_numpy(x).to(torch.bfloat16).to(torch.float32).numpy()
+    assert np.array_equal(nvfp4.bf16_round(x).view(np.uint32), ref.view(np.uint32))
+    assert np.array_equal(synth.to_bf16_f32(x).view(np.uint32), ref.view(np.uint32))
+    assert np.array_equal(nvfp4.bf16_round_from_f64(x.astype(np.float64)).view(np.uint32), ref.view(np.uint32))
+    bits = nvfp4.bf16_to_bits(ref)
+    assert np.array_equal(nvfp4.bits_to_bf16(bits), ref)
+
+
+def test_bf16_from_f64_single_rounding():
+    # 1 + 2^-8 + 2^-30 is above the bf16 midpoint: must round UP although the
+    # float32 rounding of it lands exactly on the midpoint (which ties to even = down).
+    x = np.array([1.0 + 2.0 ** -8 + 2.0 ** -30])
+    assert nvfp4.bf16_round_from_f64(x)[0] == np.float32(1.0078125)
+    assert nvfp4.bf16_round(x)[0] == np.float32(1.0)
+
+
+# ------------------------------------------------------ P-2: independent source
+@pytest.fixture(scope="module")
+def cuda_cvt_table(tmp_path_factory):
+    inc = "/usr/local/cuda/include"
+    if not (shutil.which("g++") and os.path.exists(os.path.join(inc, "cuda_fp4.h"))):
+        pytest.skip("g++ or cuda_fp4.h not available")
+    exe = str(tmp_path_factory.mktemp("cvt") / "cvt_table")
+    subprocess.check_call(["g++", "-O1", "-I", inc, os.path.join(HERE, "cuda_cvt_table.cpp"), "-o", exe])
+    out = subprocess.check_output([exe]).decode().split()
+    tab = np.array([int(v, 16) for v in out], dtype=np.int64).reshape(65536, 3)
+    assert np.array_equal(tab[:, 0], np.arange(65536))
+    return tab
+
+
+def test_e2m1_exhaustive_vs_cuda_header(cuda_cvt_table):
+    """P-2: all finite bf16 patterns, oracle E2M1 == __nv_cvt_float_to_fp4."""
+    bits = np.arange(65536, dtype=np.uint16)
+    v = nvfp4.bits_to_bf16(bits)
+    fin = np.isfinite(v)
+    assert fin.sum() == 65536 - 2 * 128
+    got = nvfp4.e2m1_encode(v[fin])
+    assert np.array_equal(got, cuda_cvt_table[fin, 1].astype(np.uint8))
+
+
+def test_e4m3_exhaustive_vs_cuda_header(cuda_cvt_table):
+    """P-2: all finite non-negative bf16 patterns, oracle E4M3 == __nv_cvt_float_to_fp8."""
+    bits = np.arange(0x8000, dtype=np.uint16)
+    v = nvfp4.bits_to_bf16(bits)
+    fin = np.isfinite(v)
+    got = nvfp4.e4m3_encode(v[fin])
+    assert np.array_equal(got, cuda_cvt_table[:0x8000][fin, 2].astype(np.uint8))
+    assert got.max() == 0x7E
+
+
+def test_e4m3_dense_float32_vs_decode_bruteforce():
+    """Q2 on float32 inputs finer than bf16: nearest of the 127 decoded values, ties to even code."""
+    grid = nvfp4.e4m3_decode(np.arange(0x7F, dtype=np.uint8))
+    assert np.all(np.diff(grid) > 0) and grid[-1] == 448.0 and grid[1] == 2.0 ** -9
+    rng = np.random.default_rng(1)
+    t = np.concatenate([np.exp(rng.uniform(np.log(1e-4), np.log(600.0), 50000)),
+                        (grid[:-1] + grid[1:]) / 2, grid]).astype(np.float32)
+    got = nvfp4.e4m3_encode(t).astype(np.int64)
+    t64 = t.astype(np.float64)
+    d = np.abs(t64[:, None] - grid[None, :])
+    best = d.min(axis=1)
+    for i in range(len(t)):
+        cands = np.nonzero(d[i] == best[i])[0]
+        want = cands[0] if len(cands) == 1 else [c for c in cands if c % 2 == 0][0]
+        assert got[i] == want, (t[i], got[i], want)
+
+
+def test_e2m1_golden_ties():
+    for line in open(os.path.join(GOLD, "e2m1_ties.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        val, code = line.split()
+        got = int(nvfp4.e2m1_encode(np.array([float(val)], np.float32))[0])
+        assert got == int(code, 16), (val, got, code)
+
+
+def test_e2m1_decode_roundtrip():
+    codes = np.arange(16, dtype=np.uint8)
+    vals = nvfp4.e2m1_decode(codes)
+    assert list(vals[:8]) == [0, 0.5, 1, 1.5, 2, 3, 4, 6]
+    assert np.array_equal(nvfp4.e2m1_encode(vals.astype(np.float32)), codes)
+
+
+# --------------------------------------------------------- P-1: hand-worked blocks
+def _golden_blocks():
+    out, packed = [], None
+    for line in open(os.path.join(GOLD, "nvfp4_blocks.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        parts = [p.strip() for p in line.split("|")]
+        if parts[0] == "PACKED_A":
+            packed = bytes(int(b, 16) for b in parts[1].split())
+            continue
+        name, amax_t, xs, sf, codes = parts
+        out.append((name, float(amax_t), [float(v) for v in xs.split()], int(sf, 16),
+                    [int(c, 16) for c in codes.split()]))
+    return out, packed
+
+
+def test_golden_blocks():
+    blocks, packed_a = _golden_blocks()
+    assert len(blocks) == 5
+    for name, amax_t, xs, sf, codes in blocks:
+        x = nvfp4.bf16_round(np.array([xs], np.float32))
+        q = nvfp4.quantize_blockwise(x, amax_t=amax_t)
+        assert int(q["sf"][0, 0]) == sf, name
+        assert list(q["codes"][0]) == codes, name
+        if name == "A":
+            assert q["packed"][0].tobytes() == packed_a
+    # values quoted in the derivations
+    g_enc, g_dec = nvfp4.tensor_scales(0.45)
+    assert abs(float(g_enc) - 5973.3335) < 1e-3 and abs(float(g_dec) - 1.674107e-4) < 1e-10
+
+
+def test_tensor_scale_special_cases():
+    assert nvfp4.tensor_scales(0.0) == (np.float32(1.0), np.float32(1.0))
+    g_enc, g_dec = nvfp4.tensor_scales(1e-38)
+    assert g_enc == np.finfo(np.float32).max and np.isfinite(g_dec)
+    assert nvfp4.tensor_scales(2688.0)[0] == np.float32(1.0)
+    assert nvfp4.tensor_scales(6.0) == (np.float32(448.0), np.float32(1.0) / np.float32(448.0))
+
+
+# ------------------------------------------------------------- P-3: invariants
+def _test_tensors():
+    rng = synth.make_rng(123)
+    return {
+        "normal": synth.normal(rng, (64, 256), 1.0),
+        "outlier": synth.outlier_normal(rng, 128, 512, 0.01, 50.0),
+        "weight": synth.normal(rng, (128, 256), 0.02),
+        "grad": synth.student_t_grad(rng, 64, 512),
+    }
+
+
+@pytest.mark.parametrize("block_rows", [1, 16])
+def test_invariants(block_rows):
+    for name, x in _test_tensors().items():
+        q = nvfp4.quantize_blockwise(x, block_rows=block_rows)
+        sf8, codes, scaled = q["sf"], q["codes"], np.abs(q["scaled"].astype(np.float64))
+        br = block_rows
+        sf_full = np.repeat(np.repeat(sf8, br, 0), 16, 1)
+        normal = sf_full >= 0x08
+        # (iv) scales are finite and the block holding amax_t gets 448
+        assert sf8.max() == 0x7E, name
+        r, c = np.unravel_index(np.argmax(np.abs(x)), x.shape)
+        assert sf8[r // br, c // 16] == 0x7E
+        # (iii) scaled magnitudes stay below 6.375 when the scale is normal
+        assert scaled[normal].max() <= 6.375, name
+        # (ii) half-ULP error of the E2M1 grid in units of the block scale
+        err = np.abs(scaled - nvfp4.E2M1_VALUES[codes & 7])
+        bound = np.where(scaled < 2, 0.25, np.where(scaled < 4, 0.5, 1.0))
+        assert np.all(err[normal] <= bound[normal]), name
+        # (i) block amax -> code 7 when the scale is normal
+        xb = np.abs(x).reshape(x.shape[0] // br, br, x.shape[1] // 16, 16)
+        amax_b = xb.max(axis=(1, 3))
+        cb = (codes & 7).reshape(xb.shape)
+        is_max = xb == amax_b[:, None, :, None]
+        blk_normal = (sf8 >= 0x08)[:, None, :, None] & is_max
+        assert np.all(cb[blk_normal] == 7), name
+        # (v) codes monotone in |x| within a block
+        order = np.argsort(xb.transpose(0, 2, 1, 3).reshape(-1, br * 16), axis=1)
+        cs = np.take_along_axis(cb.transpose(0, 2, 1, 3).reshape(-1, br * 16), order, axis=1)
+        assert np.all(np.diff(cs.astype(np.int64), axis=1) >= 0), name
+        # sign bit follows the input
+        assert np.array_equal((codes >> 3).astype(bool), np.signbit(x))
+        # dequant error relative to the block scale
+        dq = nvfp4.dequantize(q)
+        step = nvfp4.e4m3_decode(sf_full) * float(q["g_dec"])
+        assert np.all(np.abs(dq - x)[normal] <= (1.0 * step * 1.0001)[normal])
+
+
+def test_idempotent_on_representable_data():
+    """P-3 (vi): E2M1 values times one power of two per block, block amax 6*2^j,
+    and a caller-supplied amax_t = 2688 * 2^-J (so g_enc, sf and enc_b are all
+    powers of two) -> dequant(Q(x)) == x bit for bit.  (SURVEY.md's "amax_t =
+    6*2^J" does not give a power-of-two g_enc: 2688/(6*2^J) = 7*2^(6-J).)"""
+    rng = np.random.default_rng(7)
+    rows, cols = 32, 128
+    codes = rng.integers(0, 16, (rows, cols)).astype(np.uint8)
+    codes.reshape(rows, cols // 16, 16)[:, :, 0] = 7           # every block holds a 6
+    expo = rng.integers(-6, 3, (rows, cols // 16))
+    expo[0, 0] = 2                                              # largest block amax = 6 * 2^2 = 24
+    x = (nvfp4.e2m1_decode(codes) * np.repeat(np.exp2(expo), 16, 1)).astype(np.float32)
+    q = nvfp4.quantize_blockwise(x, amax_t=2688.0 / 64.0)       # g_enc = 64; block scales 2^(j+6) <= 256
+    assert q["g_enc"] == np.float32(64.0)
+    assert np.array_equal(nvfp4.dequantize(q).astype(np.float32).view(np.uint32), x.view(np.uint32))
+    assert np.array_equal(q["codes"] & 7, codes & 7)
+
+
+# --------------------------------------------------- P-4: transposition identity
+def test_transpose_identity_16x16():
+    rng = synth.make_rng(5)
+    R = synth.normal(rng, (64, 96), 0.02)
+    q = nvfp4.quantize_blockwise(R, block_rows=16)
+    qt = nvfp4.quantize_blockwise(np.ascontiguousarray(R.T), block_rows=16)
+    assert np.array_equal(qt["codes"], q["codes"].T)
+    assert np.array_equal(qt["sf"], q["sf"].T)
+    assert qt["g_dec"] == q["g_dec"]
+    # guard: the identity must FAIL for 1x16 blocks on random data
+    q1 = nvfp4.quantize_blockwise(R, block_rows=1)
+    q1t = nvfp4.quantize_blockwise(np.ascontiguousarray(R.T), block_rows=1)
+    assert not np.array_equal(q1t["codes"], q1["codes"].T)
+
+
+# ------------------------------------------------------------------ Q5: layouts
+def test_pack_unpack_and_tile_layout():
+    rng = np.random.default_rng(3)
+    codes = rng.integers(0, 16, (8, 64)).astype(np.uint8)
+    p = nvfp4.pack_codes(codes)
+    assert p[0, 0] == (codes[0, 0] | (codes[0, 1] << 4))
+    assert np.array_equal(nvfp4.unpack_codes(p), codes)
+    sf = rng.integers(1, 0x7F, (200, 12)).astype(np.uint8)
+    t = nvfp4.sf_to_tile128x4(sf)
+    assert t.size == 2 * 3 * 512
+    # independent restatement of the index: tile (r//128, c//4), 32x4x4 interleave
+    for r, c in [(0, 0), (1, 0), (31, 3), (32, 0), (127, 3), (128, 0), (199, 11), (5, 4), (130, 7)]:
+        tile = (r // 128) * 3 + c // 4
+        rr = r % 128
+        off = tile * 512 + (rr % 32) * 16 + (rr // 32) * 4 + c % 4
+        assert t[off] == sf[r, c]
+    assert np.count_nonzero(t) == sf.size      # permutation + zero padding
+
+
+# -------------------------------------------------- P-8: error-magnitude sanity
+def test_error_magnitudes():
+    rng = synth.make_rng(0)
+    x = synth.normal(rng, (256, 1024), 1.0)
+    rel = lambda q, x: np.linalg.norm(nvfp4.dequantize(q) - x) / np.linalg.norm(x)
+    e1 = rel(nvfp4.quantize_blockwise(x, 1), x)
+    e16 = rel(nvfp4.quantize_blockwise(x, 16), x)
+    assert 0.085 < e1 < 0.105 and 0.10 < e16 < 0.125 and e16 > e1
+    g = synth.student_t_grad(rng, 256, 1024)
+    eg = rel(nvfp4.quantize_blockwise(g, 1), g)
+    assert 0.07 < eg < 0.11
+    # without the tensor scale (amax_t = 2688 -> g_enc = 1) the gradients underflow E4M3:
+    # only subnormal block scales survive and most codes are zero (O-3)
+    q0 = nvfp4.quantize_blockwise(g, 1, amax_t=2688.0)
+    assert q0["sf"].max() < 0x08 and np.mean((q0["codes"] & 7) == 0) > 0.85
+    assert rel(q0, g) > 3 * eg
