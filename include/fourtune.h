@@ -1,0 +1,165 @@
+/* fourtune.h -- C ABI of the B200 (sm_100a) W4A4G4 triple-branch linear layer.
+ *
+ * The operation is the hot path of FourTune (arxiv 2607.05711); citations are
+ * lines of PAPER.md plus the section / equation they fall in, and readings
+ * Q1..Q5 / O-n of DESIGN.md where the paper is silent.
+ *
+ *   forward  (sec. 3.1, Eq. 2 recovered from Eq. 3):
+ *       Y  = GEMM4(Q(X), Q(R)) + X L1 L2 + X A B
+ *   dgrad    (sec. 3.2, Eq. 3):
+ *       dX = GEMM4(Q(G), Q(R)^T) + G L_stab^T + G (A B)^T
+ *   wgrad    (Eq. 4):   dB = (X A)^T G ,  dA = X^T (G B^T)
+ *   Q(.) is the NVFP4 block quantizer: E2M1 codes, one
+ *   E4M3 scale per block, one FP32 scale per tensor (Q1-Q5).
+ *
+ * Shapes:  X [M x K], G and Y [M x N], R [N x K].
+ * The two low-rank factors are stored "feature-major":
+ *       D_f = [L1 | A]        : [K x r_t]   (row k, r_t contiguous)
+ *       U_t = [L2 ; B]^T      : [N x r_t]   (row n, r_t contiguous)
+ * r_t = r_s + r; columns 0..r_s-1 are the frozen stabilizer, r_s..r_t-1 the
+ * trainable LoRA adapter.  With this storage forward and backward are the same
+ * kernels with (X, K, D_f, U_t) and (G, N, U_t, D_f) swapped.
+ *
+ * Conventions for EVERY call
+ *  - all data pointers are DEVICE pointers unless the comment says "host";
+ *    the structs themselves are host memory, read during the call only.
+ *  - the caller owns every buffer; the library never allocates, frees or keeps
+ *    a pointer after the call returns.  Scratch comes from `workspace`.
+ *  - `stream` is a cudaStream_t passed as void*; all work is enqueued on it and
+ *    the call returns without synchronising.  No device scalar is read by the
+ *    host (tensor scales stay on the device).
+ *  - return value: FT_OK or a negative ft_status; on error nothing (or only
+ *    part of the work) was enqueued.  Shapes are validated on the host before
+ *    the first launch.  Inputs must be finite (NaN/Inf: undefined results).
+ *  - bf16 matrices are row-major and dense (leading dimension = #columns),
+ *    16-byte aligned.
+ */
+#ifndef FOURTUNE_H_
+#define FOURTUNE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  FT_OK = 0,
+  FT_ERR_INVALID_ARG = -1,       /* NULL pointer, misaligned pointer, bad enum */
+  FT_ERR_UNSUPPORTED_SHAPE = -2, /* dimension not a multiple of the block / tile */
+  FT_ERR_WORKSPACE_TOO_SMALL = -3,
+  FT_ERR_CUDA = -4,              /* a CUDA runtime/driver call failed: see ft_last_cuda_error */
+  FT_ERR_ARCH = -5               /* device is not compute capability 10.x */
+} ft_status;
+
+/* scale-factor layouts (Q5) */
+#define FT_SF_ROWMAJOR 0  /* sf[row / block_rows][col / 16], dense                          */
+#define FT_SF_TILE128x4 1 /* per-row scales in 512-byte tiles of 128 rows x 4 blocks, the
+                             layout tcgen05.cp moves to tensor memory unchanged:
+                             off(r, c) = ((r/128) * ceil(nblk/4) + c/4) * 512
+                                         + (r%32)*16 + ((r%128)/32)*4 + c%4
+                             rows padded to 128, blocks to 4 (padding bytes are 0).  With
+                             block_rows = 16 row r carries the scale of block r/16.      */
+
+#define FT_ROUND_NEAREST_EVEN 0 /* the only mode of the paper's reading O-6 */
+
+/* A quantized tensor Q(T) of a logical [rows x cols] matrix, blocked along cols. */
+typedef struct {
+  uint8_t* codes;          /* [rows x cols/2]; byte j of a row = element 2j in bits 0-3,
+                              element 2j+1 in bits 4-7 (Q5); E2M1, bit 3 = sign (Q1)   */
+  uint8_t* sf;             /* E4M3 block scales (Q2), ft_sf_bytes() bytes, layout below  */
+  float* tensor_dec_scale; /* one float: g_dec = 1 / (2688 / amax_t)  (Q3)               */
+  int64_t rows, cols;
+  int32_t block_rows;      /* 1 (activations, gradients) or 16 (weights, 16x16 blocks)  */
+  int32_t sf_layout;       /* FT_SF_ROWMAJOR or FT_SF_TILE128x4                          */
+} ft_qtensor;
+
+/* Optional low-rank down-projection fused into the quantize pass (PAPER.md:110,
+ * "fuse ... quantization and down-projection"):  H = X * down  (fp32 accumulate). */
+typedef struct {
+  const void* down;          /* bf16 [cols x r_t]                                        */
+  void* out;                 /* bf16 [rows x r_t] = bf16(H); may be NULL                 */
+  void* out_scaled;          /* bf16 [rows x r_t] = bf16(H / alpha), alpha = g_dec(this
+                                tensor) * *other_dec_scale (O-10'); may be NULL */
+  const float* other_dec_scale; /* g_dec of the operand this tensor will meet in GEMM4;
+                                required iff out_scaled != NULL                          */
+  int32_t r_t;               /* 16..128, multiple of 16                                  */
+} ft_proj;
+
+/* Frozen parts of one layer plus the current adapter. */
+typedef struct {
+  ft_qtensor r_kmajor; /* Q(R)   as [N x K], 16x16 blocks, sf TILE128x4 (forward operand) */
+  ft_qtensor r_nmajor; /* Q(R)^T as [K x N]: the SAME codes and scales re-packed
+                          (PAPER.md:102), sf TILE128x4 (dgrad operand)                    */
+  const void* D_f;     /* bf16 [K x r_t] = [L1 | A]                                       */
+  const void* U_t;     /* bf16 [N x r_t] = [L2 ; B]^T                                     */
+  int64_t K, N;
+  int32_t r_s, r;      /* r_t = r_s + r: 0, or a multiple of 16 up to 128                 */
+} ft_layer;
+
+/* ---- a0: tensor amax (Q3).  *amax_out = max |x_i| over n bf16 values. */
+int ft_tensor_amax(const void* x_bf16, int64_t n, float* amax_out, void* stream);
+
+/* ---- a1/a3/a6: Q(.) of DESIGN.md Q3-Q5 (+ optional fused down-projection).
+ * x_bf16 [rows x cols]; blocks are out->block_rows x 16 along cols.
+ * tensor_amax: device float holding amax_t; NULL => the library computes it first
+ *   (one extra pass over x) into the workspace.
+ * proj: NULL => quantize only.  Requires out->block_rows == 1 if non-NULL.
+ * Requirements: cols % 64 == 0; rows % 16 == 0 if block_rows == 16; any rows >= 1
+ *   otherwise.  out->rows/cols must equal rows/cols.  round_mode must be
+ *   FT_ROUND_NEAREST_EVEN.  workspace >= ft_workspace_bytes(rows, cols, 0, r_t). */
+int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols,
+                          const float* tensor_amax, const ft_proj* proj,
+                          ft_qtensor* out, int32_t round_mode,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- a6 helper: build Q(R)^T ([K x N], N contiguous) from Q(R) ([N x K]) by
+ * moving nibbles and scales; nothing is re-quantized.
+ * r_kmajor: block_rows 16, sf_layout FT_SF_ROWMAJOR (S[N/16][K/16]).
+ * Outputs: r_nmajor (codes [K x N/2], sf TILE128x4 over K rows, same tensor scale
+ * value copied), and, if r_kmajor_tiled != NULL, the TILE128x4 expansion of the
+ * forward operand's scales (its codes/tensor_dec_scale pointers are not written;
+ * point them at r_kmajor's buffers). N % 64 == 0 and K % 64 == 0. */
+int ft_pack_weight(const ft_qtensor* r_kmajor, ft_qtensor* r_kmajor_tiled,
+                   ft_qtensor* r_nmajor, void* stream);
+
+/* ---- a0+a1+a2: forward.  x_bf16 [M x K] -> y_bf16 [M x N].
+ * h_saved_bf16 [M x r_t] receives bf16(X D_f) (columns r_s.. are X A, reused by
+ * ft_lora_wgrad); ignored if r_t == 0.
+ * qx_scratch: caller-allocated Q(X) buffers (codes M*K/2 bytes, sf
+ *   ft_sf_bytes(M, K, FT_SF_TILE128x4), tensor_dec_scale 1 float); filled here,
+ *   rows/cols/block_rows/sf_layout are set by the call.
+ * Requirements: K % 64 == 0, N % 64 == 0, M >= 1. */
+int ft_linear_fwd(const ft_layer* L, const void* x_bf16, int64_t M, void* y_bf16,
+                  void* h_saved_bf16, ft_qtensor* qx_scratch, void* workspace,
+                  size_t workspace_bytes, void* stream);
+
+/* ---- a0+a3+a4: input gradient.  g_bf16 [M x N] -> dx_bf16 [M x K].
+ * p_saved_bf16 [M x r_t] receives bf16(G U_t) (columns r_s.. are G B^T). */
+int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* dx_bf16,
+                        void* p_saved_bf16, ft_qtensor* qg_scratch, void* workspace,
+                        size_t workspace_bytes, void* stream);
+
+/* ---- a5: LoRA weight gradients (Eq. 4), fp32.
+ * dA  [K x r]  = X^T  * P[:, r_s:]      dBt [N x r] = G^T * H[:, r_s:]  (= dB^T)
+ * h_saved / p_saved are the [M x r_t] outputs of the two calls above.
+ * accumulate: 0 overwrite, 1 add to the existing contents.  Sums over M are
+ * accumulated with fp32 atomics: the order of additions is not fixed. */
+int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
+                  const void* h_saved_bf16, const void* p_saved_bf16, float* dA,
+                  float* dBt, int32_t accumulate, void* stream);
+
+/* ---- sizes and diagnostics (host only, no CUDA calls) */
+size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout);
+size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t);
+const char* ft_error_string(int status);
+int ft_last_cuda_error(void); /* cudaError_t / CUresult of the last FT_ERR_CUDA, thread-local */
+int ft_version(void);
+/* test / bench hook: force the N-tile of the 4-bit GEMM (128, 192, 256; 0 = library default) */
+int ft_debug_set_gemm_tile_n(int bn);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FOURTUNE_H_ */

@@ -1,0 +1,197 @@
+"""Thin Python binding of include/fourtune.h: argument marshalling only.  Every step of
+the hot path runs in the CUDA kernels of libfourtune.so; PyTorch supplies device memory and
+the stream.  There is no CPU fallback: a missing library raises at import of the symbols.
+
+Function names and argument order follow the C header.  Tensors are torch CUDA tensors;
+`QTensor` / `Layer` mirror ft_qtensor / ft_layer.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfourtune.so")
+
+FT_SF_ROWMAJOR, FT_SF_TILE128x4 = 0, 1
+FT_ROUND_NEAREST_EVEN = 0
+
+
+class FtError(RuntimeError):
+    pass
+
+
+class _QT(C.Structure):
+    _fields_ = [("codes", C.c_void_p), ("sf", C.c_void_p), ("tensor_dec_scale", C.c_void_p),
+                ("rows", C.c_int64), ("cols", C.c_int64), ("block_rows", C.c_int32), ("sf_layout", C.c_int32)]
+
+
+class _Proj(C.Structure):
+    _fields_ = [("down", C.c_void_p), ("out", C.c_void_p), ("out_scaled", C.c_void_p),
+                ("other_dec_scale", C.c_void_p), ("r_t", C.c_int32)]
+
+
+class _Layer(C.Structure):
+    _fields_ = [("r_kmajor", _QT), ("r_nmajor", _QT), ("D_f", C.c_void_p), ("U_t", C.c_void_p),
+                ("K", C.c_int64), ("N", C.c_int64), ("r_s", C.c_int32), ("r", C.c_int32)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libfourtune.so (building it is `python -m paper_2607_05711_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FtError("libfourtune.so not built: run `python -m paper_2607_05711_b200.build` "
+                          "(there is no fallback path)")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, i32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_size_t
+        L.ft_tensor_amax.argtypes = [vp, i64, vp, vp]
+        L.ft_quantize_blockwise.argtypes = [vp, i64, i64, vp, C.POINTER(_Proj), C.POINTER(_QT), i32, vp, sz, vp]
+        L.ft_pack_weight.argtypes = [C.POINTER(_QT), C.POINTER(_QT), C.POINTER(_QT), vp]
+        L.ft_linear_fwd.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
+        L.ft_linear_bwd_dgrad.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
+        L.ft_lora_wgrad.argtypes = [C.POINTER(_Layer), vp, vp, i64, vp, vp, vp, vp, i32, vp]
+        L.ft_sf_bytes.argtypes = [i64, i64, i32, i32]
+        L.ft_sf_bytes.restype = sz
+        L.ft_workspace_bytes.argtypes = [i64, i64, i64, i32]
+        L.ft_workspace_bytes.restype = sz
+        L.ft_error_string.argtypes = [C.c_int]
+        L.ft_error_string.restype = C.c_char_p
+        L.ft_debug_set_gemm_tile_n.argtypes = [C.c_int]
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != 0:
+        L = lib()
+        raise FtError("fourtune: %s (status %d, cuda error %d)" %
+                      (L.ft_error_string(rc).decode(), rc, L.ft_last_cuda_error()))
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _bf16(t):
+    assert t.is_cuda and t.dtype == torch.bfloat16 and t.is_contiguous(), "need contiguous CUDA bf16"
+    return t
+
+
+def ft_sf_bytes(rows, cols, block_rows, layout):
+    return lib().ft_sf_bytes(rows, cols, block_rows, layout)
+
+
+def ft_workspace_bytes(M, K, N, r_t):
+    return lib().ft_workspace_bytes(M, K, N, r_t)
+
+
+class QTensor:
+    """ft_qtensor with its buffers owned by torch."""
+
+    def __init__(self, rows, cols, block_rows=1, sf_layout=FT_SF_TILE128x4, device="cuda"):
+        self.rows, self.cols, self.block_rows, self.sf_layout = rows, cols, block_rows, sf_layout
+        self.codes = torch.empty((rows, cols // 2), dtype=torch.uint8, device=device)
+        self.sf = torch.zeros(ft_sf_bytes(rows, cols, block_rows, sf_layout), dtype=torch.uint8, device=device)
+        self.tensor_dec_scale = torch.zeros(1, dtype=torch.float32, device=device)
+
+    def c(self):
+        return _QT(self.codes.data_ptr(), self.sf.data_ptr(), self.tensor_dec_scale.data_ptr(),
+                   self.rows, self.cols, self.block_rows, self.sf_layout)
+
+    def sync_from(self, q):
+        self.rows, self.cols, self.block_rows, self.sf_layout = q.rows, q.cols, q.block_rows, q.sf_layout
+
+
+def ft_tensor_amax(x, out=None, stream=None):
+    _bf16(x)
+    out = torch.empty(1, dtype=torch.float32, device=x.device) if out is None else out
+    _check(lib().ft_tensor_amax(_ptr(x), x.numel(), _ptr(out), _stream(stream)))
+    return out
+
+
+def ft_quantize_blockwise(x, out, tensor_amax=None, down=None, h_out=None, hs_out=None,
+                          other_dec_scale=None, workspace=None, stream=None):
+    """x [rows x cols] bf16 -> out (QTensor).  down [cols x r_t] enables the fused projection."""
+    _bf16(x)
+    rows, cols = x.shape
+    if workspace is None:
+        workspace = torch.empty(ft_workspace_bytes(rows, cols, 0, 0 if down is None else down.shape[1]),
+                                dtype=torch.uint8, device=x.device)
+    proj = None
+    if down is not None:
+        _bf16(down)
+        proj = _Proj(down.data_ptr(), None if h_out is None else h_out.data_ptr(),
+                     None if hs_out is None else hs_out.data_ptr(),
+                     None if other_dec_scale is None else other_dec_scale.data_ptr(), down.shape[1])
+    q = out.c()
+    _check(lib().ft_quantize_blockwise(_ptr(x), rows, cols, _ptr(tensor_amax),
+                                       None if proj is None else C.byref(proj), C.byref(q),
+                                       FT_ROUND_NEAREST_EVEN, _ptr(workspace), workspace.numel(),
+                                       _stream(stream)))
+    return out
+
+
+class Layer:
+    """ft_layer: Q(R) in both orientations plus the low-rank factors D_f [K x r_t], U_t [N x r_t]."""
+
+    def __init__(self, R_bf16, D_f, U_t, r_s, r, stream=None):
+        _bf16(R_bf16)
+        N, K = R_bf16.shape
+        self.N, self.K, self.r_s, self.r = N, K, r_s, r
+        self.D_f, self.U_t = D_f, U_t
+        if r_s + r > 0:
+            _bf16(D_f), _bf16(U_t)
+            assert D_f.shape == (K, r_s + r) and U_t.shape == (N, r_s + r)
+        dev = R_bf16.device
+        # a6: offline quantize (16x16 blocks, row-major S) then re-pack both orientations
+        self.q_rowmajor = QTensor(N, K, 16, FT_SF_ROWMAJOR, dev)
+        ft_quantize_blockwise(R_bf16, self.q_rowmajor, stream=stream)
+        self.r_kmajor = QTensor(N, K, 16, FT_SF_TILE128x4, dev)
+        self.r_kmajor.codes = self.q_rowmajor.codes
+        self.r_kmajor.tensor_dec_scale = self.q_rowmajor.tensor_dec_scale
+        self.r_nmajor = QTensor(K, N, 16, FT_SF_TILE128x4, dev)
+        qk, qkt, qn = self.q_rowmajor.c(), self.r_kmajor.c(), self.r_nmajor.c()
+        _check(lib().ft_pack_weight(C.byref(qk), C.byref(qkt), C.byref(qn), _stream(stream)))
+
+    def c(self):
+        return _Layer(self.r_kmajor.c(), self.r_nmajor.c(),
+                      None if self.D_f is None else self.D_f.data_ptr(),
+                      None if self.U_t is None else self.U_t.data_ptr(), self.K, self.N, self.r_s, self.r)
+
+
+def ft_linear_fwd(layer, x, y, h_saved, qx, workspace, stream=None):
+    _bf16(x)
+    L, q = layer.c(), qx.c()
+    _check(lib().ft_linear_fwd(C.byref(L), _ptr(x), x.shape[0], _ptr(y), _ptr(h_saved), C.byref(q),
+                               _ptr(workspace), workspace.numel(), _stream(stream)))
+    qx.sync_from(q)
+    return y
+
+
+def ft_linear_bwd_dgrad(layer, g, dx, p_saved, qg, workspace, stream=None):
+    _bf16(g)
+    L, q = layer.c(), qg.c()
+    _check(lib().ft_linear_bwd_dgrad(C.byref(L), _ptr(g), g.shape[0], _ptr(dx), _ptr(p_saved), C.byref(q),
+                                     _ptr(workspace), workspace.numel(), _stream(stream)))
+    qg.sync_from(q)
+    return dx
+
+
+def ft_lora_wgrad(layer, x, g, h_saved, p_saved, dA, dBt, accumulate=False, stream=None):
+    L = layer.c()
+    _check(lib().ft_lora_wgrad(C.byref(L), _ptr(x), _ptr(g), x.shape[0], _ptr(h_saved), _ptr(p_saved),
+                               _ptr(dA), _ptr(dBt), 1 if accumulate else 0, _stream(stream)))
+    return dA, dBt
+
+
+def debug_set_gemm_tile_n(bn):
+    _check(lib().ft_debug_set_gemm_tile_n(bn))

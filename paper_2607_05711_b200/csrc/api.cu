@@ -1,0 +1,283 @@
+// api.cu -- the extern "C" boundary of include/fourtune.h: host-side validation,
+// tensor-map construction and kernel sequencing.  No computation happens here.
+#include <cstring>
+
+#include "common.cuh"
+
+namespace ft {
+
+thread_local int g_last_cuda_error = 0;
+
+// kernels' host launchers (quantize.cu, quantize_fused.cu, gemm.cu, wgrad.cu)
+int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st);
+int launch_quantize_generic(const void* x, int64_t rows, int64_t cols, const float* amax_t,
+                            ft_qtensor* out, cudaStream_t st);
+int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t,
+                          const ft_proj* proj, ft_qtensor* out, cudaStream_t st);
+int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, cudaStream_t st);
+int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
+                 const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16,
+                 cudaStream_t st);
+int launch_wgrad(const void* in_bf16, int64_t M, int64_t F, const void* lr_bf16, int r_t, int r_s,
+                 int r, float* out, cudaStream_t st);
+
+// ------------------------------------------------------------- device queries
+static int g_sm_count = 0;
+int sm_count() {
+  if (g_sm_count == 0) {
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+      g_sm_count = n;
+    else
+      return 148;
+  }
+  return g_sm_count;
+}
+
+int device_check() {
+  int dev = 0, major = 0;
+  FT_CUDA_TRY(cudaGetDevice(&dev));
+  FT_CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  return major == 10 ? FT_OK : FT_ERR_ARCH;
+}
+
+// ---------------------------------------------------------------- tensor maps
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                    const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                    const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static PFN_encodeTiled g_encode = nullptr;
+
+int make_tensor_map_2d(CUtensorMap* map, const void* base, int elem_bytes, uint64_t inner,
+                       uint64_t outer, uint64_t row_pitch_bytes, uint32_t box_inner,
+                       uint32_t box_outer, Swizzle sw) {
+  if (g_encode == nullptr) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    FT_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (fn == nullptr || qres != cudaDriverEntryPointSuccess) {
+      g_last_cuda_error = (int)cudaErrorNotSupported;
+      return FT_ERR_CUDA;
+    }
+    g_encode = reinterpret_cast<PFN_encodeTiled>(fn);
+  }
+  const cuuint64_t dims[2] = {inner, outer};
+  const cuuint64_t strides[1] = {row_pitch_bytes};
+  const cuuint32_t box[2] = {box_inner, box_outer};
+  const cuuint32_t estr[2] = {1, 1};
+  CUtensorMapSwizzle s = CU_TENSOR_MAP_SWIZZLE_NONE;
+  if (sw == Swizzle::B32) s = CU_TENSOR_MAP_SWIZZLE_32B;
+  if (sw == Swizzle::B64) s = CU_TENSOR_MAP_SWIZZLE_64B;
+  if (sw == Swizzle::B128) s = CU_TENSOR_MAP_SWIZZLE_128B;
+  const CUtensorMapDataType dt =
+      elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8;
+  const CUresult r = g_encode(map, dt, 2, const_cast<void*>(base), dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, s, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    g_last_cuda_error = (int)r;
+    return FT_ERR_CUDA;
+  }
+  return FT_OK;
+}
+
+static bool valid_rt(int r_t) { return r_t >= 0 && r_t <= 128 && r_t % 16 == 0; }
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+constexpr size_t WS_HS_OFFSET = 256;  // [0,4): tensor amax; [256, ..): pre-scaled H / P
+
+// one direction of the layer: quantize `act` [M x Kd] (+ projection by lr_down
+// [Kd x r_t]) and multiply with the weight operand `w` ([Nd x Kd]); lr_up [Nd x r_t].
+static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_up, int r_t,
+                       const void* act, int64_t M, int64_t Kd, int64_t Nd, void* out,
+                       void* saved, ft_qtensor* q, void* workspace, size_t ws_bytes,
+                       cudaStream_t st) {
+  if (!act || !out || !q || !q->codes || !q->sf || !q->tensor_dec_scale || !workspace)
+    return FT_ERR_INVALID_ARG;
+  if (r_t > 0 && (!saved || !lr_down || !lr_up)) return FT_ERR_INVALID_ARG;
+  if (M < 1 || Kd % 64 != 0 || Nd % 64 != 0 || Kd < 64 || Nd < 64) return FT_ERR_UNSUPPORTED_SHAPE;
+  if (!aligned16(act) || !aligned16(out) || !aligned16(q->codes) || !aligned16(q->sf) ||
+      !aligned16(workspace) || (r_t > 0 && (!aligned16(saved) || !aligned16(lr_down) || !aligned16(lr_up))))
+    return FT_ERR_INVALID_ARG;
+  if (ws_bytes < ft_workspace_bytes(M, Kd, Nd, r_t)) return FT_ERR_WORKSPACE_TOO_SMALL;
+  int rc = device_check();
+  if (rc != FT_OK) return rc;
+  float* amax = reinterpret_cast<float*>(workspace);
+  void* hs = reinterpret_cast<uint8_t*>(workspace) + WS_HS_OFFSET;
+  q->rows = M;
+  q->cols = Kd;
+  q->block_rows = 1;
+  q->sf_layout = FT_SF_TILE128x4;
+  rc = launch_amax(act, M * Kd, amax, st);
+  if (rc != FT_OK) return rc;
+  ft_proj pr;
+  pr.down = lr_down;
+  pr.out = saved;
+  pr.out_scaled = hs;
+  pr.other_dec_scale = w->tensor_dec_scale;
+  pr.r_t = r_t;
+  rc = launch_quantize_fused(act, M, Kd, amax, r_t > 0 ? &pr : nullptr, q, st);
+  if (rc != FT_OK) return rc;
+  return launch_gemm4(q, w, M, Nd, Kd, r_t > 0 ? hs : nullptr, lr_up, r_t, out, st);
+}
+
+static int check_layer(const ft_layer* L) {
+  if (!L) return FT_ERR_INVALID_ARG;
+  if (L->r_s < 0 || L->r < 0 || !valid_rt(L->r_s + L->r)) return FT_ERR_UNSUPPORTED_SHAPE;
+  if (L->K % 64 != 0 || L->N % 64 != 0) return FT_ERR_UNSUPPORTED_SHAPE;
+  const ft_qtensor* ws[2] = {&L->r_kmajor, &L->r_nmajor};
+  for (int i = 0; i < 2; ++i) {
+    if (!ws[i]->codes || !ws[i]->sf || !ws[i]->tensor_dec_scale) return FT_ERR_INVALID_ARG;
+    if (ws[i]->sf_layout != FT_SF_TILE128x4) return FT_ERR_INVALID_ARG;
+    if (!aligned16(ws[i]->codes) || !aligned16(ws[i]->sf)) return FT_ERR_INVALID_ARG;
+  }
+  if (L->r_kmajor.rows != L->N || L->r_kmajor.cols != L->K || L->r_nmajor.rows != L->K ||
+      L->r_nmajor.cols != L->N)
+    return FT_ERR_INVALID_ARG;
+  return FT_OK;
+}
+
+}  // namespace ft
+
+using namespace ft;
+
+extern "C" {
+
+int ft_version(void) { return 100; }
+
+const char* ft_error_string(int status) {
+  switch (status) {
+    case FT_OK: return "ok";
+    case FT_ERR_INVALID_ARG: return "invalid argument";
+    case FT_ERR_UNSUPPORTED_SHAPE: return "unsupported shape";
+    case FT_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case FT_ERR_CUDA: return "CUDA error (see ft_last_cuda_error)";
+    case FT_ERR_ARCH: return "device is not sm_100";
+    default: return "unknown status";
+  }
+}
+
+int ft_last_cuda_error(void) { return g_last_cuda_error; }
+
+size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout) {
+  if (rows <= 0 || cols <= 0 || block_rows <= 0) return 0;
+  const int64_t nblk = ceil_div(cols, 16);
+  if (layout == FT_SF_TILE128x4) return (size_t)(ceil_div(rows, 128) * ceil_div(nblk, 4) * 512);
+  return (size_t)(ceil_div(rows, block_rows) * nblk);
+}
+
+size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t) {
+  (void)K;
+  (void)N;
+  if (M < 0 || r_t < 0) return 0;
+  return WS_HS_OFFSET + align_up((size_t)M * (size_t)r_t * 2, 256) + 256;
+}
+
+int ft_tensor_amax(const void* x_bf16, int64_t n, float* amax_out, void* stream) {
+  if (!x_bf16 || !amax_out || n < 0 || !aligned16(x_bf16)) return FT_ERR_INVALID_ARG;
+  return launch_amax(x_bf16, n, amax_out, (cudaStream_t)stream);
+}
+
+int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols, const float* tensor_amax,
+                          const ft_proj* proj, ft_qtensor* out, int32_t round_mode,
+                          void* workspace, size_t workspace_bytes, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!x_bf16 || !out || !out->codes || !out->sf || !out->tensor_dec_scale) return FT_ERR_INVALID_ARG;
+  if (round_mode != FT_ROUND_NEAREST_EVEN) return FT_ERR_INVALID_ARG;
+  if (out->block_rows != 1 && out->block_rows != 16) return FT_ERR_INVALID_ARG;
+  if (out->sf_layout != FT_SF_ROWMAJOR && out->sf_layout != FT_SF_TILE128x4) return FT_ERR_INVALID_ARG;
+  if (out->rows != rows || out->cols != cols) return FT_ERR_INVALID_ARG;
+  if (rows < 1 || cols < 64 || cols % 64 != 0) return FT_ERR_UNSUPPORTED_SHAPE;
+  if (out->block_rows == 16 && rows % 16 != 0) return FT_ERR_UNSUPPORTED_SHAPE;
+  if (!aligned16(x_bf16) || !aligned16(out->codes) || (reinterpret_cast<uintptr_t>(out->sf) & 3))
+    return FT_ERR_INVALID_ARG;
+  int r_t = 0;
+  if (proj) {
+    r_t = proj->r_t;
+    if (out->block_rows != 1) return FT_ERR_INVALID_ARG;
+    if (!valid_rt(r_t) || r_t == 0) return FT_ERR_UNSUPPORTED_SHAPE;
+    if (!proj->down || !aligned16(proj->down)) return FT_ERR_INVALID_ARG;
+    if (proj->out && !aligned16(proj->out)) return FT_ERR_INVALID_ARG;
+    if (proj->out_scaled && (!aligned16(proj->out_scaled) || !proj->other_dec_scale))
+      return FT_ERR_INVALID_ARG;
+  }
+  int rc = device_check();
+  if (rc != FT_OK) return rc;
+  const float* amax = tensor_amax;
+  if (!amax) {
+    if (!workspace || !aligned16(workspace)) return FT_ERR_INVALID_ARG;
+    if (workspace_bytes < ft_workspace_bytes(rows, cols, 0, r_t)) return FT_ERR_WORKSPACE_TOO_SMALL;
+    rc = launch_amax(x_bf16, rows * cols, reinterpret_cast<float*>(workspace), st);
+    if (rc != FT_OK) return rc;
+    amax = reinterpret_cast<const float*>(workspace);
+  }
+  if (out->block_rows == 16) return launch_quantize_generic(x_bf16, rows, cols, amax, out, st);
+  return launch_quantize_fused(x_bf16, rows, cols, amax, proj, out, st);
+}
+
+int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, void* stream) {
+  if (!rk || !rn || !rk->codes || !rk->sf || !rk->tensor_dec_scale || !rn->codes || !rn->sf ||
+      !rn->tensor_dec_scale)
+    return FT_ERR_INVALID_ARG;
+  if (rk->block_rows != 16 || rk->sf_layout != FT_SF_ROWMAJOR) return FT_ERR_INVALID_ARG;
+  if (rk_tiled && !rk_tiled->sf) return FT_ERR_INVALID_ARG;
+  if (rk->rows % 64 != 0 || rk->cols % 64 != 0 || rk->rows < 64 || rk->cols < 64)
+    return FT_ERR_UNSUPPORTED_SHAPE;
+  int rc = device_check();
+  if (rc != FT_OK) return rc;
+  rn->rows = rk->cols;
+  rn->cols = rk->rows;
+  rn->block_rows = 16;
+  rn->sf_layout = FT_SF_TILE128x4;
+  if (rk_tiled) {
+    rk_tiled->rows = rk->rows;
+    rk_tiled->cols = rk->cols;
+    rk_tiled->block_rows = 16;
+    rk_tiled->sf_layout = FT_SF_TILE128x4;
+  }
+  return launch_pack_weight(rk, rk_tiled, rn, (cudaStream_t)stream);
+}
+
+int ft_linear_fwd(const ft_layer* L, const void* x_bf16, int64_t M, void* y_bf16,
+                  void* h_saved_bf16, ft_qtensor* qx_scratch, void* workspace,
+                  size_t workspace_bytes, void* stream) {
+  int rc = check_layer(L);
+  if (rc != FT_OK) return rc;
+  return linear_pass(&L->r_kmajor, L->D_f, L->U_t, L->r_s + L->r, x_bf16, M, L->K, L->N, y_bf16,
+                     h_saved_bf16, qx_scratch, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* dx_bf16,
+                        void* p_saved_bf16, ft_qtensor* qg_scratch, void* workspace,
+                        size_t workspace_bytes, void* stream) {
+  int rc = check_layer(L);
+  if (rc != FT_OK) return rc;
+  return linear_pass(&L->r_nmajor, L->U_t, L->D_f, L->r_s + L->r, g_bf16, M, L->N, L->K, dx_bf16,
+                     p_saved_bf16, qg_scratch, workspace, workspace_bytes, (cudaStream_t)stream);
+}
+
+int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
+                  const void* h_saved_bf16, const void* p_saved_bf16, float* dA, float* dBt,
+                  int32_t accumulate, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!L || !x_bf16 || !g_bf16 || !h_saved_bf16 || !p_saved_bf16 || !dA || !dBt)
+    return FT_ERR_INVALID_ARG;
+  const int r_t = L->r_s + L->r;
+  if (L->r_s < 0 || L->r <= 0 || !valid_rt(r_t) || L->r % 8 != 0 || L->r_s % 8 != 0)
+    return FT_ERR_UNSUPPORTED_SHAPE;
+  if (M < 1 || L->K % 64 != 0 || L->N % 64 != 0) return FT_ERR_UNSUPPORTED_SHAPE;
+  if (!aligned16(x_bf16) || !aligned16(g_bf16) || !aligned16(h_saved_bf16) ||
+      !aligned16(p_saved_bf16) || !aligned16(dA) || !aligned16(dBt))
+    return FT_ERR_INVALID_ARG;
+  int rc = device_check();
+  if (rc != FT_OK) return rc;
+  if (!accumulate) {
+    FT_CUDA_TRY(cudaMemsetAsync(dA, 0, (size_t)L->K * L->r * sizeof(float), st));
+    FT_CUDA_TRY(cudaMemsetAsync(dBt, 0, (size_t)L->N * L->r * sizeof(float), st));
+  }
+  rc = launch_wgrad(x_bf16, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA, st);
+  if (rc != FT_OK) return rc;
+  return launch_wgrad(g_bf16, M, L->N, h_saved_bf16, r_t, L->r_s, L->r, dBt, st);
+}
+
+}  // extern "C"

@@ -1,0 +1,190 @@
+// quantize.cu -- a0 (tensor amax), a6 (offline weight quantize + pack) and the
+// generic block quantizer.  The hot fused quantize + down-projection kernel (a1/a3)
+// is in quantize_fused.cu.
+#include "common.cuh"
+#include "quant_math.cuh"
+
+namespace ft {
+
+// ------------------------------------------------------------------ a0: amax
+// max |x| of n bf16 values.  |x| of a finite bf16 orders like its low 15 bits, so
+// the reduction runs on integers and atomicMax on the float's bit pattern is exact.
+__global__ void __launch_bounds__(256) k_amax(const uint4* __restrict__ x, int64_t n_vec,
+                                              const uint16_t* __restrict__ tail, int n_tail,
+                                              unsigned int* __restrict__ out_bits) {
+  const uint32_t m = 0x7FFF7FFFu;
+  uint32_t acc = 0;  // two 15-bit maxima packed; compared per half with vmax
+  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  // 4 independent 16-byte loads in flight per thread
+  for (; i + 3 * stride < n_vec; i += 4 * stride) {
+    uint4 v0 = __ldg(x + i), v1 = __ldg(x + i + stride), v2 = __ldg(x + i + 2 * stride),
+          v3 = __ldg(x + i + 3 * stride);
+    uint32_t a = __vmaxu2(__vmaxu2(v0.x & m, v0.y & m), __vmaxu2(v0.z & m, v0.w & m));
+    uint32_t b = __vmaxu2(__vmaxu2(v1.x & m, v1.y & m), __vmaxu2(v1.z & m, v1.w & m));
+    uint32_t c = __vmaxu2(__vmaxu2(v2.x & m, v2.y & m), __vmaxu2(v2.z & m, v2.w & m));
+    uint32_t d = __vmaxu2(__vmaxu2(v3.x & m, v3.y & m), __vmaxu2(v3.z & m, v3.w & m));
+    acc = __vmaxu2(acc, __vmaxu2(__vmaxu2(a, b), __vmaxu2(c, d)));
+  }
+  for (; i < n_vec; i += stride) {
+    uint4 v = __ldg(x + i);
+    acc = __vmaxu2(acc, __vmaxu2(__vmaxu2(v.x & m, v.y & m), __vmaxu2(v.z & m, v.w & m)));
+  }
+  if (blockIdx.x == 0 && threadIdx.x < n_tail) acc = __vmaxu2(acc, (uint32_t)(tail[threadIdx.x] & 0x7FFF));
+  uint32_t best = max(acc & 0xFFFFu, acc >> 16);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(0xffffffffu, best, o));
+  __shared__ uint32_t s_best[8];
+  if ((threadIdx.x & 31) == 0) s_best[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) best = max(best, s_best[w]);
+    atomicMax(out_bits, best << 16);  // bf16 bits -> float bits; non-negative floats order as uints
+  }
+}
+
+int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st) {
+  FT_CUDA_TRY(cudaMemsetAsync(amax_out, 0, sizeof(float), st));
+  if (n == 0) return FT_OK;
+  const int64_t n_vec = n / 8;
+  const int n_tail = (int)(n % 8);
+  int64_t blocks = ceil_div(n_vec, 256 * 4);
+  const int64_t cap = (int64_t)sm_count() * 8;
+  if (blocks > cap) blocks = cap;
+  if (blocks < 1) blocks = 1;
+  k_amax<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<const uint4*>(x_bf16), n_vec,
+                                           reinterpret_cast<const uint16_t*>(x_bf16) + n_vec * 8,
+                                           n_tail, reinterpret_cast<unsigned int*>(amax_out));
+  FT_CUDA_TRY(cudaGetLastError());
+  return FT_OK;
+}
+
+// ------------------------------------------- generic quantizer (a6, offline path)
+// One thread per 16-element row segment.  BR = 16: the 16 lanes of a half-warp own
+// the 16 rows of one 16x16 block and share its amax by shuffles.  BR = 1: 1x16 blocks.
+template <int BR>
+__global__ void __launch_bounds__(256) k_quantize_generic(
+    const uint4* __restrict__ x, int64_t rows, int64_t cols, const float* __restrict__ amax_t,
+    uint8_t* __restrict__ codes, uint8_t* __restrict__ sf, float* __restrict__ g_dec_out,
+    int sf_layout) {
+  const int64_t nblk = cols / 16;
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const TensorScale ts = tensor_scale(*amax_t);
+  if (t == 0) *g_dec_out = ts.g_dec;
+  int64_t row, bc;
+  if (BR == 16) {
+    const int64_t i = t % 16, blk = t / 16;
+    bc = blk % nblk;
+    row = (blk / nblk) * 16 + i;
+  } else {
+    bc = t % nblk;
+    row = t / nblk;
+  }
+  const bool live = row < rows;  // rows % BR == 0, so a half-warp is live or dead as a whole
+  uint4 v0 = make_uint4(0, 0, 0, 0), v1 = v0;
+  if (live) {
+    const uint4* p = x + (row * cols + bc * 16) / 8;
+    v0 = __ldg(p);
+    v1 = __ldg(p + 1);
+  }
+  float amax_b = fmaxf(amax_bf16x8(v0), amax_bf16x8(v1));
+  if (BR == 16) {
+#pragma unroll
+    for (int o = 8; o > 0; o >>= 1) amax_b = fmaxf(amax_b, __shfl_xor_sync(0xffffffffu, amax_b, o));
+  }
+  uint32_t sf8;
+  float enc_b;
+  block_scale(amax_b, ts, sf8, enc_b);
+  if (!live) return;
+  uint2 c;
+  c.x = quant_bf16x8(v0, enc_b);
+  c.y = quant_bf16x8(v1, enc_b);
+  *reinterpret_cast<uint2*>(codes + row * (cols / 2) + bc * 8) = c;
+  if (sf_layout == FT_SF_TILE128x4) {
+    sf[sf_tile_offset(row, bc, nblk)] = (uint8_t)sf8;
+  } else if (BR == 1 || (row % 16) == 0) {
+    sf[(row / BR) * nblk + bc] = (uint8_t)sf8;
+  }
+}
+
+int launch_quantize_generic(const void* x, int64_t rows, int64_t cols, const float* amax_t,
+                            ft_qtensor* out, cudaStream_t st) {
+  const int64_t threads = rows * (cols / 16);
+  const unsigned blocks = (unsigned)ceil_div(threads, 256);
+  if (out->sf_layout == FT_SF_TILE128x4)
+    FT_CUDA_TRY(cudaMemsetAsync(out->sf, 0, ft_sf_bytes(rows, cols, out->block_rows, FT_SF_TILE128x4), st));
+  if (out->block_rows == 16)
+    k_quantize_generic<16><<<blocks, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), rows, cols,
+                                                   amax_t, out->codes, out->sf,
+                                                   out->tensor_dec_scale, out->sf_layout);
+  else
+    k_quantize_generic<1><<<blocks, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), rows, cols,
+                                                  amax_t, out->codes, out->sf,
+                                                  out->tensor_dec_scale, out->sf_layout);
+  FT_CUDA_TRY(cudaGetLastError());
+  return FT_OK;
+}
+
+// --------------------------------------------------------- a6: weight re-packing
+// codes_t[k][n] = codes[n][k] for 4-bit codes: 64x64 code tile through shared memory.
+__global__ void __launch_bounds__(256) k_transpose_codes(const uint8_t* __restrict__ src,
+                                                         uint8_t* __restrict__ dst, int64_t N,
+                                                         int64_t K) {
+  __shared__ uint8_t tile[64][65];  // unpacked codes, [n][k]
+  const int64_t n0 = (int64_t)blockIdx.y * 64, k0 = (int64_t)blockIdx.x * 64;
+  for (int i = threadIdx.x; i < 64 * 32; i += 256) {
+    const int n = i / 32, kb = i % 32;
+    const uint8_t b = src[(n0 + n) * (K / 2) + k0 / 2 + kb];
+    tile[n][2 * kb] = b & 0xF;
+    tile[n][2 * kb + 1] = b >> 4;
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < 64 * 32; i += 256) {
+    const int k = i / 32, nb = i % 32;
+    dst[(k0 + k) * (N / 2) + n0 / 2 + nb] = tile[2 * nb][k] | (tile[2 * nb + 1][k] << 4);
+  }
+}
+
+// Expand S[N/16][K/16] to per-row TILE128x4 scales for both orientations:
+//   fwd  : rows n, blocks along K :  sf(n, kb) = S[n/16][kb]
+//   dgrad: rows k, blocks along N :  sf(k, nb) = S[nb][k/16]
+__global__ void __launch_bounds__(256) k_expand_sf(const uint8_t* __restrict__ S, int64_t N,
+                                                   int64_t K, uint8_t* __restrict__ sf_fwd,
+                                                   uint8_t* __restrict__ sf_bwd) {
+  const int64_t nb16 = N / 16, kb16 = K / 16;
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (sf_fwd != nullptr && t < N * kb16) {
+    const int64_t n = t / kb16, kb = t % kb16;
+    sf_fwd[sf_tile_offset(n, kb, kb16)] = S[(n / 16) * kb16 + kb];
+  }
+  if (sf_bwd != nullptr && t < K * nb16) {
+    const int64_t k = t / nb16, nb = t % nb16;
+    sf_bwd[sf_tile_offset(k, nb, nb16)] = S[nb * kb16 + k / 16];
+  }
+}
+
+int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn,
+                       cudaStream_t st) {
+  const int64_t N = rk->rows, K = rk->cols;
+  dim3 grid((unsigned)(K / 64), (unsigned)(N / 64));
+  k_transpose_codes<<<grid, 256, 0, st>>>(rk->codes, rn->codes, N, K);
+  FT_CUDA_TRY(cudaGetLastError());
+  FT_CUDA_TRY(cudaMemsetAsync(rn->sf, 0, ft_sf_bytes(K, N, 16, FT_SF_TILE128x4), st));
+  if (rk_tiled != nullptr)
+    FT_CUDA_TRY(cudaMemsetAsync(rk_tiled->sf, 0, ft_sf_bytes(N, K, 16, FT_SF_TILE128x4), st));
+  const int64_t threads = (N > K ? N : K) * ((N > K ? K : N) / 16) ;
+  const int64_t tmax = (N * (K / 16) > K * (N / 16)) ? N * (K / 16) : K * (N / 16);
+  (void)threads;
+  k_expand_sf<<<(unsigned)ceil_div(tmax, 256), 256, 0, st>>>(
+      rk->sf, N, K, rk_tiled ? rk_tiled->sf : nullptr, rn->sf);
+  FT_CUDA_TRY(cudaGetLastError());
+  FT_CUDA_TRY(cudaMemcpyAsync(rn->tensor_dec_scale, rk->tensor_dec_scale, sizeof(float),
+                              cudaMemcpyDeviceToDevice, st));
+  if (rk_tiled != nullptr && rk_tiled->tensor_dec_scale != rk->tensor_dec_scale &&
+      rk_tiled->tensor_dec_scale != nullptr)
+    FT_CUDA_TRY(cudaMemcpyAsync(rk_tiled->tensor_dec_scale, rk->tensor_dec_scale, sizeof(float),
+                                cudaMemcpyDeviceToDevice, st));
+  return FT_OK;
+}
+
+}  // namespace ft
