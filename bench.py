@@ -1,0 +1,371 @@
+#!/usr/bin/env python
+"""bench.py -- W4A4G4 triple-branch linear, fwd + bwd, on synthetic FLUX.1-dev-shaped input.
+
+A step = one pass of the whole hot path (rows a0-a5) over one batch:
+    ft_linear_fwd (amax, fused quantize + down-projection, 4-bit GEMM + up-projection)
+    ft_linear_bwd_dgrad (the same on G with Q(R)^T)
+    ft_lora_wgrad (dA, dB^T)
+Workload at N=1: BASELINE.json configs[1] (C2): fused QKV projection M=4608, K=3072, N=9216,
+stabilizer rank 32, LoRA rank 32.  N>1: every rank runs the same layer on its own batch of 4608
+tokens (weak scaling) and all-reduces the LoRA gradients (NCCL), the path's only exchange.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+prints ONE JSON line (rank 0).  --impl reference times the CPU oracle on a bounded sample.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+WORKLOAD = dict(name="C2 FLUX.1-dev fused QKV projection", M=4608, K=3072, N=9216, r_s=32, r=32, seed=1)
+METRIC = "W4A4G4 linear fwd+bwd TFLOPS (4*M*N*K per step / step time)"
+UNIT = "TFLOP/s"
+FP4_OVER_BF16 = 4.0   # nominal dense ratio 9 / 2.25 PFLOP/s (B200_PROFILING.md)
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_gemm4 launch (C2 forward), from the
+# ncu --set full capture summarised in profiles/r01_gemm4_full.md; None until captured.
+GEMM_DRAM_TRAFFIC_BYTES = None
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sustained=d.get("bf16_tflops_sustained"),
+                    source="measured")
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = sorted(int(r[0]) for r in self.rows if r and r[0].isdigit())
+        mx = [int(r[1]) for r in self.rows if len(r) > 1 and r[1].isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+# ------------------------------------------------------------------ CPU oracle arm
+def oracle_sample(rows=256, repeats=1):
+    """The oracle as it stands on a bounded sample of the workload: the first `rows` tokens of
+    the C2 batch through forward + dgrad + wgrad against the full-size weight.  Offline parts
+    (Eq. 1 split, Q(R)) are outside the timed region, as on the GPU."""
+    import numpy as np
+    from oracle import layer as olayer
+    from oracle import nvfp4
+    from paper_2607_05711_b200 import synth
+    w = WORKLOAD
+    rng = synth.make_rng(w["seed"])
+    X = synth.outlier_normal(rng, rows, w["K"])
+    R = synth.normal(rng, (w["N"], w["K"]), 0.02)
+    r_t = w["r_s"] + w["r"]
+    D_f = synth.normal(rng, (w["K"], r_t), 0.01)
+    U_f = synth.normal(rng, (r_t, w["N"]), 0.01)
+    G = synth.student_t_grad(rng, rows, w["N"])
+    qR = olayer.quantize_weight(R)
+    times = []
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        f = olayer.forward(X, qR, D_f, U_f, prescale=True)
+        b = olayer.dgrad(G, qR, D_f, U_f, prescale=True)
+        olayer.wgrad(X, G, f["H"], b["P"], w["r_s"])
+        times.append(time.perf_counter() - t0)
+    flops = 4.0 * rows * w["N"] * w["K"]
+    return flops, times
+
+
+def cpu_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    rows = WORKLOAD["M"]
+    oracle_sample(rows, 1)                                   # warm-up (BLAS threads, page faults)
+    for _ in range(max(0, min(args.warmup, 1))):
+        pass
+    steps = max(1, min(args.steps, 4))                       # each step ~5 s of CPU work
+    flops, times = oracle_sample(rows, steps)
+    t = sum(times) / len(times)
+    val = flops / t / 1e12
+    sample = "all %d tokens of C2 (M=%d), fwd+dgrad+wgrad, %d step(s)" % (rows, WORKLOAD["M"], steps)
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+           "warmup": 1, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": WORKLOAD["name"], **{k: WORKLOAD[k] for k in ("M", "K", "N", "r_s", "r")},
+                      "sample_rows": rows},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle", "sample": sample},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+# ------------------------------------------------------------------ GPU arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2607_05711_b200 import binding as B
+    from paper_2607_05711_b200 import build as _build
+    from paper_2607_05711_b200 import parallel, prepare
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    _build.build()
+    B.lib()                                   # fails loudly if the CUDA library is missing
+    w = WORKLOAD
+    M, K, N, r_s, r = w["M"], w["K"], w["N"], w["r_s"], w["r"]
+    r_t = r_s + r
+    peaks = load_peaks()
+
+    # ---- synthetic inputs, generated on the host (seeded), resident in HBM before timing
+    import numpy as np
+    from paper_2607_05711_b200 import synth
+    rng = synth.make_rng(w["seed"] + 1000 * rank)
+    Xh = torch.from_numpy(synth.outlier_normal(rng, M, K)).to(torch.bfloat16).pin_memory()
+    Wt = torch.from_numpy(synth.normal(rng, (N, K), 0.02)).to(torch.bfloat16).to(dev)
+    A = torch.from_numpy(synth.normal(rng, (K, r), 0.01)).to(torch.bfloat16).to(dev)
+    Bt = torch.from_numpy(synth.normal(rng, (N, r), 0.01)).to(torch.bfloat16).to(dev)
+    Gh = torch.from_numpy(synth.student_t_grad(rng, M, N)).to(torch.bfloat16).pin_memory()
+    R, L1, L2t = prepare.random_range_split(Wt, r_s, seed=w["seed"])     # offline (Eq. 1)
+    D_f = torch.cat([L1, A], 1).contiguous()
+    U_t = torch.cat([L2t, Bt], 1).contiguous()
+    layer = B.Layer(R, D_f, U_t, r_s, r)                                 # offline: Q(R), both packings
+    X, G = Xh.to(dev), Gh.to(dev)
+    y = torch.empty(M, N, dtype=torch.bfloat16, device=dev)
+    dx = torch.empty(M, K, dtype=torch.bfloat16, device=dev)
+    h = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
+    p = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
+    ws = torch.empty(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_t), dtype=torch.uint8, device=dev)
+    qx, qg = B.QTensor(M, K, device=dev), B.QTensor(M, N, device=dev)
+    dA = torch.empty(K, r, dtype=torch.float32, device=dev)
+    dBt = torch.empty(N, r, dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        B.ft_linear_fwd(layer, X, y, h, qx, ws)
+        B.ft_linear_bwd_dgrad(layer, G, dx, p, qg, ws)
+        B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt)
+        if world > 1:
+            parallel.allreduce_lora_grads(dA, dBt)
+    KERNELS_PER_STEP = 8   # 2 x (k_amax, k_quantize_fused, k_gemm4) + 2 x k_wgrad (memsets not counted)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    # the launch-bound prologue (amax, quantize) is short: replay the step as a CUDA graph at
+    # N=1 so the host never gates the device; eager otherwise
+    graph, launch = None, "eager"
+    if world == 1 and not args.eager:
+        try:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                step()
+            g.replay()
+            torch.cuda.synchronize()
+            graph, launch = g, "cuda_graph"
+        except Exception as e:   # noqa: BLE001
+            sys.stderr.write("graph capture failed (%s): eager launches\n" % e)
+            torch.cuda.synchronize()
+    run = (graph.replay if graph is not None else step)
+    for _ in range(3):
+        run()
+    barrier()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        run()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_per_step = float(tmax.item()) / args.steps
+    flops_step = 4.0 * M * N * K
+    value = world * flops_step / (ms_per_step * 1e-3) / 1e12
+
+    # ---- end to end through the public API with HOST buffers: H2D of X and G, D2H of every result
+    yh = torch.empty(M, N, dtype=torch.bfloat16).pin_memory()
+    dxh = torch.empty(M, K, dtype=torch.bfloat16).pin_memory()
+    dAh = torch.empty(K, r, dtype=torch.float32).pin_memory()
+    dBh = torch.empty(N, r, dtype=torch.float32).pin_memory()
+
+    def e2e_step():
+        X.copy_(Xh, non_blocking=True)
+        G.copy_(Gh, non_blocking=True)
+        step()
+        yh.copy_(y, non_blocking=True)
+        dxh.copy_(dx, non_blocking=True)
+        dAh.copy_(dA, non_blocking=True)
+        dBh.copy_(dBt, non_blocking=True)
+    e2e_step()
+    barrier()
+    n_e2e = max(3, min(args.steps, 20))
+    e0.record()
+    for _ in range(n_e2e):
+        e2e_step()
+    e1.record()
+    barrier()
+    te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_ms = float(te.item()) / n_e2e
+    clocks = sampler.stop()
+    h2d = (Xh.numel() + Gh.numel()) * 2
+    d2h = (yh.numel() + dxh.numel()) * 2 + (dAh.numel() + dBh.numel()) * 4
+
+    # ---- per-kernel breakdown: each launch alone, CUDA events on its stream, L2 flushed between
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    hs = ws[256:256 + M * r_t * 2].view(torch.bfloat16).view(M, r_t)
+    amax = torch.empty(1, dtype=torch.float32, device=dev)
+
+    def timed(fn, n=20):
+        fn()
+        tot = 0.0
+        for _ in range(n):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fn()
+            b.record(stream)
+            torch.cuda.synchronize()
+            tot += a.elapsed_time(b)
+        return tot / n * 1e3   # us
+
+    kern = {}
+    kern["amax_X_us"] = timed(lambda: B.ft_tensor_amax(X, amax))
+    kern["quant_X_us"] = timed(lambda: B.ft_quantize_blockwise(
+        X, qx, tensor_amax=amax, down=D_f, h_out=h, hs_out=hs, other_dec_scale=layer.r_kmajor.tensor_dec_scale,
+        workspace=ws))
+    kern["gemm_fwd_us"] = timed(lambda: B.ft_gemm4(qx, layer.r_kmajor, hs, U_t, y))
+    amax_g = B.ft_tensor_amax(G)
+    kern["amax_G_us"] = timed(lambda: B.ft_tensor_amax(G, amax_g))
+    kern["quant_G_us"] = timed(lambda: B.ft_quantize_blockwise(
+        G, qg, tensor_amax=amax_g, down=U_t, h_out=p, hs_out=hs, other_dec_scale=layer.r_nmajor.tensor_dec_scale,
+        workspace=ws))
+    kern["gemm_dgrad_us"] = timed(lambda: B.ft_gemm4(qg, layer.r_nmajor, hs, D_f, dx))
+    kern["wgrad_us"] = timed(lambda: B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt))
+
+    # bf16 cuBLAS LoRA layer on the same GPU, same shapes (context: speedup vs BF16 LoRA)
+    Am, Bm = A, Bt.t().contiguous()
+
+    def bf16_lora():
+        xa = X @ Am
+        yy = X @ Wt.t() + xa @ Bm                     # noqa: F841
+        gb = G @ Bm.t()
+        dxx = G @ Wt + gb @ Am.t()                    # noqa: F841
+        da = X.t() @ gb                               # noqa: F841
+        db = xa.t() @ G                               # noqa: F841
+    bf16_us = timed(bf16_lora, n=10)
+
+    out = None
+    if rank == 0:
+        gemm_us = 0.5 * (kern["gemm_fwd_us"] + kern["gemm_dgrad_us"])
+        gemm_tflops = 2.0 * M * N * K / (gemm_us * 1e-6) / 1e12
+        fp4_peak = peaks["bf16"] * FP4_OVER_BF16
+        q_bytes_x, q_bytes_g = 2.5625 * M * K, 2.5625 * M * N
+        cpu_flops, cpu_times = oracle_sample(M, 2)
+        cpu_val = cpu_flops / (sum(cpu_times) / 2) / 1e12
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "nvfp4 (e2m1 x ue4m3, fp32 accumulate) + bf16 low-rank", "data": "synthetic",
+            "config": {"workload": w["name"], "M": M, "K": K, "N": N, "r_s": r_s, "r": r, "tokens_per_gpu": M,
+                       "launch": launch, "l2": "step working set ~330 MB > 126 MB L2; per-kernel timings flush L2",
+                       "parallelism": "dp%d (tokens), all-reduce of dA,dB only" % world,
+                       "peaks": peaks["source"]},
+            "clocks": clocks,
+            "e2e": {"value": world * flops_step / (e2e_ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms,
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": KERNELS_PER_STEP * args.steps,
+            "roofline": {"kernel": "k_gemm4 (mean of fwd and dgrad launches)", "bound": "tensor",
+                         "achieved": gemm_tflops, "peak": fp4_peak, "unit": "TFLOP/s", "frac": gemm_tflops / fp4_peak,
+                         "peak_note": "measured bf16 burst %.1f x nominal fp4/bf16 ratio 4 (of %s); nominal 9000"
+                                      % (peaks["bf16"], peaks["source"]),
+                         "traffic": GEMM_DRAM_TRAFFIC_BYTES},
+            "kernels_us": {k: round(v, 2) for k, v in kern.items()},
+            "quantize": {"X_GBps": q_bytes_x / kern["quant_X_us"] / 1e3, "G_GBps": q_bytes_g / kern["quant_G_us"] / 1e3,
+                         "frac_of_hbm_X": q_bytes_x / kern["quant_X_us"] / 1e3 / peaks["hbm"],
+                         "frac_of_hbm_G": q_bytes_g / kern["quant_G_us"] / 1e3 / peaks["hbm"],
+                         "bytes_per_element": 2.5625, "hbm_peak_GBps": peaks["hbm"]},
+            "bf16_lora_baseline": {"us_per_step": bf16_us, "speedup": bf16_us / (ms_per_step * 1e3),
+                                   "how": "torch.matmul (cuBLAS) bf16, frozen W, same shapes, same GPU"},
+            "paper_context": "2.27x step time / 2.25x memory vs BF16 LoRA on RTX 5090 (PAPER.md:7,207); not the target",
+            "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle",
+                             "sample": "all 4608 tokens of C2, fwd+dgrad+wgrad, mean of 2 passes (%.1f s of CPU work)"
+                                       % sum(cpu_times)},
+        }
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--eager", action="store_true", help="no CUDA graph for the timed steps")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -141,6 +141,15 @@ int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* 
                         void* p_saved_bf16, ft_qtensor* qg_scratch, void* workspace,
                         size_t workspace_bytes, void* stream);
 
+/* ---- a2 / a4 alone: out[M x N] = bf16( alpha * ( GEMM4(a, b) + lr_a_scaled * lr_b^T ) ),
+ * alpha = *a->tensor_dec_scale * *b->tensor_dec_scale.
+ * a: Q(X) [M x K] (block_rows 1), b: Q(R) [N x K]; both sf TILE128x4, K % 64 == 0, N % 64 == 0.
+ * lr_a_scaled: bf16 [M x r_t] = bf16(H / alpha) as written by ft_quantize_blockwise's
+ * out_scaled; lr_b: bf16 [N x r_t]; r_t = 0 (both may be NULL) skips the low-rank term.
+ * ft_linear_fwd / ft_linear_bwd_dgrad are ft_tensor_amax + ft_quantize_blockwise + this. */
+int ft_gemm4(const ft_qtensor* a, const ft_qtensor* b, const void* lr_a_scaled, const void* lr_b,
+             int32_t r_t, void* out_bf16, void* stream);
+
 /* ---- a5: LoRA weight gradients (Eq. 4), fp32.
  * dA  [K x r]  = X^T  * P[:, r_s:]      dBt [N x r] = G^T * H[:, r_s:]  (= dB^T)
  * h_saved / p_saved are the [M x r_t] outputs of the two calls above.

@@ -53,6 +53,7 @@ def lib():
         L.ft_pack_weight.argtypes = [C.POINTER(_QT), C.POINTER(_QT), C.POINTER(_QT), vp]
         L.ft_linear_fwd.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
         L.ft_linear_bwd_dgrad.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
+        L.ft_gemm4.argtypes = [C.POINTER(_QT), C.POINTER(_QT), vp, vp, i32, vp, vp]
         L.ft_lora_wgrad.argtypes = [C.POINTER(_Layer), vp, vp, i64, vp, vp, vp, vp, i32, vp]
         L.ft_sf_bytes.argtypes = [i64, i64, i32, i32]
         L.ft_sf_bytes.restype = sz
@@ -184,6 +185,14 @@ def ft_linear_bwd_dgrad(layer, g, dx, p_saved, qg, workspace, stream=None):
                                      _ptr(workspace), workspace.numel(), _stream(stream)))
     qg.sync_from(q)
     return dx
+
+
+def ft_gemm4(a, b, lr_a_scaled, lr_b, out, stream=None):
+    qa, qb = a.c(), b.c()
+    r_t = 0 if lr_a_scaled is None else lr_a_scaled.shape[1]
+    _check(lib().ft_gemm4(C.byref(qa), C.byref(qb), _ptr(lr_a_scaled), _ptr(lr_b), r_t, _ptr(out),
+                          _stream(stream)))
+    return out
 
 
 def ft_lora_wgrad(layer, x, g, h_saved, p_saved, dA, dBt, accumulate=False, stream=None):

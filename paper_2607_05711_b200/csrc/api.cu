@@ -238,6 +238,25 @@ int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, v
   return launch_pack_weight(rk, rk_tiled, rn, (cudaStream_t)stream);
 }
 
+int ft_gemm4(const ft_qtensor* a, const ft_qtensor* b, const void* lr_a_scaled, const void* lr_b,
+             int32_t r_t, void* out_bf16, void* stream) {
+  if (!a || !b || !out_bf16 || !a->codes || !a->sf || !a->tensor_dec_scale || !b->codes || !b->sf ||
+      !b->tensor_dec_scale)
+    return FT_ERR_INVALID_ARG;
+  if (a->sf_layout != FT_SF_TILE128x4 || b->sf_layout != FT_SF_TILE128x4) return FT_ERR_INVALID_ARG;
+  if (!valid_rt(r_t) || (r_t > 0 && (!lr_a_scaled || !lr_b))) return FT_ERR_INVALID_ARG;
+  if (a->cols != b->cols || a->rows < 1 || a->cols % 64 != 0 || a->cols < 64 || b->rows % 64 != 0 ||
+      b->rows < 64)
+    return FT_ERR_UNSUPPORTED_SHAPE;
+  if (!aligned16(a->codes) || !aligned16(a->sf) || !aligned16(b->codes) || !aligned16(b->sf) ||
+      !aligned16(out_bf16) || (r_t > 0 && (!aligned16(lr_a_scaled) || !aligned16(lr_b))))
+    return FT_ERR_INVALID_ARG;
+  int rc = device_check();
+  if (rc != FT_OK) return rc;
+  return launch_gemm4(a, b, a->rows, b->rows, a->cols, lr_a_scaled, lr_b, r_t, out_bf16,
+                      (cudaStream_t)stream);
+}
+
 int ft_linear_fwd(const ft_layer* L, const void* x_bf16, int64_t M, void* y_bf16,
                   void* h_saved_bf16, ft_qtensor* qx_scratch, void* workspace,
                   size_t workspace_bytes, void* stream) {

@@ -1,0 +1,280 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Bars (BASELINE.json north_star, O-11): FP4 codes, block scales and the tensor scale
+bit-exact; GEMM / branch outputs within relative Frobenius error 1e-3 of the oracle's float64
+accumulation of the same dequantized operands (the oracle consumes the GPU's own bf16 low-rank
+intermediate, which is itself checked against the oracle's to 2e-3 and >= 99 % identical)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from oracle import layer as olayer
+from oracle import nvfp4
+from paper_2607_05711_b200 import synth
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-3
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2607_05711_b200 import build, binding
+    build.build()
+    binding.lib()
+    return binding
+
+
+def t16(a):
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda().to(torch.bfloat16)
+
+
+def npf(t):
+    return t.float().cpu().numpy()
+
+
+def rel(a, b):
+    d = np.linalg.norm(np.asarray(b, np.float64))
+    return np.linalg.norm(np.asarray(a, np.float64) - np.asarray(b, np.float64)) / (d if d > 0 else 1.0)
+
+
+def assert_q_equal(qt, q, layout, B):
+    rows, cols = q["codes"].shape
+    assert np.array_equal(qt.codes.cpu().numpy(), q["packed"])
+    sf = qt.sf.cpu().numpy()
+    if layout == B.FT_SF_ROWMAJOR:
+        assert np.array_equal(sf.reshape(q["sf"].shape), q["sf"])
+    else:
+        assert np.array_equal(sf, nvfp4.sf_to_tile128x4(nvfp4.sf_expand_rows(q["sf"], q["block_rows"])))
+    assert qt.tensor_dec_scale.cpu().numpy().view(np.uint32)[0] == np.float32(q["g_dec"]).view(np.uint32)
+
+
+# ------------------------------------------------------------------ a0
+@pytest.mark.parametrize("n", [8, 24, 1000, 4608 * 3072 + 3])
+def test_amax(B, n):
+    rng = synth.make_rng(n)
+    x = synth.to_bf16_f32(rng.standard_normal(n + 8, dtype=np.float32) * 3)[:n]
+    x[n // 2] = -77.5
+    xt = t16(np.concatenate([x, np.zeros(8, np.float32)]))[:n]
+    got = B.ft_tensor_amax(xt).cpu().numpy()[0]
+    assert got == nvfp4.tensor_amax(x) == np.float32(77.5)
+
+
+# ------------------------------------------------------------------ a1 / a3 / a6: quantizer
+QCASES = [  # rows, cols, kind, layout
+    (1, 64, "x", 0), (16, 64, "g", 1), (128, 256, "x", 0), (130, 512, "x", 1), (257, 1024, "g", 1),
+    (256, 3072, "x", 1), (256, 3072, "g", 1), (384, 15360, "x", 1)]
+
+
+@pytest.mark.parametrize("rows,cols,kind,layout", QCASES)
+def test_quantize_1x16_bit_exact(B, rows, cols, kind, layout):
+    rng = synth.make_rng(rows * 131 + cols)
+    x = synth.outlier_normal(rng, rows, cols) if kind == "x" else synth.student_t_grad(rng, rows, cols)
+    out = B.QTensor(rows, cols, 1, layout)
+    B.ft_quantize_blockwise(t16(x), out)
+    assert_q_equal(out, nvfp4.quantize_blockwise(x, 1), layout, B)
+
+
+def test_quantize_degenerate_inputs(B):
+    # all zeros; -0.0; a block of tiny values next to the tensor maximum; saturating ties
+    x = np.zeros((128, 128), np.float32)
+    out = B.QTensor(128, 128, 1, 0)
+    B.ft_quantize_blockwise(t16(x), out)
+    assert_q_equal(out, nvfp4.quantize_blockwise(x, 1), 0, B)
+    x[0, :16] = [0.5, -1, 1.5, 2, 3, -6, 0.25, 0.75, 1.25, 1.75, 2.5, 3.5, 5, 0, -0.0, 4]
+    x[1, 16:32] = 1e-6
+    x[2, 32:48] = -0.0
+    x[3, :] = synth.to_bf16_f32(np.linspace(-6, 6, 128, dtype=np.float32))
+    x[5, 64] = 2688.0
+    x = synth.to_bf16_f32(x)
+    B.ft_quantize_blockwise(t16(x), out)
+    assert_q_equal(out, nvfp4.quantize_blockwise(x, 1), 0, B)
+    # caller-supplied tensor amax (static scaling) is honoured
+    amax = torch.tensor([6.0 * 448], dtype=torch.float32, device="cuda")
+    B.ft_quantize_blockwise(t16(x), out, tensor_amax=amax)
+    assert_q_equal(out, nvfp4.quantize_blockwise(x, 1, amax_t=np.float32(2688.0)), 0, B)
+
+
+@pytest.mark.parametrize("N,K", [(64, 64), (256, 512), (3072, 3072)])
+def test_weight_quantize_16x16_and_pack(B, N, K):
+    rng = synth.make_rng(N + K)
+    W = synth.normal(rng, (N, K), 0.02)
+    q = nvfp4.quantize_blockwise(W, 16)
+    L = B.Layer(t16(W), None, None, 0, 0)
+    assert_q_equal(L.q_rowmajor, q, B.FT_SF_ROWMAJOR, B)
+    assert_q_equal(L.r_kmajor, q, B.FT_SF_TILE128x4, B)
+    # Q(R)^T is the same codes and scales re-indexed: compare with the
+    # transposed oracle object, and with the oracle quantizing R^T afresh (pin P-4)
+    qT = dict(q, codes=np.ascontiguousarray(q["codes"].T), sf=np.ascontiguousarray(q["sf"].T))
+    qT["packed"] = nvfp4.pack_codes(qT["codes"])
+    assert_q_equal(L.r_nmajor, qT, B.FT_SF_TILE128x4, B)
+    q2 = nvfp4.quantize_blockwise(np.ascontiguousarray(W.T), 16)
+    assert np.array_equal(q2["packed"], qT["packed"]) and np.array_equal(q2["sf"], qT["sf"])
+
+
+@pytest.mark.parametrize("rows,cols,r_t,kind", [(128, 512, 16, "x"), (200, 1024, 64, "x"), (256, 3072, 48, "x"),
+                                                (384, 2048, 96, "g"), (130, 4096, 128, "g")])
+def test_fused_projection(B, rows, cols, r_t, kind):
+    rng = synth.make_rng(rows + cols + r_t)
+    x = synth.outlier_normal(rng, rows, cols) if kind == "x" else synth.student_t_grad(rng, rows, cols)
+    D = synth.normal(rng, (cols, r_t), 0.01)
+    other = np.float32(3.7e-5)
+    out = B.QTensor(rows, cols, 1, B.FT_SF_TILE128x4)
+    h = torch.zeros(rows, r_t, dtype=torch.bfloat16, device="cuda")
+    hs = torch.zeros_like(h)
+    B.ft_quantize_blockwise(t16(x), out, down=t16(D), h_out=h, hs_out=hs,
+                            other_dec_scale=torch.tensor([other], device="cuda"))
+    q = nvfp4.quantize_blockwise(x, 1)
+    assert_q_equal(out, q, B.FT_SF_TILE128x4, B)   # fusing the projection must not change a bit
+    Hex = x.astype(np.float64) @ D.astype(np.float64)
+    Ho = nvfp4.bf16_round_from_f64(Hex)
+    alpha = np.float64(np.float32(q["g_dec"]) * other)
+    Hso = nvfp4.bf16_round_from_f64(Hex / alpha)
+    for got, want in ((npf(h), Ho), (npf(hs), Hso)):
+        assert rel(got, want) <= 2e-3
+        assert (got == want).mean() >= 0.99
+        # every element within one bf16 ulp of the oracle's, plus the fp32 accumulation error
+        # of a length-`cols` dot product on elements that cancel to nearly zero
+        assert np.all(np.abs(got - want) <= np.abs(want) * 2.0 ** -7 + 1e-5 * np.abs(want).max())
+
+
+# ------------------------------------------------------------------ a2 / a4 / a5: the layer
+def make_layer(B, seed, M, K, N, r_s, r, x_kind="outlier"):
+    d = synth.layer_inputs(seed, M, K, N, max(r, 1), x_kind)
+    R, L1, L2 = olayer.prepare_weight(d["W"], r_s)
+    D_f = np.concatenate([L1, d["A"][:, :r]], 1).astype(np.float32)
+    U_f = np.concatenate([L2, d["B"][:r, :]], 0).astype(np.float32)
+    r_t = r_s + r
+    L = B.Layer(t16(R), t16(D_f) if r_t else None, t16(U_f.T) if r_t else None, r_s, r)
+    return d, R, D_f, U_f, L
+
+
+def run_layer(B, L, X, G, M, K, N, r_t, r):
+    y = torch.zeros(M, N, dtype=torch.bfloat16, device="cuda")
+    dx = torch.zeros(M, K, dtype=torch.bfloat16, device="cuda")
+    h = torch.zeros(M, max(r_t, 1), dtype=torch.bfloat16, device="cuda")
+    p = torch.zeros_like(h)
+    ws = torch.zeros(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_t), dtype=torch.uint8, device="cuda")
+    qx, qg = B.QTensor(M, K), B.QTensor(M, N)
+    xt, gt = t16(X), t16(G)
+    scaled = lambda: (npf(ws[256:256 + M * r_t * 2].view(torch.bfloat16).reshape(M, r_t)) if r_t else None)
+    B.ft_linear_fwd(L, xt, y, h, qx, ws)
+    torch.cuda.synchronize()
+    hs = scaled()
+    B.ft_linear_bwd_dgrad(L, gt, dx, p, qg, ws)
+    torch.cuda.synchronize()
+    ps = scaled()
+    dA = dBt = None
+    if r > 0:
+        dA = torch.full((K, r), 7.0, dtype=torch.float32, device="cuda")
+        dBt = torch.full((N, r), 7.0, dtype=torch.float32, device="cuda")
+        B.ft_lora_wgrad(L, xt, gt, h, p, dA, dBt)
+    return dict(y=npf(y), dx=npf(dx), h=npf(h), p=npf(p), hs=hs, ps=ps, qx=qx, qg=qg,
+                dA=None if dA is None else dA.cpu().numpy(), dBt=None if dBt is None else dBt.cpu().numpy(),
+                xt=xt, gt=gt, ht=h, pt=p)
+
+
+LAYER_CASES = [  # seed, M, K, N, r_s, r, tile_n
+    (11, 1, 64, 64, 0, 0, 0), (12, 128, 256, 128, 0, 0, 256), (13, 130, 320, 192, 16, 16, 0),
+    (14, 256, 512, 384, 16, 16, 192), (15, 200, 1024, 768, 32, 64, 256), (16, 300, 576, 448, 32, 32, 128),
+    (17, 129, 2048, 640, 0, 16, 192)]
+
+
+@pytest.mark.parametrize("seed,M,K,N,r_s,r,bn", LAYER_CASES)
+def test_layer_small(B, seed, M, K, N, r_s, r, bn):
+    B.debug_set_gemm_tile_n(bn)
+    try:
+        d, R, D_f, U_f, L = make_layer(B, seed, M, K, N, r_s, r)
+        out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
+    finally:
+        B.debug_set_gemm_tile_n(0)
+    check_layer(B, d, R, D_f, U_f, out, r_s, r)
+
+
+def check_layer(B, d, R, D_f, U_f, out, r_s, r, rows=None):
+    """Full comparison, or on a row sample (rows) for sizes the oracle cannot finish whole."""
+    X, G = d["X"], d["dY"]
+    r_t = r_s + r
+    qR = olayer.quantize_weight(R)
+    ax, ag = nvfp4.tensor_amax(X), nvfp4.tensor_amax(G)
+    sel = slice(None) if rows is None else rows
+    # (i) codes / scales bit-exact, on the whole tensors
+    assert_q_equal(out["qx"], nvfp4.quantize_blockwise(X, 1), B.FT_SF_TILE128x4, B)
+    assert_q_equal(out["qg"], nvfp4.quantize_blockwise(G, 1), B.FT_SF_TILE128x4, B)
+    f = olayer.forward(X[sel], qR, D_f, U_f, prescale=True, x_amax=ax,
+                       H_given=None if r_t == 0 else out["hs"][sel])
+    b = olayer.dgrad(G[sel], qR, D_f, U_f, prescale=True, g_amax=ag,
+                     P_given=None if r_t == 0 else out["ps"][sel])
+    if r_t:
+        # (ii) the low-rank intermediates against the oracle's own
+        for got, want in ((out["h"][sel], f["H"]), (out["hs"][sel], f["Hs"]), (out["p"][sel], b["P"]),
+                          (out["ps"][sel], b["Ps"])):
+            assert rel(got, want) <= 2e-3 and (got == want).mean() >= 0.99
+    # (iii) outputs, both cast to bf16
+    assert rel(out["y"][sel], f["Y"]) <= TOL
+    assert rel(out["dx"][sel], b["dX"]) <= TOL
+    assert (out["y"][sel] == f["Y"]).mean() >= 0.95 and (out["dx"][sel] == b["dX"]).mean() >= 0.95
+    if r > 0 and rows is None:
+        w = olayer.wgrad(X, G, out["h"], out["p"], r_s)
+        assert rel(out["dA"], w["dA"]) <= TOL and rel(out["dBt"].T, w["dB"]) <= TOL
+
+
+def test_layer_degenerate_branches(B):
+    """B = 0 -> branch 3 contributes nothing to Y and dX, dA = 0, dB != 0; A = 0 -> dB = 0 (pin P-5)."""
+    M, K, N, r_s, r = 128, 256, 128, 16, 16
+    d, R, D_f, U_f, _ = make_layer(B, 31, M, K, N, r_s, r)
+    U0 = U_f.copy(); U0[r_s:, :] = 0
+    L0 = B.Layer(t16(R), t16(D_f), t16(U0.T), r_s, r)
+    o0 = run_layer(B, L0, d["X"], d["dY"], M, K, N, r_s + r, r)
+    Ls = B.Layer(t16(R), t16(D_f[:, :r_s]), t16(U_f[:r_s].T), r_s, 0)
+    os_ = run_layer(B, Ls, d["X"], d["dY"], M, K, N, r_s, 0)
+    assert rel(o0["y"], os_["y"]) <= 1e-3 and np.all(o0["dA"] == 0) and np.any(o0["dBt"] != 0)
+    D0 = D_f.copy(); D0[:, r_s:] = 0
+    L1 = B.Layer(t16(R), t16(D0), t16(U_f.T), r_s, r)
+    o1 = run_layer(B, L1, d["X"], d["dY"], M, K, N, r_s + r, r)
+    assert np.all(o1["dBt"] == 0) and np.any(o1["dA"] != 0)
+
+
+def test_wgrad_accumulate(B):
+    M, K, N, r_s, r = 192, 128, 192, 16, 16
+    d, R, D_f, U_f, L = make_layer(B, 41, M, K, N, r_s, r)
+    o = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
+    dA = torch.from_numpy(o["dA"]).cuda().clone(); dBt = torch.from_numpy(o["dBt"]).cuda().clone()
+    B.ft_lora_wgrad(L, o["xt"], o["gt"], o["ht"], o["pt"], dA, dBt, accumulate=True)
+    assert rel(dA.cpu().numpy(), 2 * o["dA"]) <= 1e-5 and rel(dBt.cpu().numpy(), 2 * o["dBt"]) <= 1e-5
+
+
+def test_layer_c1_full(B):
+    """BASELINE.json configs[0] in full: M=256, K=N=3072, r_s=32, r=16, seed 0."""
+    seed, M, K, N, r_s, r, kind = synth.CONFIGS["C1"]
+    d, R, D_f, U_f, L = make_layer(B, seed, M, K, N, r_s, r, kind)
+    out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
+    check_layer(B, d, R, D_f, U_f, out, r_s, r)
+
+
+@pytest.mark.parametrize("name", ["C2", "C3u", "C3d"])
+def test_layer_full_size_sampled(B, name):
+    """BASELINE.json configs[1..2] at full size in the launch configuration bench.py times:
+    codes/scales compared in full, outputs on sampled rows spanning tiles and the ragged ends
+    (rows of Y / dX depend only on their own row of X / G and the tensor amax).  The weight
+    split uses a cheap randomized range finder instead of a full SVD: any L1, L2 is a valid
+    stabilizer for parity purposes (the oracle receives the same R, L1, L2)."""
+    seed, M, K, N, r_s, r, kind = synth.CONFIGS[name]
+    d = synth.layer_inputs(seed, M, K, N, r, kind)
+    rng = synth.make_rng(seed + 100)
+    W = d["W"].astype(np.float64)
+    Qb, _ = np.linalg.qr(W @ rng.standard_normal((K, r_s)))          # N x r_s
+    L2 = nvfp4.bf16_round_from_f64(Qb.T)                              # r_s x N
+    L1 = nvfp4.bf16_round_from_f64((Qb.T @ W).T)                      # K x r_s
+    R = nvfp4.bf16_round_from_f64(W - (L1.astype(np.float64) @ L2.astype(np.float64)).T)
+    D_f = np.concatenate([L1, d["A"]], 1).astype(np.float32)
+    U_f = np.concatenate([L2, d["B"]], 0).astype(np.float32)
+    L = B.Layer(t16(R), t16(D_f), t16(U_f.T), r_s, r)
+    out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
+    rows = np.array(sorted({0, 1, 127, 128, 129, 1000, 2047, 2048, 3333, M - 129, M - 2, M - 1}))
+    check_layer(B, d, R, D_f, U_f, out, r_s, r, rows=rows)
+    # wgrad on sampled output rows: dA[k, :] = X[:, k]^T P_lora, dB[:, n] = H_lora^T G[:, n]
+    ks = np.array([0, 1, 63, 64, 777, K - 1]); ns = np.array([0, 5, 127, 128, 2000, N - 1])
+    Pl = out["p"][:, r_s:].astype(np.float64); Hl = out["h"][:, r_s:].astype(np.float64)
+    assert rel(out["dA"][ks], d["X"][:, ks].astype(np.float64).T @ Pl) <= TOL
+    assert rel(out["dBt"][ns], d["dY"][:, ns].astype(np.float64).T @ Hl) <= TOL
