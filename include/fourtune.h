@@ -165,7 +165,8 @@ size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t);
 const char* ft_error_string(int status);
 int ft_last_cuda_error(void); /* cudaError_t / CUresult of the last FT_ERR_CUDA, thread-local */
 int ft_version(void);
-/* test / bench hook: force the N-tile of the 4-bit GEMM (128, 192, 256; 0 = library default) */
+/* test / bench hook: 0 = default (CTA-pair 256x256 kernel); 128, 192, 256 = the 1-CTA kernel
+ * with that N tile */
 int ft_debug_set_gemm_tile_n(int bn);
 
 #ifdef __cplusplus

@@ -18,6 +18,8 @@ int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* r
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
                  const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16,
                  cudaStream_t st);
+int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
+                      const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st);
 int launch_wgrad(const void* in_bf16, int64_t M, int64_t F, const void* lr_bf16, int r_t, int r_s,
                  int r, float* out, cudaStream_t st);
 
@@ -70,8 +72,9 @@ int make_tensor_map_2d(CUtensorMap* map, const void* base, int elem_bytes, uint6
   if (sw == Swizzle::B32) s = CU_TENSOR_MAP_SWIZZLE_32B;
   if (sw == Swizzle::B64) s = CU_TENSOR_MAP_SWIZZLE_64B;
   if (sw == Swizzle::B128) s = CU_TENSOR_MAP_SWIZZLE_128B;
-  const CUtensorMapDataType dt =
-      elem_bytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8;
+  const CUtensorMapDataType dt = elem_bytes == 2   ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
+                                 : elem_bytes == 4 ? CU_TENSOR_MAP_DATA_TYPE_UINT32
+                                                   : CU_TENSOR_MAP_DATA_TYPE_UINT8;
   const CUresult r = g_encode(map, dt, 2, const_cast<void*>(base), dims, strides, box, estr,
                               CU_TENSOR_MAP_INTERLEAVE_NONE, s, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);

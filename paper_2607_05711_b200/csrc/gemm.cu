@@ -246,7 +246,9 @@ static int launch_gemm4_bn(const CUtensorMap& ma, const CUtensorMap& mb, const C
   return FT_OK;
 }
 
-int g_force_bn = 0;  // test/bench hook: 0 = heuristic
+int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
+                      const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st);
+int g_force_bn = 0;  // test/bench hook: 0 = CTA-pair kernel (default), else 1-CTA kernel with this N tile
 
 template <int BN>
 static int setup_and_launch(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
@@ -282,8 +284,8 @@ static int setup_and_launch(const ft_qtensor* a, const ft_qtensor* b, int64_t M,
 
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
                  const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st) {
-  int bn = g_force_bn;
-  if (bn == 0) bn = 128;
+  const int bn = g_force_bn;
+  if (bn == 0) return launch_gemm4_pair(a, b, M, N, K, lr_a_scaled, lr_b, r_t, out_bf16, st);
   if (bn == 256) return setup_and_launch<256>(a, b, M, N, K, lr_a_scaled, lr_b, r_t, out_bf16, st);
   if (bn == 192) return setup_and_launch<192>(a, b, M, N, K, lr_a_scaled, lr_b, r_t, out_bf16, st);
   return setup_and_launch<128>(a, b, M, N, K, lr_a_scaled, lr_b, r_t, out_bf16, st);

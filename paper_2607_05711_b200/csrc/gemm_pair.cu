@@ -1,0 +1,270 @@
+// gemm_pair.cu -- a2 / a4 on CTA pairs: the same computation as gemm.cu,
+//     out = bf16( alpha * ( GEMM4(a, b) + Hs * U^T ) ),
+// with tcgen05.mma.cta_group::2: the two CTAs of a cluster (2,1,1) own one 256 x 256 output
+// tile.  Each CTA stages its own 128 rows of A and its own 128-row half of B, so a CTA pulls
+// 256 operand rows from L2 per 128 x 256 of output (the 1-CTA kernel pulls 256 rows per
+// 128 x 128) -- the kernel is bound by L2 -> SM bandwidth, not by the tensor pipe (DESIGN.md
+// section 6), and this halves the bytes per MAC.
+//
+//   warp 0   : TMA producer (both CTAs; completion bytes land on the LEADER's full barrier)
+//   warp 1   : tcgen05 issuer (leader CTA only): tcgen05.cp of the scale tiles, MMAs, commits
+//              multicast to both CTAs' barriers
+//   warp 2   : TMEM allocator (cta_group::2, both CTAs)
+//   warps 4-7: epilogue of this CTA's 128 rows: tcgen05.ld, * alpha, bf16, swizzled smem, TMA store
+// TMEM: one 256-column fp32 accumulator + 48 columns of scale factors.  The accumulator is
+// single-buffered; while the epilogue drains it the producer keeps refilling the 5-stage ring.
+#include "common.cuh"
+
+namespace ft {
+
+constexpr int P_BM = 256;              // pair tile rows (128 per CTA)
+constexpr int P_BN = 256;              // pair tile columns (B: 128 rows staged per CTA)
+constexpr int P_THREADS = 256;
+constexpr int P_A_BYTES = 128 * 128;   // 128 rows x 256 fp4 (or 64 bf16)
+constexpr int P_B_BYTES = 128 * 128;
+constexpr int P_SFA_BYTES = 4 * 512;   // this CTA's 128 rows, four K=64 steps
+constexpr int P_SFB_BYTES = 2 * 4 * 512;  // all 256 columns of the tile
+constexpr int P_STAGE_BYTES = P_A_BYTES + P_B_BYTES + P_SFA_BYTES + P_SFB_BYTES;  // 38 KB
+constexpr int P_STAGES = 5;
+constexpr int P_OUT_BYTES = 128 * 128;     // one staged output box: 128 rows x 64 bf16
+constexpr int P_SMEM = P_STAGES * P_STAGE_BYTES + 2 * P_OUT_BYTES + 1024;
+constexpr int P_SF_COL = 256;
+
+struct PairParams {
+  int64_t M, N, K;
+  int r_t;
+  const float* g_dec_a;
+  const float* g_dec_b;
+  __nv_bfloat16* out;
+};
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(P_THREADS, 1)
+k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ CUtensorMap map_b,
+             const __grid_constant__ CUtensorMap map_sfa, const __grid_constant__ CUtensorMap map_sfb,
+             const __grid_constant__ CUtensorMap map_h, const __grid_constant__ CUtensorMap map_u,
+             const __grid_constant__ CUtensorMap map_out, const PairParams p) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  __shared__ uint64_t full_bar[P_STAGES], empty_bar[P_STAGES];
+  __shared__ uint64_t acc_full, acc_empty;
+  __shared__ uint32_t tmem_base_s;
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();
+  const bool leader = rank == 0;
+  const int64_t tiles_m = (p.M + P_BM - 1) / P_BM, tiles_n = (p.N + P_BN - 1) / P_BN;
+  const int64_t n_tiles = tiles_m * tiles_n;
+  const int64_t pair_id = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
+  const int k4 = (int)((p.K + 255) / 256);
+  const int klr = (p.r_t + 63) / 64;
+  const int kiters = k4 + klr;
+  const int64_t sf_tiles_k = p.K / 64;
+
+  if (threadIdx.x == 0) {
+    prefetch_tmap(&map_a);
+    prefetch_tmap(&map_b);
+    prefetch_tmap(&map_sfa);
+    prefetch_tmap(&map_sfb);
+    for (int s = 0; s < P_STAGES; ++s) {
+      mbar_init(&full_bar[s], 1);   // leader's producer arrives once (with the pair's byte count)
+      mbar_init(&empty_bar[s], 1);  // one multicast commit per use
+    }
+    mbar_init(&acc_full, 1);
+    mbar_init(&acc_empty, 8);       // 4 epilogue warps x 2 CTAs (used in the leader only)
+    fence_mbar_init();
+  }
+  if (warp == 2) {
+    tmem_alloc2(&tmem_base_s, 512);
+    tmem_relinquish2();
+  }
+  tc_fence_before();
+  cluster_sync();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
+
+  if (warp == 0) {
+    // ===================================================== TMA producer (both CTAs)
+    if (elect_one()) {
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs) {
+        const int64_t mt = tile % tiles_m, nt = tile / tiles_m;
+        const int32_t m0 = (int32_t)(mt * P_BM + rank * 128);   // this CTA's rows of A
+        const int32_t nb0 = (int32_t)(nt * P_BN + rank * 128);  // this CTA's half of B
+        const int64_t sfa_rt = mt * 2 + rank, sfb_rt = nt * 2;
+        for (int kt = 0; kt < kiters; ++kt) {
+          mbar_wait(&empty_bar[stage], phase ^ 1);
+          uint8_t* sa = smem + stage * P_STAGE_BYTES;
+          uint8_t* sb = sa + P_A_BYTES;
+          const uint32_t bar = map_to_cta(smem_u32(&full_bar[stage]), 0);  // the leader's barrier
+          if (kt < k4) {
+            if (leader) mbar_expect_tx(&full_bar[stage], 2 * P_STAGE_BYTES);
+            tma_load_2d_pair(sa, &map_a, bar, kt * 128, m0);
+            tma_load_2d_pair(sb, &map_b, bar, kt * 128, nb0);
+            uint8_t* ssfa = sb + P_B_BYTES;
+            uint8_t* ssfb = ssfa + P_SFA_BYTES;
+            tma_load_2d_pair(ssfa, &map_sfa, bar, 0, (int32_t)(sfa_rt * sf_tiles_k + kt * 4));
+            tma_load_2d_pair(ssfb, &map_sfb, bar, 0, (int32_t)(sfb_rt * sf_tiles_k + kt * 4));
+            tma_load_2d_pair(ssfb + 2048, &map_sfb, bar, 0, (int32_t)((sfb_rt + 1) * sf_tiles_k + kt * 4));
+          } else {
+            const int c0 = (kt - k4) * 64;
+            if (leader) mbar_expect_tx(&full_bar[stage], 2 * (P_A_BYTES + P_B_BYTES));
+            tma_load_2d_pair(sa, &map_h, bar, c0, m0);
+            tma_load_2d_pair(sb, &map_u, bar, c0, nb0);
+          }
+          if (++stage == P_STAGES) {
+            stage = 0;
+            phase ^= 1;
+          }
+        }
+      }
+    }
+  } else if (warp == 1 && leader) {
+    // ===================================================== MMA issuer (leader only)
+    if (elect_one()) {
+      constexpr uint32_t idesc4 = idesc_nvf4(P_BM, P_BN);
+      constexpr uint32_t idesc16 = idesc_bf16(P_BM, P_BN);
+      const uint32_t sfa_t = tmem_base + P_SF_COL;       // 16 columns
+      const uint32_t sfb_t = tmem_base + P_SF_COL + 16;  // 32 columns
+      int stage = 0;
+      uint32_t phase = 0, acc_phase = 0;
+      for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs) {
+        mbar_wait(&acc_empty, acc_phase ^ 1);
+        tc_fence_after();
+        for (int kt = 0; kt < kiters; ++kt) {
+          mbar_wait(&full_bar[stage], phase);
+          tc_fence_after();
+          const uint32_t sa = smem_u32(smem + stage * P_STAGE_BYTES);
+          const uint32_t sb = sa + P_A_BYTES;
+          if (kt < k4) {
+            const int nk = (int)min((int64_t)4, sf_tiles_k - (int64_t)kt * 4);
+            const uint32_t ssfa = sb + P_B_BYTES, ssfb = ssfa + P_SFA_BYTES;
+            for (int k = 0; k < nk; ++k) {
+              tc_cp_sf_pair(sfa_t + 4 * k, make_smem_desc(ssfa + k * 512, 128, 0, 0));
+              tc_cp_sf_pair(sfb_t + 8 * k, make_smem_desc(ssfb + k * 512, 128, 0, 0));
+              tc_cp_sf_pair(sfb_t + 8 * k + 4, make_smem_desc(ssfb + 2048 + k * 512, 128, 0, 0));
+            }
+            for (int k = 0; k < nk; ++k)
+              mma_nvf4_pair(tmem_base, make_smem_desc(sa + k * 32, 1024, 0, 2),
+                            make_smem_desc(sb + k * 32, 1024, 0, 2), idesc4, sfa_t + 4 * k, sfb_t + 8 * k,
+                            (kt | k) != 0);
+          } else {
+            const int cols = min(64, p.r_t - (kt - k4) * 64);
+            for (int k = 0; k < cols / 16; ++k)
+              mma_bf16_pair(tmem_base, make_smem_desc(sa + k * 32, 1024, 0, 2),
+                            make_smem_desc(sb + k * 32, 1024, 0, 2), idesc16, 1u);
+          }
+          tc_commit_pair(&empty_bar[stage], 3);            // frees the slot in both CTAs
+          if (kt == kiters - 1) tc_commit_pair(&acc_full, 3);
+          if (++stage == P_STAGES) {
+            stage = 0;
+            phase ^= 1;
+          }
+        }
+        acc_phase ^= 1;
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================================================== epilogue (both CTAs, own 128 rows)
+    // TMEM -> registers -> swizzled shared memory -> TMA store, 64 columns at a time through
+    // two 16 KB staging boxes; the accumulator is released as soon as it is in registers.
+    const int q = warp - 4;
+    const int et = threadIdx.x - 128;          // 0..127 = row of this CTA's half tile
+    const float alpha = __fmul_rn(__ldg(p.g_dec_a), __ldg(p.g_dec_b));
+    const uint32_t leader_acc_empty = map_to_cta(smem_u32(&acc_empty), 0);
+    uint8_t* stage_out = smem + P_STAGES * P_STAGE_BYTES;
+    uint32_t acc_phase = 0;
+    for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs) {
+      const int64_t mt = tile % tiles_m, nt = tile / tiles_m;
+      const int32_t row0 = (int32_t)(mt * P_BM + rank * 128);
+      const int32_t n0 = (int32_t)(nt * P_BN);
+      mbar_wait(&acc_full, acc_phase);
+      tc_fence_after();
+      const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16);
+#pragma unroll 1
+      for (int c = 0; c < P_BN / 64; ++c) {
+        uint32_t v[64];
+        tmem_ld32(t0 + c * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
+        tmem_ld32(t0 + c * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
+        tmem_ld_wait();
+        if (c == P_BN / 64 - 1) {   // accumulator fully in registers: hand it back to the MMA warp
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(leader_acc_empty);
+        }
+        uint8_t* buf = stage_out + (c & 1) * P_OUT_BYTES;
+        if (et == 0) tma_store_wait_read<1>();   // the store that last used this box has read it
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        uint8_t* rowp = buf + et * 128;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          uint4 o;
+          o.x = pack_bf16x2(__uint_as_float(v[8 * j + 0]) * alpha, __uint_as_float(v[8 * j + 1]) * alpha);
+          o.y = pack_bf16x2(__uint_as_float(v[8 * j + 2]) * alpha, __uint_as_float(v[8 * j + 3]) * alpha);
+          o.z = pack_bf16x2(__uint_as_float(v[8 * j + 4]) * alpha, __uint_as_float(v[8 * j + 5]) * alpha);
+          o.w = pack_bf16x2(__uint_as_float(v[8 * j + 6]) * alpha, __uint_as_float(v[8 * j + 7]) * alpha);
+          *reinterpret_cast<uint4*>(rowp + ((j ^ (et & 7)) << 4)) = o;
+        }
+        fence_proxy_async();
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (et == 0) {
+          tma_store_2d(&map_out, buf, n0 + c * 64, row0);
+          tma_store_commit();
+        }
+      }
+      acc_phase ^= 1;
+    }
+    if (et == 0) tma_store_wait<0>();
+  }
+
+  tc_fence_before();
+  cluster_sync();   // no CTA of the pair exits (or frees TMEM) while its peer still uses it
+  if (warp == 2) {
+    tc_fence_after();
+    tmem_dealloc2(tmem_base, 512);
+  }
+}
+
+int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
+                      const void* lr_a, const void* lr_b, int r_t, void* out, cudaStream_t st) {
+  CUtensorMap ma, mb, msa, msb, mh, mu, mo;
+  int rc = make_tensor_map_2d(&ma, a->codes, 1, (uint64_t)K / 2, (uint64_t)M, (uint64_t)K / 2, 128, 128,
+                              Swizzle::B128);
+  if (rc != FT_OK) return rc;
+  rc = make_tensor_map_2d(&mb, b->codes, 1, (uint64_t)K / 2, (uint64_t)N, (uint64_t)K / 2, 128, 128, Swizzle::B128);
+  if (rc != FT_OK) return rc;
+  // scale tiles: [row_tiles * K/64] tiles of 512 bytes = 128 uint32; one box = four K=64 steps
+  const uint64_t tk = (uint64_t)K / 64;
+  rc = make_tensor_map_2d(&msa, a->sf, 4, 128, (uint64_t)ceil_div(M, 128) * tk, 512, 128, 4, Swizzle::None);
+  if (rc != FT_OK) return rc;
+  rc = make_tensor_map_2d(&msb, b->sf, 4, 128, (uint64_t)ceil_div(N, 128) * tk, 512, 128, 4, Swizzle::None);
+  if (rc != FT_OK) return rc;
+  if (r_t > 0) {
+    rc = make_tensor_map_2d(&mh, lr_a, 2, (uint64_t)r_t, (uint64_t)M, (uint64_t)r_t * 2, 64, 128, Swizzle::B128);
+    if (rc != FT_OK) return rc;
+    rc = make_tensor_map_2d(&mu, lr_b, 2, (uint64_t)r_t, (uint64_t)N, (uint64_t)r_t * 2, 64, 128, Swizzle::B128);
+    if (rc != FT_OK) return rc;
+  } else {
+    mh = ma;
+    mu = mb;
+  }
+  rc = make_tensor_map_2d(&mo, out, 2, (uint64_t)N, (uint64_t)M, (uint64_t)N * 2, 64, 128, Swizzle::B128);
+  if (rc != FT_OK) return rc;
+  PairParams p;
+  p.M = M;
+  p.N = N;
+  p.K = K;
+  p.r_t = r_t;
+  p.g_dec_a = a->tensor_dec_scale;
+  p.g_dec_b = b->tensor_dec_scale;
+  p.out = reinterpret_cast<__nv_bfloat16*>(out);
+  FT_CUDA_TRY(cudaFuncSetAttribute(k_gemm4_pair, cudaFuncAttributeMaxDynamicSharedMemorySize, P_SMEM));
+  const int64_t n_tiles = ceil_div(M, P_BM) * ceil_div(N, P_BN);
+  const int64_t max_pairs = sm_count() / 2;
+  const unsigned grid = 2u * (unsigned)(n_tiles < max_pairs ? n_tiles : max_pairs);
+  k_gemm4_pair<<<grid, P_THREADS, P_SMEM, st>>>(ma, mb, msa, msb, mh, mu, mo, p);
+  FT_CUDA_TRY(cudaGetLastError());
+  return FT_OK;
+}
+
+}  // namespace ft
