@@ -83,6 +83,51 @@ __device__ __forceinline__ uint32_t quant_bf16x8(const uint4& v, float enc_b) {
   return f32x8_to_e2m1(f[0], f[1], f[2], f[3], f[4], f[5], f[6], f[7]);
 }
 
+// ---- leaner forms for the hot kernel (bit-identical results)
+// max |.| over eight bf16: max.xorsign.abs keeps max(|a|,|b|) in the magnitude bits
+__device__ __forceinline__ uint32_t absmax2_bf16(uint32_t a, uint32_t b) {
+  uint32_t d;
+  asm("max.xorsign.abs.bf16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
+  return d;
+}
+// amax of a 1x16 block held in two uint4; exact (bf16 magnitudes order like their bit patterns)
+__device__ __forceinline__ float amax_block16(const uint4& a, const uint4& b) {
+  uint32_t m = absmax2_bf16(absmax2_bf16(absmax2_bf16(a.x, a.y), absmax2_bf16(a.z, a.w)),
+                            absmax2_bf16(absmax2_bf16(b.x, b.y), absmax2_bf16(b.z, b.w)));
+  m &= 0x7FFF7FFFu;
+  const uint32_t best = max(m & 0xFFFFu, m >> 16);
+  return __uint_as_float(best << 16);
+}
+// two fp32 products with one instruction (each a single IEEE round-to-nearest multiply)
+__device__ __forceinline__ void mul2_rn(float& x0, float& x1, float s) {
+  uint64_t a, b, d;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(a) : "f"(x0), "f"(x1));
+  asm("mov.b64 %0, {%1, %1};" : "=l"(b) : "f"(s));
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(x0), "=f"(x1) : "l"(d));
+}
+__device__ __forceinline__ uint32_t quant_bf16x8_fast(const uint4& v, float enc_b) {
+  float f[8];
+  const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    f[2 * i] = __uint_as_float(w[i] << 16);
+    f[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+    mul2_rn(f[2 * i], f[2 * i + 1], enc_b);
+  }
+  return f32x8_to_e2m1(f[0], f[1], f[2], f[3], f[4], f[5], f[6], f[7]);
+}
+// enc_b of Q4 depends only on the scale byte and the tensor's g_dec: at most 127 values per
+// tensor.  Entry i of the table is computed with the same two IEEE operations.
+__device__ __forceinline__ float enc_of_sf8(uint32_t sf8, float g_dec) {
+  const float prod = __fmul_rn(e4m3_to_f32(sf8), g_dec);
+  return (sf8 == 0) ? 0.0f : __fdiv_rn(1.0f, prod);
+}
+__device__ __forceinline__ uint32_t block_sf8(float amax_b, float g_enc) {
+  float t = __fmul_rn(__fdiv_rn(amax_b, 6.0f), g_enc);
+  return f32_to_e4m3(fminf(t, 448.0f));
+}
+
 // byte offset of scale (row r, 16-wide block c) in FT_SF_TILE128x4 (include/fourtune.h)
 __host__ __device__ __forceinline__ int64_t sf_tile_offset(int64_t r, int64_t c, int64_t nblk) {
   const int64_t tiles_c = (nblk + 3) / 4;

@@ -4,13 +4,19 @@
 //
 // Decomposition: a CTA owns 128 rows x (cols / SPLIT) columns and walks them in
 // 128 x 64 chunks that TMA stages into shared memory (SWIZZLE_128B) through a
-// 4-deep mbarrier ring.  From one staged chunk
-//   - 256 threads quantize: thread (row = tid/2, half = tid%2) owns two 1x16 blocks;
-//   - 8 warps run mma.sync m16n8k16 (bf16 -> fp32) on their 16 rows against the
-//     64 x r_t slice of D staged beside it.
+// 3/4-deep mbarrier ring.  From one staged chunk
+//   - 512 threads quantize: thread (row = tid/4, quarter = tid%4) owns one 1x16 block;
+//   - one thread issues tcgen05.mma kind::f16 (M = 128, N = r_t, K = 16, four per chunk):
+//     A = the staged chunk itself (K-major, the TMA swizzle is the UMMA canonical layout),
+//     B = the 64 x r_t slice of D staged beside it (MN-major), accumulator in tensor memory.
+//     The staged bytes are read once by the tensor core instead of once per warp by ldmatrix.
+// Two CTAs are resident per SM (32 warps): the per-block scale arithmetic is a long
+// dependent chain (three IEEE divisions) and needs the warps to hide its latency.
 // The SPLIT CTAs of a 128-row tile form a thread-block cluster (1, SPLIT, 1); their
 // fp32 partial H tiles are summed through distributed shared memory, so H is
 // complete in one pass with no atomics and no second kernel.
+#include <cstdlib>
+
 #include "common.cuh"
 #include "quant_math.cuh"
 
@@ -18,8 +24,7 @@ namespace ft {
 
 constexpr int QF_ROWS = 128;    // rows per CTA
 constexpr int QF_KC = 64;       // columns per chunk (128 bytes of bf16 = one swizzle row)
-constexpr int QF_STAGES = 4;
-constexpr int QF_THREADS = 256;
+constexpr int QF_THREADS = 512;
 constexpr int QF_X_BYTES = QF_ROWS * QF_KC * 2;  // 16 KB
 constexpr int QF_DG_BYTES = QF_KC * 128;         // one 64-column group of D: 8 KB
 
@@ -68,38 +73,62 @@ __device__ __forceinline__ float ld_dsmem_f32(uint32_t local_addr, uint32_t cta_
   return v;
 }
 
+__device__ __forceinline__ float2 ld_dsmem_f32x2(uint32_t local_addr, uint32_t cta_rank) {
+  uint32_t remote;
+  float2 v;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(cta_rank));
+  asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(remote));
+  return v;
+}
+
 // R_T: width of the projection (0 = quantize only).  NG = 64-column groups of D.
 template <int R_T>
-__global__ void __launch_bounds__(QF_THREADS, 1)
+__global__ void __launch_bounds__(QF_THREADS, 2)
 k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constant__ CUtensorMap map_d,
                  const QFParams p) {
   constexpr int NG = (R_T + 63) / 64;
-  constexpr int NT = R_T / 8;
+  constexpr uint32_t TMEM_COLS = R_T <= 32 ? 32 : (R_T <= 64 ? 64 : 128);
+  constexpr int QF_STAGES = (NG == 2) ? 3 : 4;
   constexpr int STAGE_BYTES = QF_X_BYTES + NG * QF_DG_BYTES;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   // 1024-byte alignment for the 128-byte swizzle atoms
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  __shared__ uint64_t full_bar[QF_STAGES];
+  __shared__ uint64_t full_bar[4], empty_bar[4];
+  __shared__ float enc_tab[128];
+  __shared__ uint64_t acc_bar;
+  __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t row0 = (int64_t)blockIdx.x * QF_ROWS;
   const int split = p.split;
   const int64_t chunks_total = p.cols / QF_KC;
   const int n_chunks = (int)(chunks_total / split);
-  const int64_t chunk0 = (int64_t)blockIdx.y * n_chunks;
+  // chunk `it` of this CTA is global chunk it * split + blockIdx.y: the CTAs of a cluster walk
+  // the columns interleaved, so together they touch split * 128 contiguous bytes of each row at
+  // about the same time (DRAM page locality) instead of `split` far-apart 128-byte pieces.
 
   if (tid == 0) {
     prefetch_tmap(&map_x);
     if (R_T > 0) prefetch_tmap(&map_d);
-    for (int s = 0; s < QF_STAGES; ++s) mbar_init(&full_bar[s], 1);
+    for (int s = 0; s < QF_STAGES; ++s) {
+      mbar_init(&full_bar[s], 1);
+      mbar_init(&empty_bar[s], QF_THREADS / 32 + (R_T > 0 ? 1 : 0));  // every warp (+ the MMA commit)
+    }
+    mbar_init(&acc_bar, 1);
     fence_mbar_init();
   }
+  if (R_T > 0 && warp == 2) {
+    tmem_alloc(&tmem_base_s, TMEM_COLS);
+    tmem_relinquish();
+  }
+  tc_fence_before();
   __syncthreads();
+  tc_fence_after();
 
   auto issue = [&](int it) {
     const int s = it % QF_STAGES;
     uint8_t* base = smem + s * STAGE_BYTES;
-    const int32_t kcol = (int32_t)((chunk0 + it) * QF_KC);
+    const int32_t kcol = (int32_t)(((int64_t)it * split + blockIdx.y) * QF_KC);
     mbar_expect_tx(&full_bar[s], STAGE_BYTES);
     tma_load_2d(base, &map_x, &full_bar[s], kcol, (int32_t)row0);
 #pragma unroll
@@ -112,94 +141,109 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
 
   const TensorScale ts = tensor_scale(__ldg(p.amax_t));
   if (blockIdx.x == 0 && blockIdx.y == 0 && tid == 0) *p.g_dec_out = ts.g_dec;
+  if (tid < 128) enc_tab[tid] = enc_of_sf8((uint32_t)tid, ts.g_dec);
+  __syncthreads();
 
   // quantizer role of this thread
-  const int q_row = tid >> 1, q_half = tid & 1;
+  const int q_row = tid >> 2, q_quarter = tid & 3;
   const int64_t q_grow = row0 + q_row;
   const bool q_live = q_grow < p.rows;
   const int64_t nblk = p.cols / 16;
-  // projection role: warp -> rows 16*warp .. +15
-  float acc[NT > 0 ? NT : 1][4];
-#pragma unroll
-  for (int j = 0; j < (NT > 0 ? NT : 1); ++j) acc[j][0] = acc[j][1] = acc[j][2] = acc[j][3] = 0.f;
-
+  const uint32_t q_smem_base = smem_u32(smem) + q_row * 128;
+  const uint32_t q_smem_off0 = q_smem_base + (((q_quarter * 2) ^ (q_row & 7)) << 4);
+  const uint32_t q_smem_off1 = q_smem_base + (((q_quarter * 2 + 1) ^ (q_row & 7)) << 4);
+  // output cursors: chunk `it` is global chunk it * split + blockIdx.y
+  uint8_t* q_codes = p.codes + q_grow * (p.cols / 2) + ((int64_t)blockIdx.y * QF_KC + q_quarter * 16) / 2;
+  const int64_t q_codes_step = (int64_t)split * (QF_KC / 2);
+  uint8_t* q_sf = p.sf + ((p.sf_layout == FT_SF_TILE128x4) ? sf_tile_offset(q_grow, (int64_t)blockIdx.y * 4, nblk)
+                                                           : q_grow * nblk + (int64_t)blockIdx.y * 4);
+  const int64_t q_sf_step = (p.sf_layout == FT_SF_TILE128x4) ? (int64_t)split * 512 : (int64_t)split * 4;
   for (int it = 0; it < n_chunks; ++it) {
     const int s = it % QF_STAGES;
     const uint32_t parity = (it / QF_STAGES) & 1;
+    // refill, one iteration late: warp 0 re-arms the slot of chunk it-1 once every warp has
+    // released it; no block-wide barrier, so the other warps run ahead through the ring
+    if (warp == 0 && it > 0) {
+      if (lane == 0 && it - 1 + QF_STAGES < n_chunks) {
+        mbar_wait(&empty_bar[(it - 1) % QF_STAGES], ((it - 1) / QF_STAGES) & 1);
+        issue(it - 1 + QF_STAGES);
+      }
+      __syncwarp();
+    }
     mbar_wait(&full_bar[s], parity);
-    const uint8_t* xs = smem + s * STAGE_BYTES;
-    const int64_t kcol = (chunk0 + it) * QF_KC;
 
-    // ---- quantize two 1x16 blocks (32 elements = 4 x 16-byte chunks of this row)
+    // ---- quantize one 1x16 block (two 16-byte chunks of this row)
     {
-      const uint8_t* rowp = xs + q_row * 128;
-      const int sw = q_row & 7;
-      uint4 v[4];
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-        v[i] = *reinterpret_cast<const uint4*>(rowp + (((q_half * 4 + i) ^ sw) << 4));
-      uint32_t sf8a, sf8b;
-      float enca, encb;
-      block_scale(fmaxf(amax_bf16x8(v[0]), amax_bf16x8(v[1])), ts, sf8a, enca);
-      block_scale(fmaxf(amax_bf16x8(v[2]), amax_bf16x8(v[3])), ts, sf8b, encb);
-      uint4 c;
-      c.x = quant_bf16x8(v[0], enca);
-      c.y = quant_bf16x8(v[1], enca);
-      c.z = quant_bf16x8(v[2], encb);
-      c.w = quant_bf16x8(v[3], encb);
-      uint32_t sfpair = sf8a | (sf8b << 8);
-      const uint32_t other = __shfl_xor_sync(0xffffffffu, sfpair, 1);
+      uint4 v0, v1;
+      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                   : "=r"(v0.x), "=r"(v0.y), "=r"(v0.z), "=r"(v0.w) : "r"(q_smem_off0 + s * STAGE_BYTES));
+      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                   : "=r"(v1.x), "=r"(v1.y), "=r"(v1.z), "=r"(v1.w) : "r"(q_smem_off1 + s * STAGE_BYTES));
+      const uint32_t sf8 = block_sf8(amax_block16(v0, v1), ts.g_enc);
+      const float enc = enc_tab[sf8];
+      uint2 c;
+      c.x = quant_bf16x8_fast(v0, enc);
+      c.y = quant_bf16x8_fast(v1, enc);
+      // gather the row's four scale bytes into the quarter-0 lane
+      uint32_t w = sf8 << (8 * q_quarter);
+      w |= __shfl_xor_sync(0xffffffffu, w, 1);
+      w |= __shfl_xor_sync(0xffffffffu, w, 2);
       if (q_live) {
-        *reinterpret_cast<uint4*>(p.codes + q_grow * (p.cols / 2) + (kcol + q_half * 32) / 2) = c;
-        if (q_half == 0) {
-          const uint32_t word = sfpair | (other << 16);
-          const int64_t kb0 = kcol / 16;
-          const int64_t off = (p.sf_layout == FT_SF_TILE128x4) ? sf_tile_offset(q_grow, kb0, nblk)
-                                                               : q_grow * nblk + kb0;
-          *reinterpret_cast<uint32_t*>(p.sf + off) = word;
-        }
+        *reinterpret_cast<uint2*>(q_codes) = c;
+        if (q_quarter == 0) *reinterpret_cast<uint32_t*>(q_sf) = w;
       }
+      q_codes += q_codes_step;
+      q_sf += q_sf_step;
     }
 
-    // ---- projection: acc += X[16 rows, 64 k] * D[64 k, r_t]
+    // ---- projection: acc[128 x r_t] += X[128, 64 k] * D[64 k, r_t], issued by one thread
     if constexpr (R_T > 0) {
-      const uint32_t xs_u = smem_u32(xs);
-      const uint32_t ds_u = xs_u + QF_X_BYTES;
+      if (warp == 1) {
+        if (lane == 0) {
+          tc_fence_after();
+          const uint32_t xs_u = smem_u32(smem) + s * STAGE_BYTES;
+          const uint32_t ds_u = xs_u + QF_X_BYTES;
+          constexpr uint32_t idesc = idesc_bf16(QF_ROWS, R_T) | (1u << 16);  // B is MN-major
 #pragma unroll
-      for (int ks = 0; ks < 4; ++ks) {
-        uint32_t a0, a1, a2, a3;
-        {
-          const int r = warp * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
-          const int c = ks * 2 + (lane >> 4);
-          ldsm_x4(xs_u + r * 128 + ((c ^ (r & 7)) << 4), a0, a1, a2, a3);
+          for (int k = 0; k < 4; ++k)
+            mma_bf16(tmem_base_s, make_smem_desc(xs_u + k * 32, 1024, 0, 2),
+                     make_smem_desc(ds_u + k * 2048, 1024, QF_DG_BYTES, 2), idesc, (it | k) != 0);
+          tc_commit(&empty_bar[s]);                       // slot free once the MMAs have read it
+          if (it == n_chunks - 1) tc_commit(&acc_bar);    // accumulator complete
         }
-#pragma unroll
-        for (int j = 0; j < NT; j += 2) {
-          const int kr = ks * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
-          const int nt = j + (lane >> 4);
-          uint32_t b0, b1, b2, b3;
-          ldsm_x4_t(ds_u + (nt >> 3) * QF_DG_BYTES + kr * 128 + (((nt & 7) ^ (kr & 7)) << 4), b0, b1,
-                    b2, b3);
-          mma_16816(acc[j], a0, a1, a2, a3, b0, b1);
-          if (j + 1 < NT) mma_16816(acc[j + 1], a0, a1, a2, a3, b2, b3);
-        }
+        __syncwarp();
       }
     }
-    __syncthreads();  // every thread is done with stage s
-    if (tid == 0 && it + QF_STAGES < n_chunks) issue(it + QF_STAGES);
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty_bar[s]);  // this warp is done with stage s
   }
+  __syncthreads();  // every warp has consumed every stage: the ring can be reused below
 
   // ---- cluster reduction of the partial H tiles and output
   if constexpr (R_T > 0) {
     float* part = reinterpret_cast<float*>(smem);  // [128][R_T] fp32, reuses the ring
-    {
-      const int g = lane >> 2, t = lane & 3;
+    if (warp < 4) {   // warp w may read TMEM lanes 32w .. 32w+31 = rows of the tile
+      mbar_wait(&acc_bar, 0);
+      tc_fence_after();
+      const int r = warp * 32 + lane;
 #pragma unroll
-      for (int j = 0; j < NT; ++j) {
-        const int r = warp * 16 + g, c = j * 8 + 2 * t;
-        *reinterpret_cast<float2*>(part + r * R_T + c) = make_float2(acc[j][0], acc[j][1]);
-        *reinterpret_cast<float2*>(part + (r + 8) * R_T + c) = make_float2(acc[j][2], acc[j][3]);
+      for (int c0 = 0; c0 < R_T; c0 += 16) {
+        uint32_t v[16];
+        asm volatile(
+            "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+            "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+            : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+              "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+            : "r"(tmem_base_s + ((uint32_t)(warp * 32) << 16) + c0)
+            : "memory");
+        tmem_ld_wait();
+#pragma unroll
+        for (int j = 0; j < 16; j += 4)   // rotate the 16-byte pieces by row to spread the banks
+          *reinterpret_cast<uint4*>(part + r * R_T + c0 + ((j + 4 * (r & 3)) & 15)) =
+              make_uint4(v[(j + 4 * (r & 3)) & 15], v[(j + 4 * (r & 3) + 1) & 15], v[(j + 4 * (r & 3) + 2) & 15],
+                         v[(j + 4 * (r & 3) + 3) & 15]);
       }
+      tc_fence_before();
     }
     if (split > 1) cluster_sync_all(); else __syncthreads();
     const int rows_per = QF_ROWS / split;
@@ -211,10 +255,16 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       const int r = r_begin + e / (R_T / 2), c = (e % (R_T / 2)) * 2;
       float s0 = 0.f, s1 = 0.f;
       if (split > 1) {
-        for (int q = 0; q < split; ++q) {
-          s0 += ld_dsmem_f32(part_u + (r * R_T + c) * 4, q);
-          s1 += ld_dsmem_f32(part_u + (r * R_T + c + 1) * 4, q);
-        }
+        float2 v[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q)   // all remote loads in flight before the first add
+          if (q < split) v[q] = ld_dsmem_f32x2(part_u + (r * R_T + c) * 4, q);
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+          if (q < split) {
+            s0 += v[q].x;
+            s1 += v[q].y;
+          }
       } else {
         s0 = part[r * R_T + c];
         s1 = part[r * R_T + c + 1];
@@ -229,6 +279,10 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       }
     }
     if (split > 1) cluster_sync_all();  // keep this CTA's smem alive until all peers have read it
+    if (warp == 2) {
+      tc_fence_after();
+      tmem_dealloc(tmem_base_s, TMEM_COLS);
+    }
   }
 }
 
@@ -236,6 +290,7 @@ template <int R_T>
 static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, const QFParams& p,
                      cudaStream_t st) {
   constexpr int NG = (R_T + 63) / 64;
+  constexpr int QF_STAGES = (NG == 2) ? 3 : 4;
   const int smem = QF_STAGES * (QF_X_BYTES + NG * QF_DG_BYTES) + 1024;
   static_assert(QF_ROWS * (R_T > 0 ? R_T : 1) * 4 <= QF_STAGES * (QF_X_BYTES + NG * QF_DG_BYTES),
                 "partial H tile must fit in the ring");
@@ -257,15 +312,17 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, const QFParam
 }
 
 // choose the cluster size: smallest power of two <= 8 that divides the chunk count
-// and gives >= ~0.9 waves of CTAs, else the largest that divides.
+// and gives about two resident CTAs per SM (16 warps: the per-block scale arithmetic is a
+// long dependent chain and needs the extra warps to hide it), else the largest that divides.
 static int choose_split(int64_t rows, int64_t cols) {
+  if (const char* e = getenv("FT_QF_SPLIT")) { int v = atoi(e); if (v > 0 && (cols / QF_KC) % v == 0) return v; }
   const int64_t tiles = ceil_div(rows, QF_ROWS), chunks = cols / QF_KC;
   const int sms = sm_count();
   int best = 1;
   for (int s = 1; s <= 8; s *= 2) {
     if (chunks % s != 0) break;
     best = s;
-    if (tiles * s >= (int64_t)(0.9 * sms)) break;
+    if (tiles * s >= (int64_t)(1.8 * sms)) break;
   }
   return best;
 }
