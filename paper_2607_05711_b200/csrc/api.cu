@@ -285,7 +285,7 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   if (!L || !x_bf16 || !g_bf16 || !h_saved_bf16 || !p_saved_bf16 || !dA || !dBt)
     return FT_ERR_INVALID_ARG;
   const int r_t = L->r_s + L->r;
-  if (L->r_s < 0 || L->r <= 0 || !valid_rt(r_t) || L->r % 8 != 0 || L->r_s % 8 != 0)
+  if (L->r_s < 0 || L->r <= 0 || !valid_rt(r_t) || L->r % 16 != 0 || L->r_s % 8 != 0)
     return FT_ERR_UNSUPPORTED_SHAPE;
   if (M < 1 || L->K % 64 != 0 || L->N % 64 != 0) return FT_ERR_UNSUPPORTED_SHAPE;
   if (!aligned16(x_bf16) || !aligned16(g_bf16) || !aligned16(h_saved_bf16) ||

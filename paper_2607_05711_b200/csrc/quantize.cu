@@ -14,21 +14,22 @@ __global__ void __launch_bounds__(256) k_amax(const uint4* __restrict__ x, int64
                                               unsigned int* __restrict__ out_bits) {
   const uint32_t m = 0x7FFF7FFFu;
   uint32_t acc = 0;  // two 15-bit maxima packed; compared per half with vmax
-  const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  // 4 independent 16-byte loads in flight per thread
-  for (; i + 3 * stride < n_vec; i += 4 * stride) {
-    uint4 v0 = __ldg(x + i), v1 = __ldg(x + i + stride), v2 = __ldg(x + i + 2 * stride),
-          v3 = __ldg(x + i + 3 * stride);
-    uint32_t a = __vmaxu2(__vmaxu2(v0.x & m, v0.y & m), __vmaxu2(v0.z & m, v0.w & m));
-    uint32_t b = __vmaxu2(__vmaxu2(v1.x & m, v1.y & m), __vmaxu2(v1.z & m, v1.w & m));
-    uint32_t c = __vmaxu2(__vmaxu2(v2.x & m, v2.y & m), __vmaxu2(v2.z & m, v2.w & m));
-    uint32_t d = __vmaxu2(__vmaxu2(v3.x & m, v3.y & m), __vmaxu2(v3.z & m, v3.w & m));
-    acc = __vmaxu2(acc, __vmaxu2(__vmaxu2(a, b), __vmaxu2(c, d)));
-  }
-  for (; i < n_vec; i += stride) {
-    uint4 v = __ldg(x + i);
-    acc = __vmaxu2(acc, __vmaxu2(__vmaxu2(v.x & m, v.y & m), __vmaxu2(v.z & m, v.w & m)));
+  // a CTA walks 32 KB tiles (256 threads x 8 x 16 bytes); the 8 loads of a thread are issued
+  // back to back so 32 KB per CTA are in flight
+  const int64_t n_tiles = (n_vec + 2047) / 2048;
+  for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    const int64_t base = tile * 2048 + threadIdx.x;
+    uint4 v[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const int64_t i = base + j * 256;
+      v[j] = make_uint4(0, 0, 0, 0);
+      if (i < n_vec) asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                                  : "=r"(v[j].x), "=r"(v[j].y), "=r"(v[j].z), "=r"(v[j].w) : "l"(x + i));
+    }
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+      acc = __vmaxu2(acc, __vmaxu2(__vmaxu2(v[j].x & m, v[j].y & m), __vmaxu2(v[j].z & m, v[j].w & m)));
   }
   if (blockIdx.x == 0 && threadIdx.x < n_tail) acc = __vmaxu2(acc, (uint32_t)(tail[threadIdx.x] & 0x7FFF));
   uint32_t best = max(acc & 0xFFFFu, acc >> 16);
@@ -48,8 +49,8 @@ int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st)
   if (n == 0) return FT_OK;
   const int64_t n_vec = n / 8;
   const int n_tail = (int)(n % 8);
-  int64_t blocks = ceil_div(n_vec, 256 * 4);
-  const int64_t cap = (int64_t)sm_count() * 8;
+  int64_t blocks = ceil_div(n_vec, 2048);
+  const int64_t cap = (int64_t)sm_count() * 6;
   if (blocks > cap) blocks = cap;
   if (blocks < 1) blocks = 1;
   k_amax<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<const uint4*>(x_bf16), n_vec,

@@ -15,6 +15,7 @@
 // The SPLIT CTAs of a 128-row tile form a thread-block cluster (1, SPLIT, 1); their
 // fp32 partial H tiles are summed through distributed shared memory, so H is
 // complete in one pass with no atomics and no second kernel.
+#include <cstdio>
 #include <cstdlib>
 
 #include "common.cuh"
@@ -102,7 +103,7 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
   const int64_t row0 = (int64_t)blockIdx.x * QF_ROWS;
   const int split = p.split;
   const int64_t chunks_total = p.cols / QF_KC;
-  const int n_chunks = (int)(chunks_total / split);
+  const int n_chunks = (int)((chunks_total - blockIdx.y + split - 1) / split);  // interleaved, may be uneven
   // chunk `it` of this CTA is global chunk it * split + blockIdx.y: the CTAs of a cluster walk
   // the columns interleaved, so together they touch split * 128 contiguous bytes of each row at
   // about the same time (DRAM page locality) instead of `split` far-apart 128-byte pieces.
@@ -246,13 +247,14 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       tc_fence_before();
     }
     if (split > 1) cluster_sync_all(); else __syncthreads();
-    const int rows_per = QF_ROWS / split;
+    const int rows_per = (QF_ROWS + split - 1) / split;
     const int r_begin = (int)blockIdx.y * rows_per;
     float alpha = 1.0f;
     if (p.hs_out != nullptr) alpha = __fmul_rn(ts.g_dec, __ldg(p.other_dec_scale));
     const uint32_t part_u = smem_u32(part);
     for (int e = tid; e < rows_per * (R_T / 2); e += QF_THREADS) {
       const int r = r_begin + e / (R_T / 2), c = (e % (R_T / 2)) * 2;
+      if (r >= QF_ROWS) break;
       float s0 = 0.f, s1 = 0.f;
       if (split > 1) {
         float2 v[8];
@@ -287,7 +289,10 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
 }
 
 template <int R_T>
-static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, const QFParams& p,
+static int choose_split(int64_t rows, int64_t cols, int smem);
+
+template <int R_T>
+static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, const QFParams& p_in,
                      cudaStream_t st) {
   constexpr int NG = (R_T + 63) / 64;
   constexpr int QF_STAGES = (NG == 2) ? 3 : 4;
@@ -295,6 +300,10 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, const QFParam
   static_assert(QF_ROWS * (R_T > 0 ? R_T : 1) * 4 <= QF_STAGES * (QF_X_BYTES + NG * QF_DG_BYTES),
                 "partial H tile must fit in the ring");
   FT_CUDA_TRY(cudaFuncSetAttribute(k_quantize_fused<R_T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  FT_CUDA_TRY(cudaFuncSetAttribute(k_quantize_fused<R_T>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                   cudaSharedmemCarveoutMaxShared));
+  QFParams p = p_in;
+  p.split = choose_split<R_T>(p.rows, p.cols, smem);
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)ceil_div(p.rows, QF_ROWS), (unsigned)p.split, 1);
   cfg.blockDim = dim3(QF_THREADS, 1, 1);
@@ -311,18 +320,51 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, const QFParam
   return FT_OK;
 }
 
-// choose the cluster size: smallest power of two <= 8 that divides the chunk count
-// and gives about two resident CTAs per SM (16 warps: the per-block scale arithmetic is a
-// long dependent chain and needs the extra warps to hide it), else the largest that divides.
-static int choose_split(int64_t rows, int64_t cols) {
-  if (const char* e = getenv("FT_QF_SPLIT")) { int v = atoi(e); if (v > 0 && (cols / QF_KC) % v == 0) return v; }
+// Cluster size (= K split) of the fused kernel: any 1..8.  Clusters are co-scheduled inside a
+// GPC, so not every size packs the chip equally; ask the driver how many clusters of each size
+// fit at once and minimise  waves * chunks-per-CTA  (ties: the larger split = more warps).
+template <int R_T>
+static int choose_split(int64_t rows, int64_t cols, int smem) {
   const int64_t tiles = ceil_div(rows, QF_ROWS), chunks = cols / QF_KC;
-  const int sms = sm_count();
+  if (const char* e = getenv("FT_QF_SPLIT")) {
+    const int v = atoi(e);
+    if (v > 0 && v <= 8 && v <= chunks) return v;
+  }
+  static int max_active[9] = {0};   // per instantiation; device properties do not change
   int best = 1;
-  for (int s = 1; s <= 8; s *= 2) {
-    if (chunks % s != 0) break;
-    best = s;
-    if (tiles * s >= (int64_t)(1.8 * sms)) break;
+  double best_cost = 1e30;
+  for (int s = 1; s <= 8 && s <= chunks; ++s) {
+    if (max_active[s] == 0) {
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3(1, (unsigned)s, 1);
+      cfg.blockDim = dim3(QF_THREADS, 1, 1);
+      cfg.dynamicSmemBytes = smem;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeClusterDimension;
+      attr[0].val.clusterDim.x = 1;
+      attr[0].val.clusterDim.y = (unsigned)s;
+      attr[0].val.clusterDim.z = 1;
+      cfg.attrs = attr;
+      cfg.numAttrs = 1;
+      int n = 0;
+      if (cudaOccupancyMaxActiveClusters(&n, k_quantize_fused<R_T>, &cfg) != cudaSuccess || n < 1) {
+        (void)cudaGetLastError();
+        n = -1;
+      }
+      max_active[s] = n;
+    }
+    if (max_active[s] < 1) continue;
+    const double waves = (double)ceil_div(tiles, max_active[s]);
+    const double cost = waves * (double)ceil_div(chunks, s) + 1.5;   // + a fixed head/tail per CTA
+    if (cost <= best_cost) {
+      best_cost = cost;
+      best = s;
+    }
+  }
+  if (getenv("FT_QF_DEBUG")) {
+    fprintf(stderr, "[qf] r_t=%d rows=%ld cols=%ld split=%d max_active:", R_T, (long)rows, (long)cols, best);
+    for (int s = 1; s <= 8; ++s) fprintf(stderr, " %d", max_active[s]);
+    fprintf(stderr, "\n");
   }
   return best;
 }
@@ -352,7 +394,7 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
   p.h_out = proj ? reinterpret_cast<__nv_bfloat16*>(proj->out) : nullptr;
   p.hs_out = proj ? reinterpret_cast<__nv_bfloat16*>(proj->out_scaled) : nullptr;
   p.other_dec_scale = proj ? proj->other_dec_scale : nullptr;
-  p.split = choose_split(rows, cols);
+  p.split = 1;
   // padding rows of the last 128-row scale tile must read as zero
   if (out->sf_layout == FT_SF_TILE128x4 && rows % 128 != 0) {
     const int64_t tiles_c = ceil_div(cols / 16, 4);

@@ -1,10 +1,12 @@
 // wgrad.cu -- a5: LoRA weight gradients (Eq. 4)
 //     out[f, j] (+)= sum_m In[m, f] * L[m, r_s + j]        f < F, j < r
 // used twice: dA = X^T (G B^T) with In = X, L = P;  dB^T = G^T (X A) with In = G, L = H.
-// HBM-bound (reads In once).  A CTA owns 128 features x one slice of M and walks it in
-// 64-row chunks staged by TMA (SWIZZLE_128B, 4-deep ring); 8 warps x 16 features run
-// mma.sync m16n8k16 with A taken transposed from the staged chunk (ldmatrix.trans);
-// slices are combined with fp32 red.global.add.
+// HBM-bound: In is read exactly once.  A CTA owns 128 features x one slice of M and walks it in
+// 64-row chunks that TMA stages (SWIZZLE_128B) through an mbarrier ring.  One thread issues
+// tcgen05.mma kind::f16 (M = 128 features, N = r, K = 16 rows, four per chunk) with BOTH
+// operands MN-major -- the staged chunks are used as they lie in memory, nothing is transposed
+// by the SM -- into a TMEM accumulator; four warps drain it and combine the M slices with
+// fp32 vector red.global.add.
 #include "common.cuh"
 
 namespace ft {
@@ -12,7 +14,7 @@ namespace ft {
 constexpr int WG_F = 128;
 constexpr int WG_MC = 64;
 constexpr int WG_STAGES = 4;
-constexpr int WG_THREADS = 256;
+constexpr int WG_THREADS = 128;
 constexpr int WG_IN_BYTES = 2 * WG_MC * 128;  // two 64-feature boxes
 constexpr int WG_LG_BYTES = WG_MC * 128;      // one 64-column group of L
 
@@ -23,31 +25,22 @@ struct WgParams {
   float* out;
 };
 
-__device__ __forceinline__ void wg_ldsm_x4_t(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2,
-                                             uint32_t& r3) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];"
-               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
-               : "r"(addr));
-}
-__device__ __forceinline__ void wg_mma(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
-                                       uint32_t b0, uint32_t b1) {
-  asm volatile(
-      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, "
-      "{%8, %9}, {%0, %1, %2, %3};"
-      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
+__device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d)
+               : "memory");
 }
 
 template <int R>
-__global__ void __launch_bounds__(WG_THREADS, 1)
+__global__ void __launch_bounds__(WG_THREADS, 2)
 k_wgrad(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_l,
         const WgParams p) {
   constexpr int NG = (R + 63) / 64;
-  constexpr int NT = R / 8;
   constexpr int STAGE_BYTES = WG_IN_BYTES + NG * WG_LG_BYTES;
+  constexpr uint32_t TMEM_COLS = R <= 32 ? 32 : (R <= 64 ? 64 : 128);
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  __shared__ uint64_t full_bar[WG_STAGES];
+  __shared__ uint64_t full_bar[WG_STAGES], empty_bar[WG_STAGES], acc_bar;
+  __shared__ uint32_t tmem_base_s;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int32_t f0 = (int32_t)blockIdx.x * WG_F;
   const int64_t chunks_total = (p.M + WG_MC - 1) / WG_MC;
@@ -58,73 +51,86 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUte
   if (tid == 0) {
     prefetch_tmap(&map_in);
     prefetch_tmap(&map_l);
-    for (int s = 0; s < WG_STAGES; ++s) mbar_init(&full_bar[s], 1);
+    for (int s = 0; s < WG_STAGES; ++s) {
+      mbar_init(&full_bar[s], 1);
+      mbar_init(&empty_bar[s], 1);
+    }
+    mbar_init(&acc_bar, 1);
     fence_mbar_init();
   }
-  __syncthreads();
-  auto issue = [&](int it) {
-    const int s = it % WG_STAGES;
-    uint8_t* base = smem + s * STAGE_BYTES;
-    const int32_t m0 = (int32_t)((c_begin + it) * WG_MC);
-    mbar_expect_tx(&full_bar[s], STAGE_BYTES);
-    tma_load_2d(base, &map_in, &full_bar[s], f0, m0);
-    tma_load_2d(base + WG_MC * 128, &map_in, &full_bar[s], f0 + 64, m0);
-#pragma unroll
-    for (int g = 0; g < NG; ++g)
-      tma_load_2d(base + WG_IN_BYTES + g * WG_LG_BYTES, &map_l, &full_bar[s], p.r_s + g * 64, m0);
-  };
-  if (tid == 0)
-    for (int it = 0; it < WG_STAGES && it < n_chunks; ++it) issue(it);
-
-  float acc[NT][4];
-#pragma unroll
-  for (int j = 0; j < NT; ++j) acc[j][0] = acc[j][1] = acc[j][2] = acc[j][3] = 0.f;
-  // warp -> features [16*warp, 16*warp+16): box = warp / 4, 16-byte chunks 2*(warp%4), +1
-  const int box = warp >> 2, fc = (warp & 3) * 2;
-
-  for (int it = 0; it < n_chunks; ++it) {
-    const int s = it % WG_STAGES;
-    mbar_wait(&full_bar[s], (it / WG_STAGES) & 1);
-    const uint32_t in_u = smem_u32(smem + s * STAGE_BYTES) + box * (WG_MC * 128);
-    const uint32_t l_u = smem_u32(smem + s * STAGE_BYTES) + WG_IN_BYTES;
-#pragma unroll
-    for (int ks = 0; ks < 4; ++ks) {
-      uint32_t a0, a1, a2, a3;
-      {
-        const int i = lane >> 3;
-        const int mr = ks * 16 + (lane & 7) + (i >> 1) * 8;
-        const int c = fc + (i & 1);
-        wg_ldsm_x4_t(in_u + mr * 128 + ((c ^ (mr & 7)) << 4), a0, a1, a2, a3);
-      }
-#pragma unroll
-      for (int j = 0; j < NT; j += 2) {
-        const int kr = ks * 16 + (lane & 7) + ((lane >> 3) & 1) * 8;
-        const int nt = j + (lane >> 4);
-        uint32_t b0, b1, b2, b3;
-        wg_ldsm_x4_t(l_u + (nt >> 3) * WG_LG_BYTES + kr * 128 + (((nt & 7) ^ (kr & 7)) << 4), b0, b1, b2, b3);
-        wg_mma(acc[j], a0, a1, a2, a3, b0, b1);
-        if (j + 1 < NT) wg_mma(acc[j + 1], a0, a1, a2, a3, b2, b3);
-      }
-    }
-    __syncthreads();
-    if (tid == 0 && it + WG_STAGES < n_chunks) issue(it + WG_STAGES);
+  if (warp == 2) {
+    tmem_alloc(&tmem_base_s, TMEM_COLS);
+    tmem_relinquish();
   }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = tmem_base_s;
 
-  if (n_chunks > 0) {
-    const int g = lane >> 2, t = lane & 3;
-    const int64_t f = (int64_t)f0 + warp * 16 + g;
+  if (warp == 0) {
+    if (elect_one()) {   // ---- TMA producer
+      for (int it = 0; it < n_chunks; ++it) {
+        const int s = it % WG_STAGES;
+        mbar_wait(&empty_bar[s], ((it / WG_STAGES) & 1) ^ 1);
+        uint8_t* base = smem + s * STAGE_BYTES;
+        const int32_t m0 = (int32_t)((c_begin + it) * WG_MC);
+        mbar_expect_tx(&full_bar[s], STAGE_BYTES);
+        tma_load_2d(base, &map_in, &full_bar[s], f0, m0);
+        tma_load_2d(base + WG_MC * 128, &map_in, &full_bar[s], f0 + 64, m0);
 #pragma unroll
-    for (int j = 0; j < NT; ++j) {
-      const int c = j * 8 + 2 * t;
-      if (f < p.F) {
-        atomicAdd(p.out + f * R + c, acc[j][0]);
-        atomicAdd(p.out + f * R + c + 1, acc[j][1]);
-      }
-      if (f + 8 < p.F) {
-        atomicAdd(p.out + (f + 8) * R + c, acc[j][2]);
-        atomicAdd(p.out + (f + 8) * R + c + 1, acc[j][3]);
+        for (int g = 0; g < NG; ++g)
+          tma_load_2d(base + WG_IN_BYTES + g * WG_LG_BYTES, &map_l, &full_bar[s], p.r_s + g * 64, m0);
       }
     }
+  } else if (warp == 1) {
+    if (elect_one()) {   // ---- MMA issuer: acc[128 f x R] += In[64 m, 128 f]^T * L[64 m, R]
+      constexpr uint32_t idesc = idesc_bf16(WG_F, R) | (1u << 15) | (1u << 16);  // A and B MN-major
+      for (int it = 0; it < n_chunks; ++it) {
+        const int s = it % WG_STAGES;
+        mbar_wait(&full_bar[s], (it / WG_STAGES) & 1);
+        tc_fence_after();
+        const uint32_t in_u = smem_u32(smem + s * STAGE_BYTES);
+        const uint32_t l_u = in_u + WG_IN_BYTES;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)   // 16 rows of m per MMA = two 8-row swizzle groups = 2048 bytes
+          mma_bf16(tmem_base, make_smem_desc(in_u + k * 2048, 1024, WG_MC * 128, 2),
+                   make_smem_desc(l_u + k * 2048, 1024, WG_LG_BYTES, 2), idesc, (it | k) != 0);
+        tc_commit(&empty_bar[s]);
+      }
+      tc_commit(&acc_bar);
+    }
+  }
+  __syncwarp();
+
+  if (n_chunks > 0) {   // ---- drain: thread = feature (TMEM lane), R fp32 columns
+    mbar_wait(&acc_bar, 0);
+    tc_fence_after();
+    const int64_t f = (int64_t)f0 + warp * 32 + lane;
+#pragma unroll
+    for (int c0 = 0; c0 < R; c0 += 16) {
+      uint32_t v[16];
+      asm volatile(
+          "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+          "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+          : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+            "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+          : "r"(tmem_base + ((uint32_t)(warp * 32) << 16) + c0)
+          : "memory");
+      tmem_ld_wait();
+      if (f < p.F) {
+        float* o = p.out + f * R + c0;
+#pragma unroll
+        for (int j = 0; j < 16; j += 4)
+          red_add_v4(o + j, __uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]),
+                     __uint_as_float(v[j + 3]));
+      }
+    }
+    tc_fence_before();
+  }
+  __syncthreads();
+  if (warp == 2) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, TMEM_COLS);
   }
 }
 
@@ -150,7 +156,7 @@ int launch_wgrad(const void* in_bf16, int64_t M, int64_t F, const void* lr_bf16,
                           Swizzle::B128);
   if (rc != FT_OK) return rc;
   const int64_t f_tiles = ceil_div(F, WG_F), chunks = ceil_div(M, WG_MC);
-  // M slices: about two waves of CTAs, at least 4 chunks per slice
+  // M slices: about two resident CTAs per SM, at least 4 chunks per slice
   int64_t slices = ceil_div((int64_t)2 * sm_count(), f_tiles);
   if (slices > chunks / 4) slices = chunks / 4;
   if (slices < 1) slices = 1;
@@ -163,12 +169,13 @@ int launch_wgrad(const void* in_bf16, int64_t M, int64_t F, const void* lr_bf16,
   p.out = out;
   const unsigned gy = (unsigned)ceil_div(chunks, p.chunks_per_cta);
   switch (r) {
-    case 8: return launch_wg<8>(mi, ml, p, gy, st);
     case 16: return launch_wg<16>(mi, ml, p, gy, st);
     case 32: return launch_wg<32>(mi, ml, p, gy, st);
     case 48: return launch_wg<48>(mi, ml, p, gy, st);
     case 64: return launch_wg<64>(mi, ml, p, gy, st);
+    case 80: return launch_wg<80>(mi, ml, p, gy, st);
     case 96: return launch_wg<96>(mi, ml, p, gy, st);
+    case 112: return launch_wg<112>(mi, ml, p, gy, st);
     case 128: return launch_wg<128>(mi, ml, p, gy, st);
     default: return FT_ERR_UNSUPPORTED_SHAPE;
   }
