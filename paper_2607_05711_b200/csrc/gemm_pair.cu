@@ -10,24 +10,25 @@
 //   warp 1   : tcgen05 issuer (leader CTA only): tcgen05.cp of the scale tiles, MMAs, commits
 //              multicast to both CTAs' barriers
 //   warp 2   : TMEM allocator (cta_group::2, both CTAs)
-//   warps 4-7: epilogue of this CTA's 128 rows: tcgen05.ld, * alpha, bf16, swizzled smem, TMA store
+//   warps 4-11: epilogue of this CTA's 128 rows, two groups of four warps (one per 128-column half):
+//              tcgen05.ld, * alpha, bf16, swizzled smem, TMA store
 // TMEM: one 256-column fp32 accumulator + 48 columns of scale factors.  The accumulator is
-// single-buffered; while the epilogue drains it the producer keeps refilling the 5-stage ring.
+// single-buffered; while the epilogue drains it the producer keeps refilling the 4-stage ring.
 #include "common.cuh"
 
 namespace ft {
 
 constexpr int P_BM = 256;              // pair tile rows (128 per CTA)
 constexpr int P_BN = 256;              // pair tile columns (B: 128 rows staged per CTA)
-constexpr int P_THREADS = 256;
+constexpr int P_THREADS = 384;          // 4 control warps + 8 epilogue warps
 constexpr int P_A_BYTES = 128 * 128;   // 128 rows x 256 fp4 (or 64 bf16)
 constexpr int P_B_BYTES = 128 * 128;
 constexpr int P_SFA_BYTES = 4 * 512;   // this CTA's 128 rows, four K=64 steps
 constexpr int P_SFB_BYTES = 2 * 4 * 512;  // all 256 columns of the tile
 constexpr int P_STAGE_BYTES = P_A_BYTES + P_B_BYTES + P_SFA_BYTES + P_SFB_BYTES;  // 38 KB
-constexpr int P_STAGES = 5;
+constexpr int P_STAGES = 4;
 constexpr int P_OUT_BYTES = 128 * 128;     // one staged output box: 128 rows x 64 bf16
-constexpr int P_SMEM = P_STAGES * P_STAGE_BYTES + 2 * P_OUT_BYTES + 1024;
+constexpr int P_SMEM = P_STAGES * P_STAGE_BYTES + 4 * P_OUT_BYTES + 1024;
 constexpr int P_SF_COL = 256;
 
 struct PairParams {
@@ -70,7 +71,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
       mbar_init(&empty_bar[s], 1);  // one multicast commit per use
     }
     mbar_init(&acc_full, 1);
-    mbar_init(&acc_empty, 8);       // 4 epilogue warps x 2 CTAs (used in the leader only)
+    mbar_init(&acc_empty, 16);      // 8 epilogue warps x 2 CTAs (used in the leader only)
     fence_mbar_init();
   }
   if (warp == 2) {
@@ -166,35 +167,39 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
     }
   } else if (warp >= 4) {
     // ===================================================== epilogue (both CTAs, own 128 rows)
-    // TMEM -> registers -> swizzled shared memory -> TMA store, 64 columns at a time through
-    // two 16 KB staging boxes; the accumulator is released as soon as it is in registers.
-    const int q = warp - 4;
-    const int et = threadIdx.x - 128;          // 0..127 = row of this CTA's half tile
+    // TMEM -> registers -> swizzled shared memory -> TMA store.  Two groups of four warps, one
+    // per 128-column half of the accumulator (a warp may read the TMEM lane quarter warp % 4);
+    // each group moves two 64-column boxes through its own two 16 KB staging boxes.  The
+    // accumulator is released as soon as a warp has it in registers.
+    const int q = warp & 3;
+    const int half = (warp - 4) >> 2;
+    const int et = (threadIdx.x - 128) & 127;  // 0..127 = row of this CTA's half tile
     const float alpha = __fmul_rn(__ldg(p.g_dec_a), __ldg(p.g_dec_b));
     const uint32_t leader_acc_empty = map_to_cta(smem_u32(&acc_empty), 0);
-    uint8_t* stage_out = smem + P_STAGES * P_STAGE_BYTES;
+    uint8_t* stage_out = smem + P_STAGES * P_STAGE_BYTES + half * 2 * P_OUT_BYTES;
     uint32_t acc_phase = 0;
     for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs) {
       const int64_t mt = tile % tiles_m, nt = tile / tiles_m;
       const int32_t row0 = (int32_t)(mt * P_BM + rank * 128);
-      const int32_t n0 = (int32_t)(nt * P_BN);
+      const int32_t n0 = (int32_t)(nt * P_BN) + half * 128;
       mbar_wait(&acc_full, acc_phase);
       tc_fence_after();
-      const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16);
+      const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + half * 128;
 #pragma unroll 1
-      for (int c = 0; c < P_BN / 64; ++c) {
+      for (int c = 0; c < 2; ++c) {
         uint32_t v[64];
         tmem_ld32(t0 + c * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
         tmem_ld32(t0 + c * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
         tmem_ld_wait();
-        if (c == P_BN / 64 - 1) {   // accumulator fully in registers: hand it back to the MMA warp
+        if (c == 1) {   // this warp's part of the accumulator is in registers: hand it back
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster(leader_acc_empty);
         }
-        uint8_t* buf = stage_out + (c & 1) * P_OUT_BYTES;
+        uint8_t* buf = stage_out + c * P_OUT_BYTES;
         if (et == 0) tma_store_wait_read<1>();   // the store that last used this box has read it
-        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (half == 0) asm volatile("bar.sync 1, 128;" ::: "memory");
+        else asm volatile("bar.sync 2, 128;" ::: "memory");
         uint8_t* rowp = buf + et * 128;
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
@@ -206,7 +211,8 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
           *reinterpret_cast<uint4*>(rowp + ((j ^ (et & 7)) << 4)) = o;
         }
         fence_proxy_async();
-        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (half == 0) asm volatile("bar.sync 1, 128;" ::: "memory");
+        else asm volatile("bar.sync 2, 128;" ::: "memory");
         if (et == 0) {
           tma_store_2d(&map_out, buf, n0 + c * 64, row0);
           tma_store_commit();
