@@ -267,7 +267,8 @@ def run_ours(args):
     d2h = (yh.numel() + dxh.numel()) * 2 + (dAh.numel() + dBh.numel()) * 4
 
     # ---- per-kernel breakdown: each launch alone, CUDA events on its stream, L2 flushed between
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    flush = torch.zeros(256 << 20, dtype=torch.uint8, device=dev)
+    flush_sink = torch.zeros((), dtype=torch.uint8, device=dev)
     hs = ws[256:256 + M * r_t * 2].view(torch.bfloat16).view(M, r_t)
     amax = torch.empty(1, dtype=torch.float32, device=dev)
 
@@ -275,7 +276,8 @@ def run_ours(args):
         fn()
         tot = 0.0
         for _ in range(n):
-            flush.zero_()
+            flush_sink.copy_(flush.max())   # evict L2 with clean lines (a write flush would leave
+            #                                 126 MB of dirty lines to be written back under fn)
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a.record(stream)
             fn()
@@ -310,6 +312,10 @@ def run_ours(args):
         db = xa.t() @ G                               # noqa: F841
     bf16_us = timed(bf16_lora, n=10)
 
+    extra = {}
+    if rank == 0 and world == 1 and not args.no_sweep:
+        del yh, dxh
+        extra = sweep(B, prepare, dev, timed, peaks, full=args.sweep)
     out = None
     if rank == 0:
         gemm_us = 0.5 * (kern["gemm_fwd_us"] + kern["gemm_dgrad_us"])
@@ -323,7 +329,7 @@ def run_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "nvfp4 (e2m1 x ue4m3, fp32 accumulate) + bf16 low-rank", "data": "synthetic",
             "config": {"workload": w["name"], "M": M, "K": K, "N": N, "r_s": r_s, "r": r, "tokens_per_gpu": M,
-                       "launch": launch, "l2": "step working set ~330 MB > 126 MB L2; per-kernel timings flush L2",
+                       "launch": launch, "l2": "step working set ~330 MB > 126 MB L2; per-kernel timings evict L2 by reading 256 MB",
                        "parallelism": "dp%d (tokens), all-reduce of dA,dB only" % world,
                        "peaks": peaks["source"]},
             "clocks": clocks,
@@ -342,6 +348,7 @@ def run_ours(args):
                          "bytes_per_element": 2.5625, "hbm_peak_GBps": peaks["hbm"]},
             "bf16_lora_baseline": {"us_per_step": bf16_us, "speedup": bf16_us / (ms_per_step * 1e3),
                                    "how": "torch.matmul (cuBLAS) bf16, frozen W, same shapes, same GPU"},
+            **extra,
             "paper_context": "2.27x step time / 2.25x memory vs BF16 LoRA on RTX 5090 (PAPER.md:7,207); not the target",
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle",
                              "sample": "all 4608 tokens of C2, fwd+dgrad+wgrad, mean of 2 passes (%.1f s of CPU work)"
@@ -353,6 +360,131 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------ the other BASELINE.json configs
+def sweep(B, prepare, dev, timed, peaks, full=False):
+    """C4 (quantizer-only sweep; always) and, with --sweep, C1 / C3 / C5 layer timings.  Inputs are
+    torch-generated on the device with the configs' shapes (N(0,1) with 1 % channels x50; gradients
+    1e-3 N(0,1)): throughput does not depend on the values; parity on these shapes is in tests/."""
+    import torch
+    g = torch.Generator(device=dev)
+    g.manual_seed(3)
+
+    def acts(rows, cols, grad=False):
+        x = torch.randn(rows, cols, device=dev, generator=g)
+        if grad:
+            return (x * 1e-3).to(torch.bfloat16)
+        idx = torch.randperm(cols, device=dev, generator=g)[: max(1, cols // 100)]
+        x[:, idx] *= 50.0
+        return x.to(torch.bfloat16)
+
+    out = {}
+    c4 = []
+    for rows, cols in ((4608, 3072), (4608, 12288), (4608, 15360), (9216, 3072)):
+        x = acts(rows, cols)
+        q = B.QTensor(rows, cols, device=dev)
+        ws = torch.empty(B.ft_workspace_bytes(rows, cols, 0, 32), dtype=torch.uint8, device=dev)
+        amax = B.ft_tensor_amax(x)
+        d = (torch.randn(cols, 32, device=dev, generator=g) * 0.01).to(torch.bfloat16)
+        h = torch.empty(rows, 32, dtype=torch.bfloat16, device=dev)
+        t_a = timed(lambda: B.ft_tensor_amax(x, amax))
+        t_q = timed(lambda: B.ft_quantize_blockwise(x, q, tensor_amax=amax, workspace=ws))
+        t_p = timed(lambda: B.ft_quantize_blockwise(x, q, tensor_amax=amax, down=d, h_out=h, workspace=ws))
+        by = 2.5625 * rows * cols
+        c4.append({"shape": [rows, cols], "amax_us": round(t_a, 2), "amax_GBps": round(2.0 * rows * cols / t_a / 1e3),
+                   "quant_us": round(t_q, 2), "quant_GBps": round(by / t_q / 1e3),
+                   "quant_proj32_us": round(t_p, 2), "quant_proj32_GBps": round(by / t_p / 1e3),
+                   "frac_of_hbm": round(by / t_q / 1e3 / peaks["hbm"], 3),
+                   "frac_of_hbm_proj32": round(by / t_p / 1e3 / peaks["hbm"], 3)})
+        del x, q, ws, d, h
+    out["C4_quantizer_sweep"] = {"bytes_per_element": 2.5625, "hbm_peak_GBps": peaks["hbm"],
+                                 "note": "each launch timed alone (CUDA events, L2 evicted); ~6 us of every figure is "
+                                         "launch overhead of the isolated measurement", "cases": c4}
+    if not full:
+        return out
+
+    def layer_case(M, K, N, r_s, r):
+        r_t = r_s + r
+        X, G = acts(M, K), acts(M, N, grad=True)
+        W = (torch.randn(N, K, device=dev, generator=g) * 0.02).to(torch.bfloat16)
+        D_f = (torch.randn(K, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
+        U_t = (torch.randn(N, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
+        layer = B.Layer(W, D_f, U_t, r_s, r)
+        y = torch.empty(M, N, dtype=torch.bfloat16, device=dev)
+        dx = torch.empty(M, K, dtype=torch.bfloat16, device=dev)
+        h = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
+        p = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
+        ws = torch.empty(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_t), dtype=torch.uint8, device=dev)
+        qx, qg = B.QTensor(M, K, device=dev), B.QTensor(M, N, device=dev)
+        dA = torch.empty(K, r, dtype=torch.float32, device=dev)
+        dBt = torch.empty(N, r, dtype=torch.float32, device=dev)
+
+        def step():
+            B.ft_linear_fwd(layer, X, y, h, qx, ws)
+            B.ft_linear_bwd_dgrad(layer, G, dx, p, qg, ws)
+            B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt)
+        for _ in range(3):
+            step()
+        torch.cuda.synchronize()
+        gr = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gr):
+            step()
+        for _ in range(3):
+            gr.replay()
+        torch.cuda.synchronize()
+        n = 20
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(n):
+            gr.replay()
+        b.record()
+        torch.cuda.synchronize()
+        ours = a.elapsed_time(b) / n * 1e3
+        A_, B_ = D_f[:, r_s:].contiguous(), U_t[:, r_s:].t().contiguous()
+
+        def bf16():
+            xa = X @ A_
+            X @ W.t() + xa @ B_
+            gb = G @ B_.t()
+            G @ W + gb @ A_.t()
+            X.t() @ gb
+            xa.t() @ G
+        for _ in range(2):
+            bf16()
+        a.record()
+        for _ in range(5):
+            bf16()
+        b.record()
+        torch.cuda.synchronize()
+        base = a.elapsed_time(b) / 5 * 1e3
+        return ours, base
+
+    cfgs = {"C1": (256, 3072, 3072, 32, 16), "C3u": (4608, 3072, 12288, 32, 64), "C3d": (4608, 12288, 3072, 32, 64)}
+    out["configs"] = {}
+    for name, (M, K, N, r_s, r) in cfgs.items():
+        ours, base = layer_case(M, K, N, r_s, r)
+        out["configs"][name] = {"M": M, "K": K, "N": N, "r_s": r_s, "r": r, "step_us": round(ours, 1),
+                                "TFLOPs": round(4.0 * M * N * K / ours / 1e6, 1), "bf16_lora_us": round(base, 1),
+                                "speedup_vs_bf16_lora": round(base / ours, 2)}
+        torch.cuda.empty_cache()
+    from paper_2607_05711_b200 import synth
+    tot_ours = tot_base = tot_flop = 0.0
+    rows = []
+    for name, count, M, K, N in synth.C5_LAYERS:
+        ours, base = layer_case(M, K, N, 32, 32)
+        tot_ours += count * ours
+        tot_base += count * base
+        tot_flop += count * 4.0 * M * N * K
+        rows.append({"layer": name, "count": count, "M": M, "K": K, "N": N, "step_us": round(ours, 1),
+                     "bf16_lora_us": round(base, 1)})
+        torch.cuda.empty_cache()
+    out["C5_dit_linear_layers"] = {"layers": 228, "distinct_shapes": rows, "how": "each distinct (M,K,N) timed once "
+                                   "(CUDA graph, 20 replays back to back) and multiplied by its count",
+                                   "fwd_bwd_ms": round(tot_ours / 1e3, 2), "TFLOPs": round(tot_flop / tot_ours / 1e6, 1),
+                                   "bf16_lora_ms": round(tot_base / 1e3, 2),
+                                   "speedup_vs_bf16_lora": round(tot_base / tot_ours, 2)}
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -360,6 +492,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--eager", action="store_true", help="no CUDA graph for the timed steps")
+    ap.add_argument("--sweep", action="store_true", help="also time C1, C3 and the C5 layer list (slower)")
+    ap.add_argument("--no-sweep", dest="no_sweep", action="store_true", help="skip the C4 quantizer sweep")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
