@@ -189,7 +189,7 @@ def run_ours(args):
         B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt)
         if world > 1:
             parallel.allreduce_lora_grads(dA, dBt)
-    KERNELS_PER_STEP = 8   # 2 x (k_amax, k_quantize_fused, k_gemm4) + 2 x k_wgrad (memsets not counted)
+    KERNELS_PER_STEP = 7   # 2 x (k_amax, k_quantize_fused, k_gemm4_pair) + 1 x k_wgrad (memsets not counted)
 
     def barrier():
         if world > 1:

@@ -20,8 +20,9 @@ int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N,
                  cudaStream_t st);
 int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
                       const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st);
-int launch_wgrad(const void* in_bf16, int64_t M, int64_t F, const void* lr_bf16, int r_t, int r_s,
-                 int r, float* out, cudaStream_t st);
+int launch_wgrad_pair(const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
+                      const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
+                      cudaStream_t st);
 
 // ------------------------------------------------------------- device queries
 static int g_sm_count = 0;
@@ -293,13 +294,8 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
     return FT_ERR_INVALID_ARG;
   int rc = device_check();
   if (rc != FT_OK) return rc;
-  if (!accumulate) {
-    FT_CUDA_TRY(cudaMemsetAsync(dA, 0, (size_t)L->K * L->r * sizeof(float), st));
-    FT_CUDA_TRY(cudaMemsetAsync(dBt, 0, (size_t)L->N * L->r * sizeof(float), st));
-  }
-  rc = launch_wgrad(x_bf16, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA, st);
-  if (rc != FT_OK) return rc;
-  return launch_wgrad(g_bf16, M, L->N, h_saved_bf16, r_t, L->r_s, L->r, dBt, st);
+  return launch_wgrad_pair(x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
+                           accumulate, st);
 }
 
 }  // extern "C"

@@ -18,11 +18,13 @@ constexpr int WG_THREADS = 128;
 constexpr int WG_IN_BYTES = 2 * WG_MC * 128;  // two 64-feature boxes
 constexpr int WG_LG_BYTES = WG_MC * 128;      // one 64-column group of L
 
-struct WgParams {
-  int64_t M, F;
+struct WgParams {      // two problems in one launch: [0] dA = X^T P_lora, [1] dB^T = G^T H_lora
+  int64_t M;
+  int64_t F[2];
   int r_s, r;
-  int chunks_per_cta;
-  float* out;
+  int chunks_per_cta[2];
+  int direct[2];       // 1: a single M slice owns the output, plain stores (no zero-fill needed)
+  float* out[2];
 };
 
 __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
@@ -32,8 +34,16 @@ __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float 
 
 template <int R>
 __global__ void __launch_bounds__(WG_THREADS, 2)
-k_wgrad(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUtensorMap map_l,
+k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUtensorMap map_l0,
+        const __grid_constant__ CUtensorMap map_in1, const __grid_constant__ CUtensorMap map_l1,
         const WgParams p) {
+  const int z = blockIdx.z;
+  const CUtensorMap& map_in = z == 0 ? map_in0 : map_in1;
+  const CUtensorMap& map_l = z == 0 ? map_l0 : map_l1;
+  const int64_t F = p.F[z];
+  const int cpc = p.chunks_per_cta[z];
+  // CTAs beyond this problem's feature tiles or M slices have nothing to do (uniform per CTA)
+  if ((int64_t)blockIdx.x * WG_F >= F || (int64_t)blockIdx.y * cpc >= (p.M + WG_MC - 1) / WG_MC) return;
   constexpr int NG = (R + 63) / 64;
   constexpr int STAGE_BYTES = WG_IN_BYTES + NG * WG_LG_BYTES;
   constexpr uint32_t TMEM_COLS = R <= 32 ? 32 : (R <= 64 ? 64 : 128);
@@ -44,8 +54,8 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUte
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int32_t f0 = (int32_t)blockIdx.x * WG_F;
   const int64_t chunks_total = (p.M + WG_MC - 1) / WG_MC;
-  const int64_t c_begin = (int64_t)blockIdx.y * p.chunks_per_cta;
-  int n_chunks = (int)min((int64_t)p.chunks_per_cta, chunks_total - c_begin);
+  const int64_t c_begin = (int64_t)blockIdx.y * cpc;
+  int n_chunks = (int)min((int64_t)cpc, chunks_total - c_begin);
   if (n_chunks < 0) n_chunks = 0;
 
   if (tid == 0) {
@@ -117,12 +127,18 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUte
           : "r"(tmem_base + ((uint32_t)(warp * 32) << 16) + c0)
           : "memory");
       tmem_ld_wait();
-      if (f < p.F) {
-        float* o = p.out + f * R + c0;
+      if (f < F) {
+        float* o = p.out[z] + f * R + c0;
+        if (p.direct[z]) {
 #pragma unroll
-        for (int j = 0; j < 16; j += 4)
-          red_add_v4(o + j, __uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]),
-                     __uint_as_float(v[j + 3]));
+          for (int j = 0; j < 16; j += 4)
+            *reinterpret_cast<uint4*>(o + j) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+        } else {
+#pragma unroll
+          for (int j = 0; j < 16; j += 4)
+            red_add_v4(o + j, __uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]),
+                       __uint_as_float(v[j + 3]));
+        }
       }
     }
     tc_fence_before();
@@ -135,48 +151,64 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CUte
 }
 
 template <int R>
-static int launch_wg(const CUtensorMap& mi, const CUtensorMap& ml, const WgParams& p, unsigned gy,
-                     cudaStream_t st) {
+static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, cudaStream_t st) {
   constexpr int NG = (R + 63) / 64;
   const int smem = WG_STAGES * (WG_IN_BYTES + NG * WG_LG_BYTES) + 1024;
   FT_CUDA_TRY(cudaFuncSetAttribute(k_wgrad<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  dim3 grid((unsigned)ceil_div(p.F, WG_F), gy, 1);
-  k_wgrad<R><<<grid, WG_THREADS, smem, st>>>(mi, ml, p);
+  k_wgrad<R><<<grid, WG_THREADS, smem, st>>>(maps[0], maps[1], maps[2], maps[3], p);
   FT_CUDA_TRY(cudaGetLastError());
   return FT_OK;
 }
 
-int launch_wgrad(const void* in_bf16, int64_t M, int64_t F, const void* lr_bf16, int r_t, int r_s, int r,
-                 float* out, cudaStream_t st) {
-  CUtensorMap mi, ml;
-  int rc = make_tensor_map_2d(&mi, in_bf16, 2, (uint64_t)F, (uint64_t)M, (uint64_t)F * 2, 64, WG_MC,
-                              Swizzle::B128);
-  if (rc != FT_OK) return rc;
-  rc = make_tensor_map_2d(&ml, lr_bf16, 2, (uint64_t)r_t, (uint64_t)M, (uint64_t)r_t * 2, 64, WG_MC,
-                          Swizzle::B128);
-  if (rc != FT_OK) return rc;
-  const int64_t f_tiles = ceil_div(F, WG_F), chunks = ceil_div(M, WG_MC);
-  // M slices: about two resident CTAs per SM, at least 4 chunks per slice
-  int64_t slices = ceil_div((int64_t)2 * sm_count(), f_tiles);
-  if (slices > chunks / 4) slices = chunks / 4;
-  if (slices < 1) slices = 1;
+// dA [K x r] = X^T P[:, r_s:]  and  dBt [N x r] = G^T H[:, r_s:]  in ONE launch (blockIdx.z picks the
+// problem).  accumulate == 0 and a single M slice: plain stores; otherwise the buffers are zeroed
+// first (accumulate == 0) and the slices combine with fp32 reductions.
+int launch_wgrad_pair(const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
+                      const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
+                      cudaStream_t st) {
+  CUtensorMap maps[4];
+  const void* in[2] = {x, g};
+  const void* lr[2] = {p_saved, h_saved};
+  const int64_t F[2] = {K, N};
+  float* out[2] = {dA, dBt};
   WgParams p;
   p.M = M;
-  p.F = F;
   p.r_s = r_s;
   p.r = r;
-  p.chunks_per_cta = (int)ceil_div(chunks, slices);
-  p.out = out;
-  const unsigned gy = (unsigned)ceil_div(chunks, p.chunks_per_cta);
+  const int64_t chunks = ceil_div(M, WG_MC);
+  unsigned gx = 0, gy = 0;
+  for (int z = 0; z < 2; ++z) {
+    int rc = make_tensor_map_2d(&maps[2 * z], in[z], 2, (uint64_t)F[z], (uint64_t)M, (uint64_t)F[z] * 2, 64, WG_MC,
+                                Swizzle::B128);
+    if (rc != FT_OK) return rc;
+    rc = make_tensor_map_2d(&maps[2 * z + 1], lr[z], 2, (uint64_t)r_t, (uint64_t)M, (uint64_t)r_t * 2, 64, WG_MC,
+                            Swizzle::B128);
+    if (rc != FT_OK) return rc;
+    const int64_t f_tiles = ceil_div(F[z], WG_F);
+    // M slices: about two resident CTAs per SM, at least 8 chunks (512 rows) per slice
+    int64_t slices = ceil_div((int64_t)2 * sm_count(), f_tiles);
+    if (slices > chunks / 8) slices = chunks / 8;
+    if (slices < 1) slices = 1;
+    p.F[z] = F[z];
+    p.chunks_per_cta[z] = (int)ceil_div(chunks, slices);
+    const unsigned sl = (unsigned)ceil_div(chunks, p.chunks_per_cta[z]);
+    p.direct[z] = (sl == 1 && !accumulate) ? 1 : 0;
+    p.out[z] = out[z];
+    if (!accumulate && !p.direct[z])
+      FT_CUDA_TRY(cudaMemsetAsync(out[z], 0, (size_t)F[z] * r * sizeof(float), st));
+    if ((unsigned)f_tiles > gx) gx = (unsigned)f_tiles;
+    if (sl > gy) gy = sl;
+  }
+  const dim3 grid(gx, gy, 2);
   switch (r) {
-    case 16: return launch_wg<16>(mi, ml, p, gy, st);
-    case 32: return launch_wg<32>(mi, ml, p, gy, st);
-    case 48: return launch_wg<48>(mi, ml, p, gy, st);
-    case 64: return launch_wg<64>(mi, ml, p, gy, st);
-    case 80: return launch_wg<80>(mi, ml, p, gy, st);
-    case 96: return launch_wg<96>(mi, ml, p, gy, st);
-    case 112: return launch_wg<112>(mi, ml, p, gy, st);
-    case 128: return launch_wg<128>(mi, ml, p, gy, st);
+    case 16: return launch_wg<16>(maps, p, grid, st);
+    case 32: return launch_wg<32>(maps, p, grid, st);
+    case 48: return launch_wg<48>(maps, p, grid, st);
+    case 64: return launch_wg<64>(maps, p, grid, st);
+    case 80: return launch_wg<80>(maps, p, grid, st);
+    case 96: return launch_wg<96>(maps, p, grid, st);
+    case 112: return launch_wg<112>(maps, p, grid, st);
+    case 128: return launch_wg<128>(maps, p, grid, st);
     default: return FT_ERR_UNSUPPORTED_SHAPE;
   }
 }
