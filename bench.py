@@ -189,7 +189,9 @@ def run_ours(args):
         B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt)
         if world > 1:
             parallel.allreduce_lora_grads(dA, dBt)
-    KERNELS_PER_STEP = 7   # 2 x (k_amax, k_quantize_fused, k_gemm4_pair) + 1 x k_wgrad (memsets not counted)
+    # fwd: k_quantize_fused (single pass, amax inside) + k_gemm4_pair; bwd: k_amax + k_quantize_fused +
+    # k_gemm4_pair; wgrad: k_wgrad (memsets not counted)
+    KERNELS_PER_STEP = 6
 
     def barrier():
         if world > 1:
@@ -291,6 +293,8 @@ def run_ours(args):
     kern["quant_X_us"] = timed(lambda: B.ft_quantize_blockwise(
         X, qx, tensor_amax=amax, down=D_f, h_out=h, hs_out=hs, other_dec_scale=layer.r_kmajor.tensor_dec_scale,
         workspace=ws))
+    kern["amax_quant_X_fused_us"] = timed(lambda: B.ft_quantize_blockwise(
+        X, qx, down=D_f, h_out=h, hs_out=hs, other_dec_scale=layer.r_kmajor.tensor_dec_scale, workspace=ws))
     kern["gemm_fwd_us"] = timed(lambda: B.ft_gemm4(qx, layer.r_kmajor, hs, U_t, y))
     amax_g = B.ft_tensor_amax(G)
     kern["amax_G_us"] = timed(lambda: B.ft_tensor_amax(G, amax_g))

@@ -98,13 +98,17 @@ typedef struct {
   int32_t r_s, r;      /* r_t = r_s + r: 0, or a multiple of 16 up to 128                 */
 } ft_layer;
 
-/* ---- a0: tensor amax (Q3).  *amax_out = max |x_i| over n bf16 values. */
+/* ---- a0: tensor amax (Q3).  *amax_out = max |x_i| over n bf16 values.
+ * (ft_quantize_blockwise / ft_linear_* with tensor_amax == NULL find the amax themselves: inside
+ * the quantize kernel when the tensor fits the SMs' shared memory, with this kernel otherwise.) */
 int ft_tensor_amax(const void* x_bf16, int64_t n, float* amax_out, void* stream);
 
 /* ---- a1/a3/a6: Q(.) of DESIGN.md Q3-Q5 (+ optional fused down-projection).
  * x_bf16 [rows x cols]; blocks are out->block_rows x 16 along cols.
- * tensor_amax: device float holding amax_t; NULL => the library computes it first
- *   (one extra pass over x) into the workspace.
+ * tensor_amax: device float holding amax_t; NULL => the library computes it: inside the same
+ *   kernel (one HBM read of x in total) when x is at most ~29 MB, by an extra pass otherwise.
+ *   The fused projection accumulates H with fp32 reductions in the workspace (addition order not
+ *   fixed).  workspace may be NULL only if tensor_amax != NULL and proj == NULL.
  * proj: NULL => quantize only.  Requires out->block_rows == 1 if non-NULL.
  * Requirements: cols % 64 == 0; rows % 16 == 0 if block_rows == 16; any rows >= 1
  *   otherwise.  out->rows/cols must equal rows/cols.  round_mode must be
@@ -168,6 +172,9 @@ int ft_version(void);
 /* test / bench hook: 0 = default (CTA-pair 256x256 kernel); 128, 192, 256 = the 1-CTA kernel
  * with that N tile */
 int ft_debug_set_gemm_tile_n(int bn);
+/* test / bench hook: 0 = default (single-pass amax + quantize when the tensor fits), 1 = always
+ * the two-pass path (k_amax, then the streaming quantize kernel) */
+int ft_debug_set_quantize_mode(int mode);
 
 #ifdef __cplusplus
 }

@@ -62,6 +62,7 @@ def lib():
         L.ft_error_string.argtypes = [C.c_int]
         L.ft_error_string.restype = C.c_char_p
         L.ft_debug_set_gemm_tile_n.argtypes = [C.c_int]
+        L.ft_debug_set_quantize_mode.argtypes = [C.c_int]
         _lib = L
     return _lib
 
@@ -204,3 +205,7 @@ def ft_lora_wgrad(layer, x, g, h_saved, p_saved, dA, dBt, accumulate=False, stre
 
 def debug_set_gemm_tile_n(bn):
     _check(lib().ft_debug_set_gemm_tile_n(bn))
+
+
+def debug_set_quantize_mode(mode):
+    _check(lib().ft_debug_set_quantize_mode(mode))

@@ -9,11 +9,12 @@ namespace ft {
 thread_local int g_last_cuda_error = 0;
 
 // kernels' host launchers (quantize.cu, quantize_fused.cu, gemm.cu, wgrad.cu)
-int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st);
+int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first);
+void set_quantize_mode(int mode);
 int launch_quantize_generic(const void* x, int64_t rows, int64_t cols, const float* amax_t,
                             ft_qtensor* out, cudaStream_t st);
 int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t,
-                          const ft_proj* proj, ft_qtensor* out, cudaStream_t st);
+                          const ft_proj* proj, ft_qtensor* out, void* workspace, cudaStream_t st);
 int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, cudaStream_t st);
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
                  const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16,
@@ -87,8 +88,6 @@ int make_tensor_map_2d(CUtensorMap* map, const void* base, int elem_bytes, uint6
 }
 
 static bool valid_rt(int r_t) { return r_t >= 0 && r_t <= 128 && r_t % 16 == 0; }
-static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
-constexpr size_t WS_HS_OFFSET = 256;  // [0,4): tensor amax; [256, ..): pre-scaled H / P
 
 // one direction of the layer: quantize `act` [M x Kd] (+ projection by lr_down
 // [Kd x r_t]) and multiply with the weight operand `w` ([Nd x Kd]); lr_up [Nd x r_t].
@@ -106,21 +105,20 @@ static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_
   if (ws_bytes < ft_workspace_bytes(M, Kd, Nd, r_t)) return FT_ERR_WORKSPACE_TOO_SMALL;
   int rc = device_check();
   if (rc != FT_OK) return rc;
-  float* amax = reinterpret_cast<float*>(workspace);
-  void* hs = reinterpret_cast<uint8_t*>(workspace) + WS_HS_OFFSET;
+  void* hs = reinterpret_cast<uint8_t*>(workspace) + ws_layout(M, r_t).hs_off;
   q->rows = M;
   q->cols = Kd;
   q->block_rows = 1;
   q->sf_layout = FT_SF_TILE128x4;
-  rc = launch_amax(act, M * Kd, amax, st);
-  if (rc != FT_OK) return rc;
   ft_proj pr;
   pr.down = lr_down;
   pr.out = saved;
   pr.out_scaled = hs;
   pr.other_dec_scale = w->tensor_dec_scale;
   pr.r_t = r_t;
-  rc = launch_quantize_fused(act, M, Kd, amax, r_t > 0 ? &pr : nullptr, q, st);
+  // a0 + a1/a3: the tensor amax is found inside the quantize pass when the tensor fits the SMs'
+  // shared memory (single pass), by a preceding k_amax launch otherwise
+  rc = launch_quantize_fused(act, M, Kd, nullptr, r_t > 0 ? &pr : nullptr, q, workspace, st);
   if (rc != FT_OK) return rc;
   return launch_gemm4(q, w, M, Nd, Kd, r_t > 0 ? hs : nullptr, lr_up, r_t, out, st);
 }
@@ -147,7 +145,13 @@ using namespace ft;
 
 extern "C" {
 
-int ft_version(void) { return 100; }
+int ft_version(void) { return 110; }
+
+int ft_debug_set_quantize_mode(int mode) {
+  if (mode < 0 || mode > 2) return FT_ERR_INVALID_ARG;
+  set_quantize_mode(mode);
+  return FT_OK;
+}
 
 const char* ft_error_string(int status) {
   switch (status) {
@@ -174,12 +178,12 @@ size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t) {
   (void)K;
   (void)N;
   if (M < 0 || r_t < 0) return 0;
-  return WS_HS_OFFSET + align_up((size_t)M * (size_t)r_t * 2, 256) + 256;
+  return ws_layout(M, r_t).total;
 }
 
 int ft_tensor_amax(const void* x_bf16, int64_t n, float* amax_out, void* stream) {
   if (!x_bf16 || !amax_out || n < 0 || !aligned16(x_bf16)) return FT_ERR_INVALID_ARG;
-  return launch_amax(x_bf16, n, amax_out, (cudaStream_t)stream);
+  return launch_amax(x_bf16, n, amax_out, (cudaStream_t)stream, true);
 }
 
 int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols, const float* tensor_amax,
@@ -207,16 +211,21 @@ int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols, const 
   }
   int rc = device_check();
   if (rc != FT_OK) return rc;
-  const float* amax = tensor_amax;
-  if (!amax) {
+  if (!tensor_amax || r_t > 0) {
     if (!workspace || !aligned16(workspace)) return FT_ERR_INVALID_ARG;
     if (workspace_bytes < ft_workspace_bytes(rows, cols, 0, r_t)) return FT_ERR_WORKSPACE_TOO_SMALL;
-    rc = launch_amax(x_bf16, rows * cols, reinterpret_cast<float*>(workspace), st);
-    if (rc != FT_OK) return rc;
-    amax = reinterpret_cast<const float*>(workspace);
   }
-  if (out->block_rows == 16) return launch_quantize_generic(x_bf16, rows, cols, amax, out, st);
-  return launch_quantize_fused(x_bf16, rows, cols, amax, proj, out, st);
+  if (out->block_rows == 16) {
+    const float* amax = tensor_amax;
+    if (!amax) {
+      float* a = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + ws_layout(rows, r_t).amax_off);
+      rc = launch_amax(x_bf16, rows * cols, a, st, true);
+      if (rc != FT_OK) return rc;
+      amax = a;
+    }
+    return launch_quantize_generic(x_bf16, rows, cols, amax, out, st);
+  }
+  return launch_quantize_fused(x_bf16, rows, cols, tensor_amax, proj, out, workspace, st);
 }
 
 int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, void* stream) {

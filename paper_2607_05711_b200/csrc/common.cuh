@@ -36,6 +36,29 @@ int make_tensor_map_2d(CUtensorMap* map, const void* base, int elem_bytes, uint6
 int device_check();  // FT_OK if the current device is sm_100-class
 int sm_count();
 
+// Caller-provided workspace of one quantize (+ GEMM) pass over an [M x *] activation with a rank-r_t
+// projection.  [hs_off, +M*r_t*2): the pre-scaled bf16 intermediate Hs.  The "zero region" (256 bytes)
+// is cleared by one memset per call: the tensor-amax word and two grid-barrier counters.  Behind it:
+// one 128 x r_t fp32 slot per (CTA, row tile) segment of the quantize kernel -- at most
+// WS_MAX_QUANT_CTAS + row tiles of them -- holding partial H tiles.
+constexpr int WS_MAX_QUANT_CTAS = 320;   // 2 CTAs per SM, <= 160 SMs
+struct WsLayout {
+  size_t hs_off, zero_off, zero_bytes, amax_off, bar_off, slots_off, total;
+};
+inline WsLayout ws_layout(int64_t M, int r_t) {
+  auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+  WsLayout w;
+  const size_t tiles = (size_t)((M + 127) / 128);
+  w.hs_off = 256;
+  w.zero_off = w.hs_off + up((size_t)M * (size_t)r_t * 2);
+  w.amax_off = w.zero_off;
+  w.bar_off = w.zero_off + 4;
+  w.zero_bytes = 256;
+  w.slots_off = w.zero_off + w.zero_bytes;
+  w.total = w.slots_off + (WS_MAX_QUANT_CTAS + tiles) * 128 * (size_t)r_t * 4 + 256;
+  return w;
+}
+
 // ---------------------------------------------------------------- device side
 #ifdef __CUDACC__
 

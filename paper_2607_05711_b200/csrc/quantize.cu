@@ -44,8 +44,8 @@ __global__ void __launch_bounds__(256) k_amax(const uint4* __restrict__ x, int64
   }
 }
 
-int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st) {
-  FT_CUDA_TRY(cudaMemsetAsync(amax_out, 0, sizeof(float), st));
+int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first) {
+  if (zero_first) FT_CUDA_TRY(cudaMemsetAsync(amax_out, 0, sizeof(float), st));
   if (n == 0) return FT_OK;
   const int64_t n_vec = n / 8;
   const int n_tail = (int)(n % 8);

@@ -1,20 +1,34 @@
-// quantize_fused.cu -- a1 / a3: one pass over X (or G) that emits the NVFP4 codes,
-// the block scales and the low-rank down-projection H = X * D ("fuse
-// ... quantization and down-projection").
+// quantize_fused.cu -- a1 / a3 (and a0 folded in): one kernel that emits the NVFP4 codes, the
+// block scales and the low-rank down-projection H = X * D of a bf16 matrix (PAPER.md:110,
+// "fuse ... quantization and down-projection").
 //
-// Decomposition: a CTA owns 128 rows x (cols / SPLIT) columns and walks them in
-// 128 x 64 chunks that TMA stages into shared memory (SWIZZLE_128B) through a
-// 3/4-deep mbarrier ring.  From one staged chunk
+// Decomposition.  The matrix is cut into 128-row x 64-column chunks (16 KB), numbered row tile
+// major.  CTA i of a persistent grid owns the contiguous chunk range [i*TC/G, (i+1)*TC/G): every
+// CTA has the same number of chunks (+-1) whatever the shape -- no row-tile x split quantisation --
+// and a range touches at most two row tiles when it is no longer than a row of chunks.
+// From one TMA-staged chunk (SWIZZLE_128B)
 //   - 512 threads quantize: thread (row = tid/4, quarter = tid%4) owns one 1x16 block;
 //   - one thread issues tcgen05.mma kind::f16 (M = 128, N = r_t, K = 16, four per chunk):
-//     A = the staged chunk itself (K-major, the TMA swizzle is the UMMA canonical layout),
-//     B = the 64 x r_t slice of D staged beside it (MN-major), accumulator in tensor memory.
-//     The staged bytes are read once by the tensor core instead of once per warp by ldmatrix.
-// Two CTAs are resident per SM (32 warps): the per-block scale arithmetic is a long
-// dependent chain (three IEEE divisions) and needs the warps to hide its latency.
-// The SPLIT CTAs of a 128-row tile form a thread-block cluster (1, SPLIT, 1); their
-// fp32 partial H tiles are summed through distributed shared memory, so H is
-// complete in one pass with no atomics and no second kernel.
+//     A = the staged chunk itself (K-major), B = the 64 x r_t slice of D staged in its own ring
+//     (MN-major), accumulator in tensor memory.
+// Warps 0-15 quantize, warp 16 is the TMA producer, warp 17 the tcgen05 issuer (a quantizer warp that
+// also issues the MMAs is ~400 cycles slower per chunk than its peers and sets the pace of the ring).
+// At the end of a row-tile segment the fp32 partial H tile goes TMEM -> plain vector stores into the
+// segment's own 128 x r_t slot of the workspace (slot = CTA index + row tile: unique, and the slots of
+// one row tile are consecutive).  After a grid-wide barrier (all CTAs are co-resident: cooperative
+// launch) every CTA completes an equal share of the rows: it sums the row tile's slots in CTA order
+// and writes bf16 H and Hs = H * (1 / alpha) -- no second kernel, no atomics on the data, a fixed
+// summation order.  Measured and dropped: fp32 reductions into one accumulator (REDG issues at ~1.3
+// cycles per lane and word: 10 k cycles per 128 x 64 tile) and a last-arriver CTA finishing a whole
+// row tile alone (a 9-17 k-cycle tail on 36 of 296 CTAs).
+//
+// Two modes, one kernel:
+//   streaming (amax known): chunks stream through a 4-deep ring, two CTAs per SM;
+//   single pass (amax not known, tensor <= 12 chunks per SM = 29 MB on 148 SMs): every chunk of
+//     the CTA stays resident in shared memory; phase 1 finds the tensor amax (and runs the
+//     projection MMAs) as the chunks land, a grid-wide barrier publishes it, phase 2 quantizes
+//     from shared memory.  The tensor is read from HBM exactly once and the separate amax kernel
+//     (a0) disappears.  Launched cooperatively (all CTAs co-resident).
 #include <cstdio>
 #include <cstdlib>
 
@@ -23,15 +37,22 @@
 
 namespace ft {
 
-constexpr int QF_ROWS = 128;    // rows per CTA
+constexpr int QF_ROWS = 128;    // rows per chunk
 constexpr int QF_KC = 64;       // columns per chunk (128 bytes of bf16 = one swizzle row)
-constexpr int QF_THREADS = 512;
+constexpr int QF_QTHREADS = 512;              // quantizer threads (warps 0-15)
+constexpr int QF_THREADS = QF_QTHREADS + 64;  // + warp 16: TMA producer, warp 17: tcgen05 issuer
 constexpr int QF_X_BYTES = QF_ROWS * QF_KC * 2;  // 16 KB
 constexpr int QF_DG_BYTES = QF_KC * 128;         // one 64-column group of D: 8 KB
+constexpr int QF_MAX_NX = 12;   // resident chunks per CTA in single-pass mode
+constexpr int QF_MAX_ND = 4;
+constexpr int QF_MAX_GRID = WS_MAX_QUANT_CTAS;   // the workspace has one slot per CTA + one per row tile
 
 struct QFParams {
   int64_t rows, cols;
-  const float* amax_t;
+  const float* amax_in;         // streaming: tensor amax (device)
+  uint32_t* amax_bits;          // single pass: zeroed word, receives the amax bit pattern
+  uint32_t* grid_bar;           // two zeroed arrival counters: [0] amax published (single pass), [1] slots written
+  float* slots;                 // [(grid + row tiles) x 128 x r_t] fp32 partial H tiles (not zeroed)
   uint8_t* codes;
   uint8_t* sf;
   float* g_dec_out;
@@ -39,195 +60,182 @@ struct QFParams {
   __nv_bfloat16* h_out;         // [rows x r_t] or null
   __nv_bfloat16* hs_out;        // [rows x r_t] or null
   const float* other_dec_scale; // for hs_out
-  int split;                    // CTAs per row tile (cluster size)
+  int single;                   // 1: single-pass mode
+  int nx, nd;                   // ring depths (single pass: nx = max chunks per CTA)
+  int chunks_per_tile;          // C = cols / 64
+  int64_t total_chunks;         // TC = row tiles * C
+#ifdef FT_QF_TIMING
+  long long* dbg;               // [grid x 8] clock64 stamps (debug builds only)
+#endif
 };
+#ifdef FT_QF_TIMING
+#define QF_STAMP(k) do { if (p.dbg && threadIdx.x == 0) p.dbg[blockIdx.x * 8 + (k)] = clock64(); } while (0)
+#else
+#define QF_STAMP(k) do { } while (0)
+#endif
 
-__device__ __forceinline__ void ldsm_x4(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2,
-                                        uint32_t& r3) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0, %1, %2, %3}, [%4];"
-               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
-               : "r"(addr));
+__device__ __forceinline__ void red_add_v4_f32(float* addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(__uint_as_float(a)),
+               "f"(__uint_as_float(b)), "f"(__uint_as_float(c)), "f"(__uint_as_float(d))
+               : "memory");
 }
-__device__ __forceinline__ void ldsm_x4_t(uint32_t addr, uint32_t& r0, uint32_t& r1, uint32_t& r2,
-                                          uint32_t& r3) {
-  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];"
-               : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3)
-               : "r"(addr));
-}
-__device__ __forceinline__ void mma_16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2,
-                                          uint32_t a3, uint32_t b0, uint32_t b1) {
-  asm volatile(
-      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, "
-      "{%8, %9}, {%0, %1, %2, %3};"
-      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
-      : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
-}
-__device__ __forceinline__ void cluster_sync_all() {
-  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;"
-               ::: "memory");
-}
-__device__ __forceinline__ float ld_dsmem_f32(uint32_t local_addr, uint32_t cta_rank) {
-  uint32_t remote;
-  float v;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(cta_rank));
-  asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(remote));
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-
-__device__ __forceinline__ float2 ld_dsmem_f32x2(uint32_t local_addr, uint32_t cta_rank) {
-  uint32_t remote;
+__device__ __forceinline__ float2 ld_cg_f32x2(const float* p) {
   float2 v;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(local_addr), "r"(cta_rank));
-  asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(remote));
+  asm volatile("ld.global.cg.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p) : "memory");
   return v;
+}
+__device__ __forceinline__ uint64_t globaltimer_ns() {
+  uint64_t t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
 }
 
 // R_T: width of the projection (0 = quantize only).  NG = 64-column groups of D.
-template <int R_T>
-__global__ void __launch_bounds__(QF_THREADS, 2)
+template <int R_T, bool SINGLE>
+__global__ void __launch_bounds__(QF_THREADS, SINGLE ? 1 : 2)
 k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constant__ CUtensorMap map_d,
                  const QFParams p) {
   constexpr int NG = (R_T + 63) / 64;
-  constexpr uint32_t TMEM_COLS = R_T <= 32 ? 32 : (R_T <= 64 ? 64 : 128);
-  constexpr int QF_STAGES = (NG == 2) ? 3 : 4;
-  constexpr int STAGE_BYTES = QF_X_BYTES + NG * QF_DG_BYTES;
+  constexpr uint32_t ACC_COLS = R_T <= 32 ? 32 : (R_T <= 64 ? 64 : 128);
+  constexpr int D_BYTES = NG * QF_DG_BYTES;
+  constexpr int NXS = NG == 2 ? 3 : 4;     // streaming mode: ring depth of X and of D
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   // 1024-byte alignment for the 128-byte swizzle atoms
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  __shared__ uint64_t full_bar[4], empty_bar[4];
+  __shared__ uint64_t full_x[QF_MAX_NX], empty_x[QF_MAX_ND], full_d[QF_MAX_ND], empty_d[QF_MAX_ND];
+  __shared__ uint64_t acc_full[2], acc_free[2];
   __shared__ float enc_tab[128];
-  __shared__ uint64_t acc_bar;
-  __shared__ uint32_t tmem_base_s;
+  __shared__ uint32_t tmem_base_s, s_red[QF_QTHREADS / 32], s_amax;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int64_t row0 = (int64_t)blockIdx.x * QF_ROWS;
-  const int split = p.split;
-  const int64_t chunks_total = p.cols / QF_KC;
-  const int n_chunks = (int)((chunks_total - blockIdx.y + split - 1) / split);  // interleaved, may be uneven
-  // chunk `it` of this CTA is global chunk it * split + blockIdx.y: the CTAs of a cluster walk
-  // the columns interleaved, so together they touch split * 128 contiguous bytes of each row at
-  // about the same time (DRAM page locality) instead of `split` far-apart 128-byte pieces.
+  const int64_t c_begin = (int64_t)blockIdx.x * p.total_chunks / gridDim.x;
+  const int n = (int)(((int64_t)blockIdx.x + 1) * p.total_chunks / gridDim.x - c_begin);   // >= 1 (grid <= TC)
+  const int C = p.chunks_per_tile;
+  const uint32_t xs_u = smem_u32(smem);
+  const uint32_t ds_u = xs_u + (uint32_t)p.nx * QF_X_BYTES;
 
   if (tid == 0) {
     prefetch_tmap(&map_x);
     if (R_T > 0) prefetch_tmap(&map_d);
-    for (int s = 0; s < QF_STAGES; ++s) {
-      mbar_init(&full_bar[s], 1);
-      mbar_init(&empty_bar[s], QF_THREADS / 32 + (R_T > 0 ? 1 : 0));  // every warp (+ the MMA commit)
+    for (int s = 0; s < QF_MAX_NX; ++s) mbar_init(&full_x[s], 1);
+    for (int s = 0; s < QF_MAX_ND; ++s) {
+      mbar_init(&empty_x[s], QF_QTHREADS / 32 + (R_T > 0 ? 1 : 0));  // every quantizer warp (+ the MMA commit)
+      mbar_init(&full_d[s], 1);
+      mbar_init(&empty_d[s], 1);
     }
-    mbar_init(&acc_bar, 1);
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(&acc_full[a], 1);   // tcgen05.commit of a segment's last MMA
+      mbar_init(&acc_free[a], 4);   // the four drain warps
+    }
     fence_mbar_init();
   }
   if (R_T > 0 && warp == 2) {
-    tmem_alloc(&tmem_base_s, TMEM_COLS);
+    tmem_alloc(&tmem_base_s, 2 * ACC_COLS);
     tmem_relinquish();
   }
+  QF_STAMP(0);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  QF_STAMP(1);
 
-  auto issue = [&](int it) {
-    const int s = it % QF_STAGES;
-    uint8_t* base = smem + s * STAGE_BYTES;
-    const int32_t kcol = (int32_t)(((int64_t)it * split + blockIdx.y) * QF_KC);
-    mbar_expect_tx(&full_bar[s], STAGE_BYTES);
-    tma_load_2d(base, &map_x, &full_bar[s], kcol, (int32_t)row0);
+  // chunk `it` of this CTA is global chunk c_begin + it = (row tile t, column chunk kc)
+  auto issue_x = [&](int it, int slot) {
+    const int64_t c = c_begin + it;
+    const int t = (int)(c / C), kc = (int)(c % C);
+    mbar_expect_tx(&full_x[slot], QF_X_BYTES);
+    tma_load_2d(smem + slot * QF_X_BYTES, &map_x, &full_x[slot], kc * QF_KC, t * QF_ROWS);
+  };
+  auto issue_d = [&](int it, int slot) {
+    const int kc = (int)((c_begin + it) % C);
+    mbar_expect_tx(&full_d[slot], D_BYTES);
 #pragma unroll
     for (int g = 0; g < NG; ++g)
-      tma_load_2d(base + QF_X_BYTES + g * QF_DG_BYTES, &map_d, &full_bar[s], g * 64, kcol);
+      tma_load_2d(smem + p.nx * QF_X_BYTES + slot * D_BYTES + g * QF_DG_BYTES, &map_d, &full_d[slot], g * 64,
+                  kc * QF_KC);
   };
-  if (tid == 0) {
-    for (int it = 0; it < QF_STAGES && it < n_chunks; ++it) issue(it);
-  }
+  // the four MMAs of one chunk: acc[128 x r_t] (+)= X[128, 64 k] * D[64 k, r_t]
+  auto issue_mma = [&](uint32_t x_u, uint32_t d_u, uint32_t acc, bool first) {
+    constexpr uint32_t idesc = idesc_bf16(QF_ROWS, R_T > 0 ? R_T : 16) | (1u << 16);  // B is MN-major
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      mma_bf16(acc, make_smem_desc(x_u + k * 32, 1024, 0, 2), make_smem_desc(d_u + k * 2048, 1024, QF_DG_BYTES, 2),
+               idesc, !(first && k == 0));
+  };
 
-  const TensorScale ts = tensor_scale(__ldg(p.amax_t));
-  if (blockIdx.x == 0 && blockIdx.y == 0 && tid == 0) *p.g_dec_out = ts.g_dec;
-  if (tid < 128) enc_tab[tid] = enc_of_sf8((uint32_t)tid, ts.g_dec);
-  __syncthreads();
-
-  // quantizer role of this thread
+  // quantizer role of this thread: one 1x16 block (two 16-byte pieces of a swizzled row) per chunk
   const int q_row = tid >> 2, q_quarter = tid & 3;
-  const int64_t q_grow = row0 + q_row;
-  const bool q_live = q_grow < p.rows;
-  const int64_t nblk = p.cols / 16;
-  const uint32_t q_smem_base = smem_u32(smem) + q_row * 128;
-  const uint32_t q_smem_off0 = q_smem_base + (((q_quarter * 2) ^ (q_row & 7)) << 4);
-  const uint32_t q_smem_off1 = q_smem_base + (((q_quarter * 2 + 1) ^ (q_row & 7)) << 4);
-  // output cursors: chunk `it` is global chunk it * split + blockIdx.y
-  uint8_t* q_codes = p.codes + q_grow * (p.cols / 2) + ((int64_t)blockIdx.y * QF_KC + q_quarter * 16) / 2;
-  const int64_t q_codes_step = (int64_t)split * (QF_KC / 2);
-  uint8_t* q_sf = p.sf + ((p.sf_layout == FT_SF_TILE128x4) ? sf_tile_offset(q_grow, (int64_t)blockIdx.y * 4, nblk)
-                                                           : q_grow * nblk + (int64_t)blockIdx.y * 4);
-  const int64_t q_sf_step = (p.sf_layout == FT_SF_TILE128x4) ? (int64_t)split * 512 : (int64_t)split * 4;
-  for (int it = 0; it < n_chunks; ++it) {
-    const int s = it % QF_STAGES;
-    const uint32_t parity = (it / QF_STAGES) & 1;
-    // refill, one iteration late: warp 0 re-arms the slot of chunk it-1 once every warp has
-    // released it; no block-wide barrier, so the other warps run ahead through the ring
-    if (warp == 0 && it > 0) {
-      if (lane == 0 && it - 1 + QF_STAGES < n_chunks) {
-        mbar_wait(&empty_bar[(it - 1) % QF_STAGES], ((it - 1) / QF_STAGES) & 1);
-        issue(it - 1 + QF_STAGES);
-      }
-      __syncwarp();
-    }
-    mbar_wait(&full_bar[s], parity);
-
-    // ---- quantize one 1x16 block (two 16-byte chunks of this row)
-    {
-      uint4 v0, v1;
-      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                   : "=r"(v0.x), "=r"(v0.y), "=r"(v0.z), "=r"(v0.w) : "r"(q_smem_off0 + s * STAGE_BYTES));
-      asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
-                   : "=r"(v1.x), "=r"(v1.y), "=r"(v1.z), "=r"(v1.w) : "r"(q_smem_off1 + s * STAGE_BYTES));
-      const uint32_t sf8 = block_sf8(amax_block16(v0, v1), ts.g_enc);
-      const float enc = enc_tab[sf8];
-      uint2 c;
-      c.x = quant_bf16x8_fast(v0, enc);
-      c.y = quant_bf16x8_fast(v1, enc);
-      // gather the row's four scale bytes into the quarter-0 lane
-      uint32_t w = sf8 << (8 * q_quarter);
-      w |= __shfl_xor_sync(0xffffffffu, w, 1);
-      w |= __shfl_xor_sync(0xffffffffu, w, 2);
-      if (q_live) {
-        *reinterpret_cast<uint2*>(q_codes) = c;
-        if (q_quarter == 0) *reinterpret_cast<uint32_t*>(q_sf) = w;
-      }
-      q_codes += q_codes_step;
-      q_sf += q_sf_step;
-    }
-
-    // ---- projection: acc[128 x r_t] += X[128, 64 k] * D[64 k, r_t], issued by one thread
-    if constexpr (R_T > 0) {
-      if (warp == 1) {
-        if (lane == 0) {
-          tc_fence_after();
-          const uint32_t xs_u = smem_u32(smem) + s * STAGE_BYTES;
-          const uint32_t ds_u = xs_u + QF_X_BYTES;
-          constexpr uint32_t idesc = idesc_bf16(QF_ROWS, R_T) | (1u << 16);  // B is MN-major
-#pragma unroll
-          for (int k = 0; k < 4; ++k)
-            mma_bf16(tmem_base_s, make_smem_desc(xs_u + k * 32, 1024, 0, 2),
-                     make_smem_desc(ds_u + k * 2048, 1024, QF_DG_BYTES, 2), idesc, (it | k) != 0);
-          tc_commit(&empty_bar[s]);                       // slot free once the MMAs have read it
-          if (it == n_chunks - 1) tc_commit(&acc_bar);    // accumulator complete
-        }
-        __syncwarp();
-      }
-    }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&empty_bar[s]);  // this warp is done with stage s
+  const uint32_t q_off0 = q_row * 128 + (((q_quarter * 2) ^ (q_row & 7)) << 4);
+  const uint32_t q_off1 = q_off0 ^ 16;
+  const bool sf_tiled = p.sf_layout == FT_SF_TILE128x4;
+  // output cursor (32-bit byte offsets; the host rejects tensors whose codes exceed 4 GB): advanced
+  // one chunk at a time, no per-chunk index arithmetic
+  int o_t = (int)(c_begin / C), o_kc = (int)(c_begin % C);
+  uint32_t o_co, o_so;
+  bool o_live;
+  {
+    const uint32_t nblk = (uint32_t)(p.cols / 16), half_cols = (uint32_t)(p.cols / 2);
+    const uint32_t grow = (uint32_t)o_t * QF_ROWS + q_row;
+    o_live = (int64_t)grow < p.rows;
+    o_co = grow * half_cols + o_kc * 32 + q_quarter * 8;
+    o_so = sf_tiled ? ((uint32_t)o_t * C + o_kc) * 512 + (q_row & 31) * 16 + (q_row >> 5) * 4 : grow * nblk + o_kc * 4;
   }
-  __syncthreads();  // every warp has consumed every stage: the ring can be reused below
+  auto advance_out = [&]() {
+    o_co += 32;
+    o_so += sf_tiled ? 512 : 4;
+    if (++o_kc == C) {     // row tile change: 128 rows down, C chunks back
+      o_kc = 0;
+      ++o_t;
+      o_co += 127u * (uint32_t)(p.cols / 2);
+      if (!sf_tiled) o_so += 127u * (uint32_t)(p.cols / 16);
+      o_live = (int64_t)o_t * QF_ROWS + q_row < p.rows;
+    }
+  };
+  auto load_block = [&](uint32_t x_u, uint4& v0, uint4& v1) {
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v0.x), "=r"(v0.y), "=r"(v0.z), "=r"(v0.w) : "r"(x_u + q_off0));
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(v1.x), "=r"(v1.y), "=r"(v1.z), "=r"(v1.w) : "r"(x_u + q_off1));
+  };
+  auto quantize_chunk = [&](uint32_t x_u, float g_enc) {
+    uint4 v0, v1;
+    load_block(x_u, v0, v1);
+    const uint32_t sf8 = block_sf8(amax_block16(v0, v1), g_enc);
+    const float enc = enc_tab[sf8];
+    uint2 c;
+    c.x = quant_bf16x8_fast(v0, enc);
+    c.y = quant_bf16x8_fast(v1, enc);
+    // gather the row's four scale bytes into the quarter-0 lane
+    uint32_t w = sf8 << (8 * q_quarter);
+    w |= __shfl_xor_sync(0xffffffffu, w, 1);
+    w |= __shfl_xor_sync(0xffffffffu, w, 2);
+    if (o_live) {
+      *reinterpret_cast<uint2*>(p.codes + o_co) = c;
+      if (q_quarter == 0) *reinterpret_cast<uint32_t*>(p.sf + o_so) = w;
+    }
+  };
 
-  // ---- cluster reduction of the partial H tiles and output
-  if constexpr (R_T > 0) {
-    float* part = reinterpret_cast<float*>(smem);  // [128][R_T] fp32, reuses the ring
+  // barrier of the 16 quantizer warps only (the producer and the issuer warp run free)
+  auto qsync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(QF_QTHREADS) : "memory"); };
+
+  // ---- projection bookkeeping.  A "segment" is this CTA's run of chunks inside one row tile; its
+  // fp32 partial H tile accumulates in TMEM accumulator (segment & 1).
+  // drain: TMEM -> the segment's slot in the workspace, by warps 0-3, with no block-wide barrier (the
+  // other warps keep quantizing).
+  auto drain_segment = [&](int t, int seg) {
+    const int a = seg & 1;
     if (warp < 4) {   // warp w may read TMEM lanes 32w .. 32w+31 = rows of the tile
-      mbar_wait(&acc_bar, 0);
+      mbar_wait(&acc_full[a], (uint32_t)(seg >> 1) & 1);
       tc_fence_after();
-      const int r = warp * 32 + lane;
-#pragma unroll
+      // slot layout [column quad q = c / 4][row][4 floats]: a warp's store instruction covers 512
+      // contiguous bytes (full sectors), and so does a warp's load in the finalizer
+      float* dst = p.slots + ((int64_t)blockIdx.x + t) * (QF_ROWS * R_T) + (warp * 32 + lane) * 4;
+#pragma unroll 1
       for (int c0 = 0; c0 < R_T; c0 += 16) {
         uint32_t v[16];
         asm volatile(
@@ -235,158 +243,405 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
             "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
               "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-            : "r"(tmem_base_s + ((uint32_t)(warp * 32) << 16) + c0)
+            : "r"(tmem_base_s + ((uint32_t)(warp * 32) << 16) + a * ACC_COLS + c0)
             : "memory");
         tmem_ld_wait();
 #pragma unroll
-        for (int j = 0; j < 16; j += 4)   // rotate the 16-byte pieces by row to spread the banks
-          *reinterpret_cast<uint4*>(part + r * R_T + c0 + ((j + 4 * (r & 3)) & 15)) =
-              make_uint4(v[(j + 4 * (r & 3)) & 15], v[(j + 4 * (r & 3) + 1) & 15], v[(j + 4 * (r & 3) + 2) & 15],
-                         v[(j + 4 * (r & 3) + 3) & 15]);
+        for (int j = 0; j < 16; j += 4)
+          *reinterpret_cast<uint4*>(dst + (c0 + j) / 4 * (QF_ROWS * 4)) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
       }
       tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&acc_free[a]);   // the accumulator may be overwritten
     }
-    if (split > 1) cluster_sync_all(); else __syncthreads();
-    const int rows_per = (QF_ROWS + split - 1) / split;
-    const int r_begin = (int)blockIdx.y * rows_per;
-    float alpha = 1.0f;
-    if (p.hs_out != nullptr) alpha = __fmul_rn(ts.g_dec, __ldg(p.other_dec_scale));
-    const uint32_t part_u = smem_u32(part);
-    for (int e = tid; e < rows_per * (R_T / 2); e += QF_THREADS) {
-      const int r = r_begin + e / (R_T / 2), c = (e % (R_T / 2)) * 2;
-      if (r >= QF_ROWS) break;
-      float s0 = 0.f, s1 = 0.f;
-      if (split > 1) {
-        float2 v[8];
+  };
+  // grid-wide barrier on a zeroed counter (every CTA of the launch is resident: cooperative launch).
+  // Quantizer warps only; release / acquire at gpu scope, cumulative through the CTA barrier.
+  auto grid_barrier = [&](uint32_t* counter) {
+    qsync();
+    if (tid == 0) {
+      asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+      const uint64_t t0 = globaltimer_ns();
+      while (ld_acquire_u32(counter) < gridDim.x) {
+        if (globaltimer_ns() - t0 > 2000000000ull) __trap();   // co-residency broken: fail, do not hang
+      }
+    }
+    qsync();
+  };
+  // After the grid barrier every partial H tile is in its slot.  CTA i completes rows
+  // [i * rows / G, (i + 1) * rows / G): fp32 sum of the row tile's slots in CTA order (fixed order:
+  // the result does not depend on timing) -> bf16 H and Hs = H * (1 / alpha).
+  auto finalize_share = [&](float inv_alpha) {
+    constexpr int QUADS = R_T > 0 ? R_T / 4 : 1;
+    constexpr int SLOT_F4 = QF_ROWS * (R_T > 0 ? R_T : 4) / 4;
+    const int64_t TC = p.total_chunks, G = gridDim.x;
+    const int64_t r_begin = (int64_t)blockIdx.x * p.rows / G;
+    const int nrows = (int)(((int64_t)blockIdx.x + 1) * p.rows / G - r_begin);
+    // item e -> (row e % nrows, column quad e / nrows): neighbouring threads read neighbouring rows
+    for (int e = tid; e < nrows * QUADS; e += QF_QTHREADS) {
+      const int64_t gr = r_begin + e % nrows;
+      const int q = e / nrows;
+      const int t = (int)(gr / QF_ROWS), r = (int)(gr % QF_ROWS);
+      // the CTAs whose ranges meet row tile t: owner(c) = floor(((c + 1) * G - 1) / TC)
+      const int i_lo = (int)((((int64_t)t * C + 1) * G - 1) / TC);
+      const int i_hi = (int)((((int64_t)(t + 1) * C) * G - 1) / TC);
+      const float4* src = reinterpret_cast<const float4*>(p.slots) + ((int64_t)i_lo + t) * SLOT_F4 + q * QF_ROWS + r;
+      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+      for (int i = i_lo; i <= i_hi; i += 4) {   // four loads in flight, added in order
+        float4 v[4];
 #pragma unroll
-        for (int q = 0; q < 8; ++q)   // all remote loads in flight before the first add
-          if (q < split) v[q] = ld_dsmem_f32x2(part_u + (r * R_T + c) * 4, q);
+        for (int j = 0; j < 4; ++j)
+          v[j] = (i + j <= i_hi) ? __ldcg(src + (int64_t)j * SLOT_F4) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-        for (int q = 0; q < 8; ++q)
-          if (q < split) {
-            s0 += v[q].x;
-            s1 += v[q].y;
+        for (int j = 0; j < 4; ++j) {
+          acc.x += v[j].x;
+          acc.y += v[j].y;
+          acc.z += v[j].z;
+          acc.w += v[j].w;
+        }
+        src += 4 * (int64_t)SLOT_F4;
+      }
+      if (p.h_out != nullptr)
+        *reinterpret_cast<uint2*>(p.h_out + gr * R_T + q * 4) =
+            make_uint2(pack_bf16x2(acc.x, acc.y), pack_bf16x2(acc.z, acc.w));
+      if (p.hs_out != nullptr)
+        *reinterpret_cast<uint2*>(p.hs_out + gr * R_T + q * 4) =
+            make_uint2(pack_bf16x2(__fmul_rn(acc.x, inv_alpha), __fmul_rn(acc.y, inv_alpha)),
+                       pack_bf16x2(__fmul_rn(acc.z, inv_alpha), __fmul_rn(acc.w, inv_alpha)));
+    }
+  };
+
+  if constexpr (!SINGLE) {
+    // =========================================================== streaming mode (amax known)
+    // a stage = the X chunk and its D slice; both land on full_x[slot] (issue_d is given that barrier)
+    auto issue_stage = [&](int it, int slot) {
+      const int64_t c = c_begin + it;
+      const int t = (int)(c / C), kc = (int)(c % C);
+#ifdef QF_EXP_NO_D
+      mbar_expect_tx(&full_x[slot], QF_X_BYTES);
+#else
+      mbar_expect_tx(&full_x[slot], QF_X_BYTES + (R_T > 0 ? D_BYTES : 0));
+#endif
+      tma_load_2d(smem + slot * QF_X_BYTES, &map_x, &full_x[slot], kc * QF_KC, t * QF_ROWS);
+#ifndef QF_EXP_NO_D
+      if constexpr (R_T > 0) {
+#pragma unroll
+        for (int g = 0; g < NG; ++g)
+          tma_load_2d(smem + NXS * QF_X_BYTES + slot * D_BYTES + g * QF_DG_BYTES, &map_d, &full_x[slot], g * 64,
+                      kc * QF_KC);
+      }
+#endif
+    };
+    const TensorScale ts = tensor_scale(__ldg(p.amax_in));
+    // Hs = bf16(H * (1 / alpha)), alpha = g_dec(this) * g_dec(other): one IEEE divide per CTA
+    float inv_alpha = 1.0f;
+    if (R_T > 0 && p.hs_out != nullptr) inv_alpha = __fdiv_rn(1.0f, __fmul_rn(ts.g_dec, __ldg(p.other_dec_scale)));
+    if (blockIdx.x == 0 && tid == 0) *p.g_dec_out = ts.g_dec;
+    if (tid < 128) enc_tab[tid] = enc_of_sf8((uint32_t)tid, ts.g_dec);
+    __syncthreads();
+
+    if (warp == 16) {
+      // ===== TMA producer: keeps the ring full; a slot is re-armed once the 16 quantizer warps and
+      // the MMAs that read it have released it
+      if (lane == 0) {
+        int sx = 0;
+        uint32_t phx = 0;
+        for (int it = 0; it < n; ++it) {
+          if (it >= NXS) mbar_wait(&empty_x[sx], phx ^ 1);
+          issue_stage(it, sx);
+          if (++sx == NXS) {
+            sx = 0;
+            phx ^= 1;
           }
-      } else {
-        s0 = part[r * R_T + c];
-        s1 = part[r * R_T + c + 1];
+        }
       }
-      const int64_t gr = row0 + r;
-      if (gr < p.rows) {
-        if (p.h_out != nullptr)
-          *reinterpret_cast<uint32_t*>(p.h_out + gr * R_T + c) = pack_bf16x2(s0, s1);
-        if (p.hs_out != nullptr)
-          *reinterpret_cast<uint32_t*>(p.hs_out + gr * R_T + c) =
-              pack_bf16x2(__fdiv_rn(s0, alpha), __fdiv_rn(s1, alpha));
+    } else if (warp == 17) {
+      // ===== tcgen05 issuer: never waits for an MMA to complete, the MMAs of successive chunks pipeline
+      if constexpr (R_T > 0) {
+        if (lane == 0) {
+          int sx = 0, kc = o_kc, seg = 0;
+          uint32_t phx = 0;
+          bool first = true;
+          for (int it = 0; it < n; ++it) {
+            const bool seg_end = (kc == C - 1) || (it == n - 1);
+            mbar_wait(&full_x[sx], phx);
+            if (first && seg >= 2) mbar_wait(&acc_free[seg & 1], (uint32_t)((seg >> 1) - 1) & 1);
+            tc_fence_after();
+            issue_mma(xs_u + sx * QF_X_BYTES, ds_u + sx * D_BYTES, tmem_base_s + (seg & 1) * ACC_COLS, first);
+            tc_commit(&empty_x[sx]);                      // slot free once the MMAs have read it
+            first = false;
+            if (seg_end) {
+              tc_commit(&acc_full[seg & 1]);              // this segment's accumulator is complete
+              ++seg;
+              first = true;
+            }
+            if (++kc == C) kc = 0;
+            if (++sx == NXS) {
+              sx = 0;
+              phx ^= 1;
+            }
+          }
+        }
       }
+    } else {
+      // ===== quantizer warps
+      int seg = 0;
+      int sx = 0;            // ring slot of chunk `it`
+      uint32_t phx = 0;      // and its barrier parity
+      for (int it = 0; it < n; ++it) {
+        mbar_wait(&full_x[sx], phx);
+        quantize_chunk(xs_u + sx * QF_X_BYTES, ts.g_enc);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty_x[sx]);  // this warp is done with the slot
+        if constexpr (R_T > 0) {
+          if ((o_kc == C - 1) || (it == n - 1)) {   // end of a row-tile segment
+            drain_segment(o_t, seg);
+            ++seg;
+          }
+        }
+        advance_out();
+        if (++sx == NXS) {
+          sx = 0;
+          phx ^= 1;
+        }
+      }
+      QF_STAMP(2);
+      if constexpr (R_T > 0) {
+        grid_barrier(p.grid_bar + 1);
+        QF_STAMP(3);
+        finalize_share(inv_alpha);
+      }
+      QF_STAMP(4);
     }
-    if (split > 1) cluster_sync_all();  // keep this CTA's smem alive until all peers have read it
+  } else {
+    // =========================================================== single-pass mode
+    const int nd = p.nd;
+    const int n0 = min(n, C - o_kc);                         // chunks in the first row tile
+    if (warp == 16) {
+      // ===== TMA producer: the whole range stays resident; the D slices go through a small ring
+      if (lane == 0) {
+        for (int it = 0; it < n; ++it) issue_x(it, it);
+        if constexpr (R_T > 0) {
+          int sd = 0;
+          uint32_t phd = 0;
+          for (int it = 0; it < n; ++it) {
+            if (it >= nd) mbar_wait(&empty_d[sd], phd ^ 1);
+            issue_d(it, sd);
+            if (++sd == nd) {
+              sd = 0;
+              phd ^= 1;
+            }
+          }
+        }
+      }
+    } else if (warp == 17) {
+      // ===== tcgen05 issuer: the projection MMAs as the chunks land (row-tile segment 0 / 1)
+      if constexpr (R_T > 0) {
+        if (lane == 0) {
+          int sd = 0;
+          uint32_t phd = 0;
+          for (int it = 0; it < n; ++it) {
+            const int sg = it < n0 ? 0 : 1;
+            mbar_wait(&full_x[it], 0);
+            mbar_wait(&full_d[sd], phd);
+            tc_fence_after();
+            issue_mma(xs_u + it * QF_X_BYTES, ds_u + sd * D_BYTES, tmem_base_s + sg * ACC_COLS,
+                      it == 0 || it == n0);
+            tc_commit(&empty_d[sd]);
+            if (it == n0 - 1 || it == n - 1) tc_commit(&acc_full[sg]);
+            if (++sd == nd) {
+              sd = 0;
+              phd ^= 1;
+            }
+          }
+        }
+      }
+    } else {
+    // ===== quantizer warps
+    // ---- phase 1: tensor amax as the chunks land
+    uint32_t m2 = 0;
+    for (int it = 0; it < n; ++it) {
+      mbar_wait(&full_x[it], 0);
+      uint4 v0, v1;
+      load_block(xs_u + it * QF_X_BYTES, v0, v1);
+      m2 = absmax2_bf16(m2, absmax2_bf16(absmax2_bf16(absmax2_bf16(v0.x, v0.y), absmax2_bf16(v0.z, v0.w)),
+                                         absmax2_bf16(absmax2_bf16(v1.x, v1.y), absmax2_bf16(v1.z, v1.w))));
+    }
+    QF_STAMP(2);
+    m2 &= 0x7FFF7FFFu;
+    uint32_t best = max(m2 & 0xFFFFu, m2 >> 16);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(0xffffffffu, best, o));
+    if (lane == 0) s_red[warp] = best;
+    qsync();
+    if (tid == 0) {
+      for (int w = 1; w < QF_QTHREADS / 32; ++w) best = max(best, s_red[w]);
+      atomicMax(p.amax_bits, best << 16);   // bf16 bits -> float bits; non-negative floats order as uints
+      __threadfence();
+      atomicAdd(p.grid_bar, 1u);
+    }
+    // ---- partial H tiles out while the other CTAs arrive
+    if constexpr (R_T > 0) {
+      drain_segment(o_t, 0);
+      if (n > n0) drain_segment(o_t + 1, 1);
+    }
+    QF_STAMP(3);
+    // ---- grid-wide barrier: every CTA has published its amax
+    if (tid == 0) {
+      const uint64_t t0 = globaltimer_ns();
+      while (ld_acquire_u32(p.grid_bar) < gridDim.x) {
+        if (globaltimer_ns() - t0 > 2000000000ull) __trap();   // co-residency broken: fail, do not hang
+      }
+      s_amax = ld_acquire_u32(p.amax_bits);
+    }
+    qsync();
+    const TensorScale ts = tensor_scale(__uint_as_float(s_amax));
+    float inv_alpha = 1.0f;
+    if (R_T > 0 && p.hs_out != nullptr) inv_alpha = __fdiv_rn(1.0f, __fmul_rn(ts.g_dec, __ldg(p.other_dec_scale)));
+    if (blockIdx.x == 0 && tid == 0) *p.g_dec_out = ts.g_dec;
+    if (tid < 128) enc_tab[tid] = enc_of_sf8((uint32_t)tid, ts.g_dec);
+    qsync();
+    QF_STAMP(4);
+    // ---- phase 2: quantize from shared memory
+    for (int it = 0; it < n; ++it) {
+      quantize_chunk(xs_u + it * QF_X_BYTES, ts.g_enc);
+      advance_out();
+    }
+    QF_STAMP(5);
+    if constexpr (R_T > 0) {
+      grid_barrier(p.grid_bar + 1);   // every CTA's slots are written
+      finalize_share(inv_alpha);
+    }
+    QF_STAMP(6);
+    }
+  }
+
+  if constexpr (R_T > 0) {
+    tc_fence_before();
+    __syncthreads();
     if (warp == 2) {
       tc_fence_after();
-      tmem_dealloc(tmem_base_s, TMEM_COLS);
+      tmem_dealloc(tmem_base_s, 2 * ACC_COLS);
     }
   }
 }
 
-template <int R_T>
-static int choose_split(int64_t rows, int64_t cols, int smem);
+int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first);
+
+#ifdef FT_QF_TIMING
+static long long* g_qf_dbg = nullptr;
+extern "C" void ft_debug_set_timing_buffer(void* b) { g_qf_dbg = reinterpret_cast<long long*>(b); }
+#endif
+static int g_qf_mode = 0;   // 0 auto, 1 never single pass, 2 (= auto; single pass whenever it fits)
+void set_quantize_mode(int mode) { g_qf_mode = mode; }
 
 template <int R_T>
-static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, const QFParams& p_in,
+static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, const void* x, const float* amax_t,
                      cudaStream_t st) {
   constexpr int NG = (R_T + 63) / 64;
-  constexpr int QF_STAGES = (NG == 2) ? 3 : 4;
-  const int smem = QF_STAGES * (QF_X_BYTES + NG * QF_DG_BYTES) + 1024;
-  static_assert(QF_ROWS * (R_T > 0 ? R_T : 1) * 4 <= QF_STAGES * (QF_X_BYTES + NG * QF_DG_BYTES),
-                "partial H tile must fit in the ring");
-  FT_CUDA_TRY(cudaFuncSetAttribute(k_quantize_fused<R_T>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  FT_CUDA_TRY(cudaFuncSetAttribute(k_quantize_fused<R_T>, cudaFuncAttributePreferredSharedMemoryCarveout,
-                                   cudaSharedmemCarveoutMaxShared));
-  QFParams p = p_in;
-  p.split = choose_split<R_T>(p.rows, p.cols, smem);
+  constexpr int D_BYTES = NG * QF_DG_BYTES;
+  constexpr int SMEM_MAX = 227 * 1024 - 2048;   // minus the static shared memory (barriers, table)
+  const int nsm = sm_count();
+  const int64_t TC = p.total_chunks;
+  const int C = p.chunks_per_tile;
+  static bool attr_set = false;
+  if (!attr_set) {
+    FT_CUDA_TRY(cudaFuncSetAttribute(k_quantize_fused<R_T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    FT_CUDA_TRY(cudaFuncSetAttribute(k_quantize_fused<R_T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_MAX));
+    FT_CUDA_TRY(cudaFuncSetAttribute(k_quantize_fused<R_T, false>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                     cudaSharedmemCarveoutMaxShared));
+    attr_set = true;
+  }
+  // ---- single pass: the tensor amax is not known and every CTA can keep its whole range resident
+  if (amax_t == nullptr && g_qf_mode != 1) {
+    const int64_t G = TC < nsm ? TC : (nsm < QF_MAX_GRID ? nsm : QF_MAX_GRID);
+    const int64_t n_max = ceil_div(TC, G);
+    const int nd = R_T == 0 ? 0 : (NG == 2 ? 2 : 3);
+    int smem = (int)n_max * QF_X_BYTES + nd * D_BYTES + 1024;
+    if (smem < 512 * R_T + 1024) smem = 512 * R_T + 1024;   // the finalizer stages two bf16 tiles in the ring
+    if (n_max <= QF_MAX_NX && smem <= SMEM_MAX && (R_T == 0 || n_max <= C)) {
+      p.single = 1;
+      p.nx = (int)n_max;
+      p.nd = nd > 0 ? nd : 1;
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)G, 1, 1);
+      cfg.blockDim = dim3(QF_THREADS, 1, 1);
+      cfg.dynamicSmemBytes = smem;
+      cfg.stream = st;
+      cudaLaunchAttribute attr[1];
+      attr[0].id = cudaLaunchAttributeCooperative;   // the grid barrier needs every CTA resident
+      attr[0].val.cooperative = 1;
+      cfg.attrs = attr;
+      cfg.numAttrs = 1;
+      const cudaError_t e = cudaLaunchKernelEx(&cfg, k_quantize_fused<R_T, true>, mx, md, p);
+      if (e == cudaSuccess) return FT_OK;
+      if (e != cudaErrorCooperativeLaunchTooLarge && e != cudaErrorNotSupported) {
+        g_last_cuda_error = (int)e;
+        return FT_ERR_CUDA;
+      }
+      (void)cudaGetLastError();   // cannot be co-resident here: two passes instead
+    }
+  }
+  // ---- streaming: amax first (unless the caller supplied it), then a 2-CTA/SM ring kernel
+  if (amax_t == nullptr) {
+    int rc = launch_amax(x, p.rows * p.cols, reinterpret_cast<float*>(p.amax_bits), st, /*zero_first=*/false);
+    if (rc != FT_OK) return rc;
+    amax_t = reinterpret_cast<const float*>(p.amax_bits);
+  }
+  p.single = 0;
+  p.amax_in = amax_t;
+  p.nx = NG == 2 ? 3 : 4;   // = NXS of the kernel
+  p.nd = p.nx;
+  const int smem = p.nx * QF_X_BYTES + (R_T == 0 ? 0 : p.nd * D_BYTES) + 1024;
+  static int occ = 0;       // resident CTAs per SM of this instantiation (the grid barrier needs co-residency)
+  if (occ == 0) {
+    FT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_quantize_fused<R_T, false>, QF_THREADS, smem));
+    if (occ < 1) return FT_ERR_CUDA;
+    if (occ > 2) occ = 2;
+  }
+  int64_t cap = (int64_t)nsm * occ;
+  if (cap > QF_MAX_GRID) cap = QF_MAX_GRID;
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)ceil_div(p.rows, QF_ROWS), (unsigned)p.split, 1);
+  cfg.gridDim = dim3((unsigned)(TC < cap ? TC : cap), 1, 1);
   cfg.blockDim = dim3(QF_THREADS, 1, 1);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = 1;
-  attr[0].val.clusterDim.y = (unsigned)p.split;
-  attr[0].val.clusterDim.z = 1;
+  attr[0].id = cudaLaunchAttributeCooperative;
+  attr[0].val.cooperative = R_T > 0 ? 1 : 0;   // only the projection ends in a grid barrier
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_quantize_fused<R_T>, mx, md, p));
+  FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_quantize_fused<R_T, false>, mx, md, p));
   return FT_OK;
 }
 
-// Cluster size (= K split) of the fused kernel: any 1..8.  Clusters are co-scheduled inside a
-// GPC, so not every size packs the chip equally; ask the driver how many clusters of each size
-// fit at once and minimise  waves * chunks-per-CTA  (ties: the larger split = more warps).
-template <int R_T>
-static int choose_split(int64_t rows, int64_t cols, int smem) {
-  const int64_t tiles = ceil_div(rows, QF_ROWS), chunks = cols / QF_KC;
-  if (const char* e = getenv("FT_QF_SPLIT")) {
-    const int v = atoi(e);
-    if (v > 0 && v <= 8 && v <= chunks) return v;
-  }
-  static int max_active[9] = {0};   // per instantiation; device properties do not change
-  int best = 1;
-  double best_cost = 1e30;
-  for (int s = 1; s <= 8 && s <= chunks; ++s) {
-    if (max_active[s] == 0) {
-      cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3(1, (unsigned)s, 1);
-      cfg.blockDim = dim3(QF_THREADS, 1, 1);
-      cfg.dynamicSmemBytes = smem;
-      cudaLaunchAttribute attr[1];
-      attr[0].id = cudaLaunchAttributeClusterDimension;
-      attr[0].val.clusterDim.x = 1;
-      attr[0].val.clusterDim.y = (unsigned)s;
-      attr[0].val.clusterDim.z = 1;
-      cfg.attrs = attr;
-      cfg.numAttrs = 1;
-      int n = 0;
-      if (cudaOccupancyMaxActiveClusters(&n, k_quantize_fused<R_T>, &cfg) != cudaSuccess || n < 1) {
-        (void)cudaGetLastError();
-        n = -1;
-      }
-      max_active[s] = n;
-    }
-    if (max_active[s] < 1) continue;
-    const double waves = (double)ceil_div(tiles, max_active[s]);
-    const double cost = waves * (double)ceil_div(chunks, s) + 1.5;   // + a fixed head/tail per CTA
-    if (cost <= best_cost) {
-      best_cost = cost;
-      best = s;
-    }
-  }
-  if (getenv("FT_QF_DEBUG")) {
-    fprintf(stderr, "[qf] r_t=%d rows=%ld cols=%ld split=%d max_active:", R_T, (long)rows, (long)cols, best);
-    for (int s = 1; s <= 8; ++s) fprintf(stderr, " %d", max_active[s]);
-    fprintf(stderr, "\n");
-  }
-  return best;
-}
-
-int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t,
-                          const ft_proj* proj, ft_qtensor* out, cudaStream_t st) {
+// Workspace use (offsets from ws_layout, common.cuh): the zero region holds the amax word and the two
+// grid-barrier counters; it is cleared here with one 256-byte memset node.  The partial-H slots behind
+// it need no clearing.
+int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t, const ft_proj* proj,
+                          ft_qtensor* out, void* workspace, cudaStream_t st) {
   const int r_t = proj ? proj->r_t : 0;
   CUtensorMap mx, md;
-  int rc = make_tensor_map_2d(&mx, x, 2, (uint64_t)cols, (uint64_t)rows, (uint64_t)cols * 2, QF_KC,
-                              QF_ROWS, Swizzle::B128);
+  int rc = make_tensor_map_2d(&mx, x, 2, (uint64_t)cols, (uint64_t)rows, (uint64_t)cols * 2, QF_KC, QF_ROWS,
+                              Swizzle::B128);
   if (rc != FT_OK) return rc;
   if (r_t > 0) {
-    rc = make_tensor_map_2d(&md, proj->down, 2, (uint64_t)r_t, (uint64_t)cols, (uint64_t)r_t * 2, 64,
-                            QF_KC, Swizzle::B128);
+    rc = make_tensor_map_2d(&md, proj->down, 2, (uint64_t)r_t, (uint64_t)cols, (uint64_t)r_t * 2, 64, QF_KC,
+                            Swizzle::B128);
     if (rc != FT_OK) return rc;
   } else {
     md = mx;
   }
-  QFParams p;
+  if (rows * (cols / 2) >= ((int64_t)1 << 32)) return FT_ERR_UNSUPPORTED_SHAPE;   // 32-bit output cursors
+  const WsLayout w = ws_layout(rows, r_t);
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  QFParams p = {};
   p.rows = rows;
   p.cols = cols;
-  p.amax_t = amax_t;
+  p.amax_in = amax_t;
+  p.amax_bits = reinterpret_cast<uint32_t*>(ws + w.amax_off);
+  p.grid_bar = reinterpret_cast<uint32_t*>(ws + w.bar_off);
+  p.slots = reinterpret_cast<float*>(ws + w.slots_off);
   p.codes = out->codes;
   p.sf = out->sf;
   p.g_dec_out = out->tensor_dec_scale;
@@ -394,22 +649,27 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
   p.h_out = proj ? reinterpret_cast<__nv_bfloat16*>(proj->out) : nullptr;
   p.hs_out = proj ? reinterpret_cast<__nv_bfloat16*>(proj->out_scaled) : nullptr;
   p.other_dec_scale = proj ? proj->other_dec_scale : nullptr;
-  p.split = 1;
+#ifdef FT_QF_TIMING
+  p.dbg = g_qf_dbg;
+#endif
+  p.chunks_per_tile = (int)(cols / QF_KC);
+  p.total_chunks = ceil_div(rows, QF_ROWS) * (cols / QF_KC);
+  if (amax_t == nullptr || r_t > 0) FT_CUDA_TRY(cudaMemsetAsync(ws + w.zero_off, 0, w.zero_bytes, st));
   // padding rows of the last 128-row scale tile must read as zero
   if (out->sf_layout == FT_SF_TILE128x4 && rows % 128 != 0) {
     const int64_t tiles_c = ceil_div(cols / 16, 4);
     FT_CUDA_TRY(cudaMemsetAsync(out->sf + (rows / 128) * tiles_c * 512, 0, tiles_c * 512, st));
   }
   switch (r_t) {
-    case 0: return launch_qf<0>(mx, md, p, st);
-    case 16: return launch_qf<16>(mx, md, p, st);
-    case 32: return launch_qf<32>(mx, md, p, st);
-    case 48: return launch_qf<48>(mx, md, p, st);
-    case 64: return launch_qf<64>(mx, md, p, st);
-    case 80: return launch_qf<80>(mx, md, p, st);
-    case 96: return launch_qf<96>(mx, md, p, st);
-    case 112: return launch_qf<112>(mx, md, p, st);
-    case 128: return launch_qf<128>(mx, md, p, st);
+    case 0: return launch_qf<0>(mx, md, p, x, amax_t, st);
+    case 16: return launch_qf<16>(mx, md, p, x, amax_t, st);
+    case 32: return launch_qf<32>(mx, md, p, x, amax_t, st);
+    case 48: return launch_qf<48>(mx, md, p, x, amax_t, st);
+    case 64: return launch_qf<64>(mx, md, p, x, amax_t, st);
+    case 80: return launch_qf<80>(mx, md, p, x, amax_t, st);
+    case 96: return launch_qf<96>(mx, md, p, x, amax_t, st);
+    case 112: return launch_qf<112>(mx, md, p, x, amax_t, st);
+    case 128: return launch_qf<128>(mx, md, p, x, amax_t, st);
     default: return FT_ERR_UNSUPPORTED_SHAPE;
   }
 }

@@ -66,13 +66,32 @@ QCASES = [  # rows, cols, kind, layout
     (256, 3072, "x", 1), (256, 3072, "g", 1), (384, 15360, "x", 1)]
 
 
-@pytest.mark.parametrize("rows,cols,kind,layout", QCASES)
-def test_quantize_1x16_bit_exact(B, rows, cols, kind, layout):
+@pytest.fixture(params=[0, 1], ids=["single_pass", "two_pass"])
+def qmode(request, B):
+    """Both routes to the tensor amax: inside the quantize kernel (grid barrier, tensor resident
+    in shared memory) and the separate k_amax launch followed by the streaming kernel."""
+    B.debug_set_quantize_mode(request.param)
+    yield request.param
+    B.debug_set_quantize_mode(0)
+
+
+@pytest.mark.parametrize("rows,cols,kind,layout", QCASES + [(2304, 3072, "x", 1), (4608, 3072, "g", 1)])
+def test_quantize_1x16_bit_exact(B, qmode, rows, cols, kind, layout):
     rng = synth.make_rng(rows * 131 + cols)
     x = synth.outlier_normal(rng, rows, cols) if kind == "x" else synth.student_t_grad(rng, rows, cols)
     out = B.QTensor(rows, cols, 1, layout)
     B.ft_quantize_blockwise(t16(x), out)
     assert_q_equal(out, nvfp4.quantize_blockwise(x, 1), layout, B)
+
+
+def test_quantize_with_caller_amax(B):
+    """tensor_amax supplied by the caller (delayed / static scaling): streaming kernel only."""
+    rng = synth.make_rng(77)
+    x = synth.outlier_normal(rng, 300, 1024)
+    xt = t16(x)
+    out = B.QTensor(300, 1024, 1, B.FT_SF_TILE128x4)
+    B.ft_quantize_blockwise(xt, out, tensor_amax=B.ft_tensor_amax(xt))
+    assert_q_equal(out, nvfp4.quantize_blockwise(x, 1), B.FT_SF_TILE128x4, B)
 
 
 def test_quantize_degenerate_inputs(B):
@@ -113,8 +132,9 @@ def test_weight_quantize_16x16_and_pack(B, N, K):
 
 
 @pytest.mark.parametrize("rows,cols,r_t,kind", [(128, 512, 16, "x"), (200, 1024, 64, "x"), (256, 3072, 48, "x"),
-                                                (384, 2048, 96, "g"), (130, 4096, 128, "g")])
-def test_fused_projection(B, rows, cols, r_t, kind):
+                                                (384, 2048, 96, "g"), (130, 4096, 128, "g"), (1, 64, 32, "x"),
+                                                (2000, 128, 64, "x"), (4608, 3072, 64, "x"), (2304, 3072, 128, "g")])
+def test_fused_projection(B, qmode, rows, cols, r_t, kind):
     rng = synth.make_rng(rows + cols + r_t)
     x = synth.outlier_normal(rng, rows, cols) if kind == "x" else synth.student_t_grad(rng, rows, cols)
     D = synth.normal(rng, (cols, r_t), 0.01)
