@@ -185,12 +185,11 @@ def run_ours(args):
 
     def step():
         B.ft_linear_fwd(layer, X, y, h, qx, ws)
-        B.ft_linear_bwd_dgrad(layer, G, dx, p, qg, ws)
-        B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt)
+        B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws)
         if world > 1:
             parallel.allreduce_lora_grads(dA, dBt)
-    # fwd: k_quantize_fused (single pass, amax inside) + k_gemm4_pair; bwd: k_amax + k_quantize_fused +
-    # k_gemm4_pair; wgrad: k_wgrad (memsets not counted)
+    # fwd: k_quantize_fused (single pass, amax inside) + k_gemm4_pair; bwd (ft_linear_bwd): k_wgrad (dB^T + amax
+    # of G) + k_quantize_fused + k_gemm4_pair + k_wgrad (dA); memsets not counted
     KERNELS_PER_STEP = 6
 
     def barrier():
@@ -303,6 +302,8 @@ def run_ours(args):
         workspace=ws))
     kern["gemm_dgrad_us"] = timed(lambda: B.ft_gemm4(qg, layer.r_nmajor, hs, D_f, dx))
     kern["wgrad_us"] = timed(lambda: B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt))
+    kern["bwd_fused_us"] = timed(lambda: B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws))
+    kern["fwd_us"] = timed(lambda: B.ft_linear_fwd(layer, X, y, h, qx, ws))
 
     # bf16 cuBLAS LoRA layer on the same GPU, same shapes (context: speedup vs BF16 LoRA)
     Am, Bm = A, Bt.t().contiguous()
@@ -424,8 +425,7 @@ def sweep(B, prepare, dev, timed, peaks, full=False):
 
         def step():
             B.ft_linear_fwd(layer, X, y, h, qx, ws)
-            B.ft_linear_bwd_dgrad(layer, G, dx, p, qg, ws)
-            B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt)
+            B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws)
         for _ in range(3):
             step()
         torch.cuda.synchronize()

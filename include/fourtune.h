@@ -163,6 +163,16 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
                   const void* h_saved_bf16, const void* p_saved_bf16, float* dA,
                   float* dBt, int32_t accumulate, void* stream);
 
+/* ---- a0+a3+a4+a5 in one call: the whole backward of the layer (Eq. 3 and Eq. 4).
+ * Same results as ft_linear_bwd_dgrad followed by ft_lora_wgrad, different schedule: the pass
+ * over G that computes dBt = G^T (X A) also finds max |G|, so the separate amax pass of the
+ * quantizer disappears (G is read twice instead of three times); dA = X^T (G B^T) runs last
+ * because it needs P.  Arguments as in the two calls above. */
+int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
+                  const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
+                  int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
+                  void* stream);
+
 /* ---- sizes and diagnostics (host only, no CUDA calls) */
 size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout);
 size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t);

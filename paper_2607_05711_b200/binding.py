@@ -55,6 +55,7 @@ def lib():
         L.ft_linear_bwd_dgrad.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
         L.ft_gemm4.argtypes = [C.POINTER(_QT), C.POINTER(_QT), vp, vp, i32, vp, vp]
         L.ft_lora_wgrad.argtypes = [C.POINTER(_Layer), vp, vp, i64, vp, vp, vp, vp, i32, vp]
+        L.ft_linear_bwd.argtypes = [C.POINTER(_Layer), vp, vp, i64, vp, vp, vp, vp, vp, i32, C.POINTER(_QT), vp, sz, vp]
         L.ft_sf_bytes.argtypes = [i64, i64, i32, i32]
         L.ft_sf_bytes.restype = sz
         L.ft_workspace_bytes.argtypes = [i64, i64, i64, i32]
@@ -201,6 +202,17 @@ def ft_lora_wgrad(layer, x, g, h_saved, p_saved, dA, dBt, accumulate=False, stre
     _check(lib().ft_lora_wgrad(C.byref(L), _ptr(x), _ptr(g), x.shape[0], _ptr(h_saved), _ptr(p_saved),
                                _ptr(dA), _ptr(dBt), 1 if accumulate else 0, _stream(stream)))
     return dA, dBt
+
+
+def ft_linear_bwd(layer, x, g, h_saved, dx, p_saved, dA, dBt, qg, workspace, accumulate=False, stream=None):
+    """dgrad + LoRA wgrad in one call (one pass over g serves dBt and the tensor amax)."""
+    _bf16(x), _bf16(g)
+    L, q = layer.c(), qg.c()
+    _check(lib().ft_linear_bwd(C.byref(L), _ptr(x), _ptr(g), g.shape[0], _ptr(h_saved), _ptr(dx), _ptr(p_saved),
+                               _ptr(dA), _ptr(dBt), 1 if accumulate else 0, C.byref(q), _ptr(workspace),
+                               workspace.numel(), _stream(stream)))
+    qg.sync_from(q)
+    return dx, dA, dBt
 
 
 def debug_set_gemm_tile_n(bn):

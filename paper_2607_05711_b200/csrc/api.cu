@@ -21,9 +21,9 @@ int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N,
                  cudaStream_t st);
 int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
                       const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st);
-int launch_wgrad_pair(const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
-                      const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                      cudaStream_t st);
+int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
+                 const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
+                 unsigned int* amax_g, cudaStream_t st);
 
 // ------------------------------------------------------------- device queries
 static int g_sm_count = 0;
@@ -91,10 +91,11 @@ static bool valid_rt(int r_t) { return r_t >= 0 && r_t <= 128 && r_t % 16 == 0; 
 
 // one direction of the layer: quantize `act` [M x Kd] (+ projection by lr_down
 // [Kd x r_t]) and multiply with the weight operand `w` ([Nd x Kd]); lr_up [Nd x r_t].
+// act_amax: device float with max |act| if the caller already has it (the fused backward), else NULL.
 static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_up, int r_t,
                        const void* act, int64_t M, int64_t Kd, int64_t Nd, void* out,
                        void* saved, ft_qtensor* q, void* workspace, size_t ws_bytes,
-                       cudaStream_t st) {
+                       const float* act_amax, cudaStream_t st) {
   if (!act || !out || !q || !q->codes || !q->sf || !q->tensor_dec_scale || !workspace)
     return FT_ERR_INVALID_ARG;
   if (r_t > 0 && (!saved || !lr_down || !lr_up)) return FT_ERR_INVALID_ARG;
@@ -118,7 +119,7 @@ static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_
   pr.r_t = r_t;
   // a0 + a1/a3: the tensor amax is found inside the quantize pass when the tensor fits the SMs'
   // shared memory (single pass), by a preceding k_amax launch otherwise
-  rc = launch_quantize_fused(act, M, Kd, nullptr, r_t > 0 ? &pr : nullptr, q, workspace, st);
+  rc = launch_quantize_fused(act, M, Kd, act_amax, r_t > 0 ? &pr : nullptr, q, workspace, st);
   if (rc != FT_OK) return rc;
   return launch_gemm4(q, w, M, Nd, Kd, r_t > 0 ? hs : nullptr, lr_up, r_t, out, st);
 }
@@ -276,7 +277,7 @@ int ft_linear_fwd(const ft_layer* L, const void* x_bf16, int64_t M, void* y_bf16
   int rc = check_layer(L);
   if (rc != FT_OK) return rc;
   return linear_pass(&L->r_kmajor, L->D_f, L->U_t, L->r_s + L->r, x_bf16, M, L->K, L->N, y_bf16,
-                     h_saved_bf16, qx_scratch, workspace, workspace_bytes, (cudaStream_t)stream);
+                     h_saved_bf16, qx_scratch, workspace, workspace_bytes, nullptr, (cudaStream_t)stream);
 }
 
 int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* dx_bf16,
@@ -285,26 +286,56 @@ int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* 
   int rc = check_layer(L);
   if (rc != FT_OK) return rc;
   return linear_pass(&L->r_nmajor, L->U_t, L->D_f, L->r_s + L->r, g_bf16, M, L->N, L->K, dx_bf16,
-                     p_saved_bf16, qg_scratch, workspace, workspace_bytes, (cudaStream_t)stream);
+                     p_saved_bf16, qg_scratch, workspace, workspace_bytes, nullptr, (cudaStream_t)stream);
+}
+
+static int check_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M, const void* h_saved_bf16,
+                       const void* p_saved_bf16, float* dA, float* dBt) {
+  if (!L || !x_bf16 || !g_bf16 || !h_saved_bf16 || !p_saved_bf16 || !dA || !dBt) return FT_ERR_INVALID_ARG;
+  const int r_t = L->r_s + L->r;
+  if (L->r_s < 0 || L->r <= 0 || !valid_rt(r_t) || L->r % 16 != 0 || L->r_s % 8 != 0)
+    return FT_ERR_UNSUPPORTED_SHAPE;
+  if (M < 1 || L->K % 64 != 0 || L->N % 64 != 0) return FT_ERR_UNSUPPORTED_SHAPE;
+  if (!aligned16(x_bf16) || !aligned16(g_bf16) || !aligned16(h_saved_bf16) || !aligned16(p_saved_bf16) ||
+      !aligned16(dA) || !aligned16(dBt))
+    return FT_ERR_INVALID_ARG;
+  return device_check();
 }
 
 int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
                   const void* h_saved_bf16, const void* p_saved_bf16, float* dA, float* dBt,
                   int32_t accumulate, void* stream) {
-  cudaStream_t st = (cudaStream_t)stream;
-  if (!L || !x_bf16 || !g_bf16 || !h_saved_bf16 || !p_saved_bf16 || !dA || !dBt)
-    return FT_ERR_INVALID_ARG;
-  const int r_t = L->r_s + L->r;
-  if (L->r_s < 0 || L->r <= 0 || !valid_rt(r_t) || L->r % 16 != 0 || L->r_s % 8 != 0)
-    return FT_ERR_UNSUPPORTED_SHAPE;
-  if (M < 1 || L->K % 64 != 0 || L->N % 64 != 0) return FT_ERR_UNSUPPORTED_SHAPE;
-  if (!aligned16(x_bf16) || !aligned16(g_bf16) || !aligned16(h_saved_bf16) ||
-      !aligned16(p_saved_bf16) || !aligned16(dA) || !aligned16(dBt))
-    return FT_ERR_INVALID_ARG;
-  int rc = device_check();
+  int rc = check_wgrad(L, x_bf16, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt);
   if (rc != FT_OK) return rc;
-  return launch_wgrad_pair(x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                           accumulate, st);
+  return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, L->r_s + L->r, L->r_s, L->r, dA,
+                      dBt, accumulate, nullptr, (cudaStream_t)stream);
+}
+
+int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
+                  const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
+                  int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
+                  void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc = check_layer(L);
+  if (rc != FT_OK) return rc;
+  rc = check_wgrad(L, x_bf16, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt);
+  if (rc != FT_OK) return rc;
+  if (!workspace || !aligned16(workspace)) return FT_ERR_INVALID_ARG;
+  if (workspace_bytes < ft_workspace_bytes(M, L->N, L->K, L->r_s + L->r)) return FT_ERR_WORKSPACE_TOO_SMALL;
+  const int r_t = L->r_s + L->r;
+  // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0)
+  unsigned int* amax_g = reinterpret_cast<unsigned int*>(workspace);   // header word of the workspace
+  FT_CUDA_TRY(cudaMemsetAsync(amax_g, 0, sizeof(unsigned int), st));
+  rc = launch_wgrad(2, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
+                    accumulate, amax_g, st);
+  if (rc != FT_OK) return rc;
+  // 2. a3 + a4 with that amax: Q(G), P = G U_t, dX
+  rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
+                   workspace, workspace_bytes, reinterpret_cast<const float*>(amax_g), st);
+  if (rc != FT_OK) return rc;
+  // 3. dA = X^T (G B^T) needs P
+  return launch_wgrad(1, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
+                      accumulate, nullptr, st);
 }
 
 }  // extern "C"

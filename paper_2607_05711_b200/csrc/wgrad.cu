@@ -25,6 +25,7 @@ struct WgParams {      // two problems in one launch: [0] dA = X^T P_lora, [1] d
   int chunks_per_cta[2];
   int direct[2];       // 1: a single M slice owns the output, plain stores (no zero-fill needed)
   float* out[2];
+  unsigned int* amax_bits[2];   // non-null: atomicMax target for max |In| (bf16 bits << 16), pre-zeroed
 };
 
 __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
@@ -63,7 +64,7 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
     prefetch_tmap(&map_l);
     for (int s = 0; s < WG_STAGES; ++s) {
       mbar_init(&full_bar[s], 1);
-      mbar_init(&empty_bar[s], 1);
+      mbar_init(&empty_bar[s], p.amax_bits[z] != nullptr ? 3 : 1);   // MMA commit (+ the two amax warps)
     }
     mbar_init(&acc_bar, 1);
     fence_mbar_init();
@@ -109,6 +110,27 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
       }
       tc_commit(&acc_bar);
     }
+  } else if (p.amax_bits[z] != nullptr) {
+    // ---- warps 2-3: max |In| over the staged chunks (|bf16| orders like its low 15 bits)
+    const uint32_t m = 0x7FFF7FFFu;
+    uint32_t acc = 0;
+    const int t64 = tid - 64;
+    for (int it = 0; it < n_chunks; ++it) {
+      const int s = it % WG_STAGES;
+      mbar_wait(&full_bar[s], (it / WG_STAGES) & 1);
+      const uint4* src = reinterpret_cast<const uint4*>(smem + s * STAGE_BYTES);
+#pragma unroll 4
+      for (int j = 0; j < WG_IN_BYTES / 16 / 64; ++j) {
+        const uint4 v = src[t64 + j * 64];
+        acc = __vmaxu2(acc, __vmaxu2(__vmaxu2(v.x & m, v.y & m), __vmaxu2(v.z & m, v.w & m)));
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty_bar[s]);
+    }
+    uint32_t best = max(acc & 0xFFFFu, acc >> 16);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(0xffffffffu, best, o));
+    if (lane == 0 && best != 0) atomicMax(p.amax_bits[z], best << 16);
   }
   __syncwarp();
 
@@ -160,46 +182,57 @@ static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, cuda
   return FT_OK;
 }
 
-// dA [K x r] = X^T P[:, r_s:]  and  dBt [N x r] = G^T H[:, r_s:]  in ONE launch (blockIdx.z picks the
-// problem).  accumulate == 0 and a single M slice: plain stores; otherwise the buffers are zeroed
-// first (accumulate == 0) and the slices combine with fp32 reductions.
-int launch_wgrad_pair(const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
-                      const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                      cudaStream_t st) {
+// which = 1: dA [K x r] = X^T P[:, r_s:];  which = 2: dBt [N x r] = G^T H[:, r_s:];  which = 3: both in
+// ONE launch (blockIdx.z picks the problem).  accumulate == 0 and a single M slice: plain stores;
+// otherwise the buffers are zeroed first (accumulate == 0) and the slices combine with fp32 reductions.
+// amax_g (which & 2 only): pre-zeroed word that receives the bit pattern of max |G|.
+int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
+                 const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
+                 unsigned int* amax_g, cudaStream_t st) {
   CUtensorMap maps[4];
-  const void* in[2] = {x, g};
-  const void* lr[2] = {p_saved, h_saved};
-  const int64_t F[2] = {K, N};
-  float* out[2] = {dA, dBt};
+  const void* in_all[2] = {x, g};
+  const void* lr_all[2] = {p_saved, h_saved};
+  const int64_t F_all[2] = {K, N};
+  float* out_all[2] = {dA, dBt};
   WgParams p;
   p.M = M;
   p.r_s = r_s;
   p.r = r;
   const int64_t chunks = ceil_div(M, WG_MC);
+  // the enabled problems, compacted into z = 0 .. nz-1
+  int sel[2], nz = 0;
+  for (int z = 0; z < 2; ++z)
+    if (which & (1 << z)) sel[nz++] = z;
+  int64_t f_tiles_total = 0;
+  for (int i = 0; i < nz; ++i) f_tiles_total += ceil_div(F_all[sel[i]], WG_F);
+  // M slices: one wave of two resident CTAs per SM over all feature tiles (rounded DOWN: a second,
+  // mostly empty wave costs more than slightly longer slices), at least 8 chunks (512 rows) each
+  int64_t slices = (int64_t)2 * sm_count() / f_tiles_total;
+  if (slices > chunks / 8) slices = chunks / 8;
+  if (slices < 1) slices = 1;
   unsigned gx = 0, gy = 0;
-  for (int z = 0; z < 2; ++z) {
-    int rc = make_tensor_map_2d(&maps[2 * z], in[z], 2, (uint64_t)F[z], (uint64_t)M, (uint64_t)F[z] * 2, 64, WG_MC,
-                                Swizzle::B128);
+  for (int i = 0; i < 2; ++i) {
+    const int z = i < nz ? sel[i] : sel[0];
+    int rc = make_tensor_map_2d(&maps[2 * i], in_all[z], 2, (uint64_t)F_all[z], (uint64_t)M, (uint64_t)F_all[z] * 2, 64,
+                                WG_MC, Swizzle::B128);
     if (rc != FT_OK) return rc;
-    rc = make_tensor_map_2d(&maps[2 * z + 1], lr[z], 2, (uint64_t)r_t, (uint64_t)M, (uint64_t)r_t * 2, 64, WG_MC,
+    rc = make_tensor_map_2d(&maps[2 * i + 1], lr_all[z], 2, (uint64_t)r_t, (uint64_t)M, (uint64_t)r_t * 2, 64, WG_MC,
                             Swizzle::B128);
     if (rc != FT_OK) return rc;
-    const int64_t f_tiles = ceil_div(F[z], WG_F);
-    // M slices: about two resident CTAs per SM, at least 8 chunks (512 rows) per slice
-    int64_t slices = ceil_div((int64_t)2 * sm_count(), f_tiles);
-    if (slices > chunks / 8) slices = chunks / 8;
-    if (slices < 1) slices = 1;
-    p.F[z] = F[z];
-    p.chunks_per_cta[z] = (int)ceil_div(chunks, slices);
-    const unsigned sl = (unsigned)ceil_div(chunks, p.chunks_per_cta[z]);
-    p.direct[z] = (sl == 1 && !accumulate) ? 1 : 0;
-    p.out[z] = out[z];
-    if (!accumulate && !p.direct[z])
-      FT_CUDA_TRY(cudaMemsetAsync(out[z], 0, (size_t)F[z] * r * sizeof(float), st));
-    if ((unsigned)f_tiles > gx) gx = (unsigned)f_tiles;
+    p.F[i] = F_all[z];
+    p.chunks_per_cta[i] = (int)ceil_div(chunks, slices);
+    const unsigned sl = (unsigned)ceil_div(chunks, p.chunks_per_cta[i]);
+    p.direct[i] = (sl == 1 && !accumulate) ? 1 : 0;
+    p.out[i] = out_all[z];
+    p.amax_bits[i] = z == 1 ? amax_g : nullptr;
+    if (i >= nz) continue;
+    if (!accumulate && !p.direct[i])
+      FT_CUDA_TRY(cudaMemsetAsync(out_all[z], 0, (size_t)F_all[z] * r * sizeof(float), st));
+    const unsigned ft = (unsigned)ceil_div(F_all[z], WG_F);
+    if (ft > gx) gx = ft;
     if (sl > gy) gy = sl;
   }
-  const dim3 grid(gx, gy, 2);
+  const dim3 grid(gx, gy, (unsigned)nz);
   switch (r) {
     case 16: return launch_wg<16>(maps, p, grid, st);
     case 32: return launch_wg<32>(maps, p, grid, st);

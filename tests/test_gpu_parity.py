@@ -169,7 +169,7 @@ def make_layer(B, seed, M, K, N, r_s, r, x_kind="outlier"):
     return d, R, D_f, U_f, L
 
 
-def run_layer(B, L, X, G, M, K, N, r_t, r):
+def run_layer(B, L, X, G, M, K, N, r_t, r, fused_bwd=False):
     y = torch.zeros(M, N, dtype=torch.bfloat16, device="cuda")
     dx = torch.zeros(M, K, dtype=torch.bfloat16, device="cuda")
     h = torch.zeros(M, max(r_t, 1), dtype=torch.bfloat16, device="cuda")
@@ -181,13 +181,17 @@ def run_layer(B, L, X, G, M, K, N, r_t, r):
     B.ft_linear_fwd(L, xt, y, h, qx, ws)
     torch.cuda.synchronize()
     hs = scaled()
-    B.ft_linear_bwd_dgrad(L, gt, dx, p, qg, ws)
-    torch.cuda.synchronize()
-    ps = scaled()
     dA = dBt = None
     if r > 0:
         dA = torch.full((K, r), 7.0, dtype=torch.float32, device="cuda")
         dBt = torch.full((N, r), 7.0, dtype=torch.float32, device="cuda")
+    if fused_bwd:
+        B.ft_linear_bwd(L, xt, gt, h, dx, p, dA, dBt, qg, ws)
+    else:
+        B.ft_linear_bwd_dgrad(L, gt, dx, p, qg, ws)
+    torch.cuda.synchronize()
+    ps = scaled()
+    if r > 0 and not fused_bwd:
         B.ft_lora_wgrad(L, xt, gt, h, p, dA, dBt)
     return dict(y=npf(y), dx=npf(dx), h=npf(h), p=npf(p), hs=hs, ps=ps, qx=qx, qg=qg,
                 dA=None if dA is None else dA.cpu().numpy(), dBt=None if dBt is None else dBt.cpu().numpy(),
@@ -209,6 +213,19 @@ def test_layer_small(B, seed, M, K, N, r_s, r, bn):
     finally:
         B.debug_set_gemm_tile_n(0)
     check_layer(B, d, R, D_f, U_f, out, r_s, r)
+
+
+@pytest.mark.parametrize("seed,M,K,N,r_s,r", [(21, 130, 320, 192, 16, 16), (22, 300, 1024, 768, 32, 32),
+                                               (23, 1000, 512, 2048, 0, 16), (24, 64, 2048, 640, 32, 64)])
+def test_layer_fused_backward(B, seed, M, K, N, r_s, r):
+    """ft_linear_bwd = ft_linear_bwd_dgrad + ft_lora_wgrad with the amax of G found by the dB pass."""
+    d, R, D_f, U_f, L = make_layer(B, seed, M, K, N, r_s, r)
+    out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=True)
+    check_layer(B, d, R, D_f, U_f, out, r_s, r)
+    ref = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
+    assert np.array_equal(out["dx"], ref["dx"]) and np.array_equal(out["p"], ref["p"])
+    assert np.array_equal(out["qg"].codes.cpu().numpy(), ref["qg"].codes.cpu().numpy())
+    assert rel(out["dA"], ref["dA"]) < 1e-5 and rel(out["dBt"], ref["dBt"]) < 1e-5
 
 
 def check_layer(B, d, R, D_f, U_f, out, r_s, r, rows=None):
