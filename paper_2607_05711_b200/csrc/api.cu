@@ -14,7 +14,8 @@ void set_quantize_mode(int mode);
 int launch_quantize_generic(const void* x, int64_t rows, int64_t cols, const float* amax_t,
                             ft_qtensor* out, cudaStream_t st);
 int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t,
-                          const ft_proj* proj, ft_qtensor* out, void* workspace, cudaStream_t st);
+                          const ft_proj* proj, ft_qtensor* out, void* workspace, bool zero_region_cleared,
+                          cudaStream_t st);
 int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, cudaStream_t st);
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
                  const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16,
@@ -23,7 +24,7 @@ int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64
                       const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st);
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, cudaStream_t st);
+                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, cudaStream_t st);
 
 // ------------------------------------------------------------- device queries
 static int g_sm_count = 0;
@@ -91,7 +92,8 @@ static bool valid_rt(int r_t) { return r_t >= 0 && r_t <= 128 && r_t % 16 == 0; 
 
 // one direction of the layer: quantize `act` [M x Kd] (+ projection by lr_down
 // [Kd x r_t]) and multiply with the weight operand `w` ([Nd x Kd]); lr_up [Nd x r_t].
-// act_amax: device float with max |act| if the caller already has it (the fused backward), else NULL.
+// act_amax: device float with max |act| if the caller already has it (the fused backward, which has
+// also cleared the workspace's zero region), else NULL.
 static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_up, int r_t,
                        const void* act, int64_t M, int64_t Kd, int64_t Nd, void* out,
                        void* saved, ft_qtensor* q, void* workspace, size_t ws_bytes,
@@ -119,7 +121,7 @@ static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_
   pr.r_t = r_t;
   // a0 + a1/a3: the tensor amax is found inside the quantize pass when the tensor fits the SMs'
   // shared memory (single pass), by a preceding k_amax launch otherwise
-  rc = launch_quantize_fused(act, M, Kd, act_amax, r_t > 0 ? &pr : nullptr, q, workspace, st);
+  rc = launch_quantize_fused(act, M, Kd, act_amax, r_t > 0 ? &pr : nullptr, q, workspace, act_amax != nullptr, st);
   if (rc != FT_OK) return rc;
   return launch_gemm4(q, w, M, Nd, Kd, r_t > 0 ? hs : nullptr, lr_up, r_t, out, st);
 }
@@ -226,7 +228,7 @@ int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols, const 
     }
     return launch_quantize_generic(x_bf16, rows, cols, amax, out, st);
   }
-  return launch_quantize_fused(x_bf16, rows, cols, tensor_amax, proj, out, workspace, st);
+  return launch_quantize_fused(x_bf16, rows, cols, tensor_amax, proj, out, workspace, false, st);
 }
 
 int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, void* stream) {
@@ -308,7 +310,7 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   int rc = check_wgrad(L, x_bf16, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt);
   if (rc != FT_OK) return rc;
   return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, L->r_s + L->r, L->r_s, L->r, dA,
-                      dBt, accumulate, nullptr, (cudaStream_t)stream);
+                      dBt, accumulate, nullptr, nullptr, 0, (cudaStream_t)stream);
 }
 
 int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
@@ -323,19 +325,23 @@ int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   if (!workspace || !aligned16(workspace)) return FT_ERR_INVALID_ARG;
   if (workspace_bytes < ft_workspace_bytes(M, L->N, L->K, L->r_s + L->r)) return FT_ERR_WORKSPACE_TOO_SMALL;
   const int r_t = L->r_s + L->r;
-  // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0)
-  unsigned int* amax_g = reinterpret_cast<unsigned int*>(workspace);   // header word of the workspace
-  FT_CUDA_TRY(cudaMemsetAsync(amax_g, 0, sizeof(unsigned int), st));
+  // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0).  One memset
+  //    clears the workspace's control words (the amax word among them); the kernel also zero-fills dA
+  //    for step 3, so the call enqueues two memset nodes (control words, dBt) instead of four.
+  const WsLayout w = ws_layout(M, r_t);
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  FT_CUDA_TRY(cudaMemsetAsync(ws + w.zero_off, 0, w.zero_bytes, st));
+  unsigned int* amax_g = reinterpret_cast<unsigned int*>(ws + w.amax_ext_off);
   rc = launch_wgrad(2, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                    accumulate, amax_g, st);
+                    accumulate, amax_g, accumulate ? nullptr : dA, accumulate ? 0 : L->K * (int64_t)L->r, st);
   if (rc != FT_OK) return rc;
   // 2. a3 + a4 with that amax: Q(G), P = G U_t, dX
   rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
                    workspace, workspace_bytes, reinterpret_cast<const float*>(amax_g), st);
   if (rc != FT_OK) return rc;
-  // 3. dA = X^T (G B^T) needs P
+  // 3. dA = X^T (G B^T) needs P; its buffer was cleared by step 1 (accumulate == 1: nothing to clear)
   return launch_wgrad(1, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                      accumulate, nullptr, st);
+                      1, nullptr, nullptr, 0, st);
 }
 
 }  // extern "C"

@@ -38,12 +38,13 @@ int sm_count();
 
 // Caller-provided workspace of one quantize (+ GEMM) pass over an [M x *] activation with a rank-r_t
 // projection.  [hs_off, +M*r_t*2): the pre-scaled bf16 intermediate Hs.  The "zero region" (256 bytes)
-// is cleared by one memset per call: the tensor-amax word and two grid-barrier counters.  Behind it:
+// is cleared by one memset per call: the tensor-amax word, two grid-barrier counters and the word for
+// an amax found outside the quantize kernel.  Behind it:
 // one 128 x r_t fp32 slot per (CTA, row tile) segment of the quantize kernel -- at most
 // WS_MAX_QUANT_CTAS + row tiles of them -- holding partial H tiles.
 constexpr int WS_MAX_QUANT_CTAS = 320;   // 2 CTAs per SM, <= 160 SMs
 struct WsLayout {
-  size_t hs_off, zero_off, zero_bytes, amax_off, bar_off, slots_off, total;
+  size_t hs_off, zero_off, zero_bytes, amax_off, bar_off, amax_ext_off, slots_off, total;
 };
 inline WsLayout ws_layout(int64_t M, int r_t) {
   auto up = [](size_t v) { return (v + 255) / 256 * 256; };
@@ -53,6 +54,7 @@ inline WsLayout ws_layout(int64_t M, int r_t) {
   w.zero_off = w.hs_off + up((size_t)M * (size_t)r_t * 2);
   w.amax_off = w.zero_off;
   w.bar_off = w.zero_off + 4;
+  w.amax_ext_off = w.zero_off + 16;   // amax found by another kernel (the dB^T pass of ft_linear_bwd)
   w.zero_bytes = 256;
   w.slots_off = w.zero_off + w.zero_bytes;
   w.total = w.slots_off + (WS_MAX_QUANT_CTAS + tiles) * 128 * (size_t)r_t * 4 + 256;

@@ -619,7 +619,7 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
 // grid-barrier counters; it is cleared here with one 256-byte memset node.  The partial-H slots behind
 // it need no clearing.
 int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t, const ft_proj* proj,
-                          ft_qtensor* out, void* workspace, cudaStream_t st) {
+                          ft_qtensor* out, void* workspace, bool zero_region_cleared, cudaStream_t st) {
   const int r_t = proj ? proj->r_t : 0;
   CUtensorMap mx, md;
   int rc = make_tensor_map_2d(&mx, x, 2, (uint64_t)cols, (uint64_t)rows, (uint64_t)cols * 2, QF_KC, QF_ROWS,
@@ -654,7 +654,8 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
 #endif
   p.chunks_per_tile = (int)(cols / QF_KC);
   p.total_chunks = ceil_div(rows, QF_ROWS) * (cols / QF_KC);
-  if (amax_t == nullptr || r_t > 0) FT_CUDA_TRY(cudaMemsetAsync(ws + w.zero_off, 0, w.zero_bytes, st));
+  if (!zero_region_cleared && (amax_t == nullptr || r_t > 0))
+    FT_CUDA_TRY(cudaMemsetAsync(ws + w.zero_off, 0, w.zero_bytes, st));
   // padding rows of the last 128-row scale tile must read as zero
   if (out->sf_layout == FT_SF_TILE128x4 && rows % 128 != 0) {
     const int64_t tiles_c = ceil_div(cols / 16, 4);

@@ -26,6 +26,8 @@ struct WgParams {      // two problems in one launch: [0] dA = X^T P_lora, [1] d
   int direct[2];       // 1: a single M slice owns the output, plain stores (no zero-fill needed)
   float* out[2];
   unsigned int* amax_bits[2];   // non-null: atomicMax target for max |In| (bf16 bits << 16), pre-zeroed
+  float4* zero_fill;            // non-null: buffer this launch clears for a LATER launch (zero_fill_n4 float4s)
+  int64_t zero_fill_n4;
 };
 
 __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
@@ -39,6 +41,11 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
         const __grid_constant__ CUtensorMap map_in1, const __grid_constant__ CUtensorMap map_l1,
         const WgParams p) {
   const int z = blockIdx.z;
+  if (p.zero_fill != nullptr) {   // grid-stride clear, every CTA of the launch (before any early return)
+    const int64_t nthr = (int64_t)gridDim.x * gridDim.y * gridDim.z * WG_THREADS;
+    const int64_t me = ((int64_t)(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * WG_THREADS + threadIdx.x;
+    for (int64_t i = me; i < p.zero_fill_n4; i += nthr) p.zero_fill[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
   const CUtensorMap& map_in = z == 0 ? map_in0 : map_in1;
   const CUtensorMap& map_l = z == 0 ? map_l0 : map_l1;
   const int64_t F = p.F[z];
@@ -188,7 +195,7 @@ static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, cuda
 // amax_g (which & 2 only): pre-zeroed word that receives the bit pattern of max |G|.
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, cudaStream_t st) {
+                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, cudaStream_t st) {
   CUtensorMap maps[4];
   const void* in_all[2] = {x, g};
   const void* lr_all[2] = {p_saved, h_saved};
@@ -198,6 +205,8 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
   p.M = M;
   p.r_s = r_s;
   p.r = r;
+  p.zero_fill = reinterpret_cast<float4*>(zero_fill);
+  p.zero_fill_n4 = zero_fill_n / 4;   // K * r, r % 16 == 0
   const int64_t chunks = ceil_div(M, WG_MC);
   // the enabled problems, compacted into z = 0 .. nz-1
   int sel[2], nz = 0;
