@@ -1,5 +1,6 @@
 // api.cu -- the extern "C" boundary of include/fourtune.h: host-side validation,
 // tensor-map construction and kernel sequencing.  No computation happens here.
+#include <cstdlib>
 #include <cstring>
 
 #include "common.cuh"
@@ -38,6 +39,15 @@ int sm_count() {
       return 148;
   }
   return g_sm_count;
+}
+
+bool pdl_enabled() {
+  static int on = -1;
+  if (on < 0) {
+    const char* e = getenv("FT_PDL");
+    on = (e != nullptr && e[0] == '0') ? 0 : 1;
+  }
+  return on == 1;
 }
 
 int device_check() {

@@ -35,6 +35,7 @@ int make_tensor_map_2d(CUtensorMap* map, const void* base, int elem_bytes, uint6
                        uint32_t box_outer, Swizzle sw);
 int device_check();  // FT_OK if the current device is sm_100-class
 int sm_count();
+bool pdl_enabled();  // programmatic dependent launch of the GEMM and dA kernels (FT_PDL=0 turns it off)
 
 // Caller-provided workspace of one quantize (+ GEMM) pass over an [M x *] activation with a rank-r_t
 // projection.  [hs_off, +M*r_t*2): the pre-scaled bf16 intermediate Hs.  The "zero region" (256 bytes)
@@ -248,6 +249,13 @@ __host__ __device__ constexpr uint32_t idesc_bf16(int M, int N) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) |
          ((uint32_t)(M >> 4) << 24);
 }
+
+// ---- programmatic dependent launch: a kernel launched with the programmatic-stream-serialization
+// attribute may start (prologue: barriers, TMEM, tensor-map prefetch) while its predecessor drains;
+// pdl_wait() blocks until the predecessor grid has completed and its writes are visible.  Without the
+// attribute both are no-ops.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // ---- misc
 __device__ __forceinline__ float bf16_bits_to_f32(uint32_t hi16) {

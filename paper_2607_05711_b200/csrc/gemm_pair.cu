@@ -82,6 +82,8 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
   cluster_sync();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
+  pdl_wait();      // the operands (codes, scales, Hs, tensor scales) come from the preceding quantize kernel
+  pdl_trigger();   // the next kernel may set itself up while this one runs
 
   if (warp == 0) {
     // ===================================================== TMA producer (both CTAs)
@@ -268,8 +270,17 @@ int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64
   const int64_t n_tiles = ceil_div(M, P_BM) * ceil_div(N, P_BN);
   const int64_t max_pairs = sm_count() / 2;
   const unsigned grid = 2u * (unsigned)(n_tiles < max_pairs ? n_tiles : max_pairs);
-  k_gemm4_pair<<<grid, P_THREADS, P_SMEM, st>>>(ma, mb, msa, msb, mh, mu, mo, p);
-  FT_CUDA_TRY(cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid, 1, 1);
+  cfg.blockDim = dim3(P_THREADS, 1, 1);
+  cfg.dynamicSmemBytes = P_SMEM;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_gemm4_pair, ma, mb, msa, msb, mh, mu, mo, p));
   return FT_OK;
 }
 

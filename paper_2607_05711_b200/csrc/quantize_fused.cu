@@ -143,6 +143,7 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
   __syncthreads();
   tc_fence_after();
   QF_STAMP(1);
+  pdl_trigger();   // the GEMM that follows may set itself up while this kernel runs (it waits for our end)
 
   // chunk `it` of this CTA is global chunk c_begin + it = (row tile t, column chunk kc)
   auto issue_x = [&](int it, int slot) {

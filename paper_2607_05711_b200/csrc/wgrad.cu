@@ -84,6 +84,8 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
+  pdl_wait();      // dA reads P, written by the kernels before it (no-op without a programmatic edge)
+  pdl_trigger();
 
   if (warp == 0) {
     if (elect_one()) {   // ---- TMA producer
@@ -180,12 +182,21 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
 }
 
 template <int R>
-static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, cudaStream_t st) {
+static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, bool pdl, cudaStream_t st) {
   constexpr int NG = (R + 63) / 64;
   const int smem = WG_STAGES * (WG_IN_BYTES + NG * WG_LG_BYTES) + 1024;
   FT_CUDA_TRY(cudaFuncSetAttribute(k_wgrad<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-  k_wgrad<R><<<grid, WG_THREADS, smem, st>>>(maps[0], maps[1], maps[2], maps[3], p);
-  FT_CUDA_TRY(cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = dim3(WG_THREADS, 1, 1);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = (pdl && pdl_enabled()) ? 1 : 0;
+  FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_wgrad<R>, maps[0], maps[1], maps[2], maps[3], p));
   return FT_OK;
 }
 
@@ -242,15 +253,18 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
     if (sl > gy) gy = sl;
   }
   const dim3 grid(gx, gy, (unsigned)nz);
+  // a dA-only launch directly follows the dgrad GEMM in ft_linear_bwd and enqueues no memset of its own
+  // (accumulate): it may start while the GEMM drains
+  const bool pdl = which == 1 && accumulate != 0;
   switch (r) {
-    case 16: return launch_wg<16>(maps, p, grid, st);
-    case 32: return launch_wg<32>(maps, p, grid, st);
-    case 48: return launch_wg<48>(maps, p, grid, st);
-    case 64: return launch_wg<64>(maps, p, grid, st);
-    case 80: return launch_wg<80>(maps, p, grid, st);
-    case 96: return launch_wg<96>(maps, p, grid, st);
-    case 112: return launch_wg<112>(maps, p, grid, st);
-    case 128: return launch_wg<128>(maps, p, grid, st);
+    case 16: return launch_wg<16>(maps, p, grid, pdl, st);
+    case 32: return launch_wg<32>(maps, p, grid, pdl, st);
+    case 48: return launch_wg<48>(maps, p, grid, pdl, st);
+    case 64: return launch_wg<64>(maps, p, grid, pdl, st);
+    case 80: return launch_wg<80>(maps, p, grid, pdl, st);
+    case 96: return launch_wg<96>(maps, p, grid, pdl, st);
+    case 112: return launch_wg<112>(maps, p, grid, pdl, st);
+    case 128: return launch_wg<128>(maps, p, grid, pdl, st);
     default: return FT_ERR_UNSUPPORTED_SHAPE;
   }
 }
