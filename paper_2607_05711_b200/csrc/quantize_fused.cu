@@ -15,20 +15,24 @@
 // also issues the MMAs is ~400 cycles slower per chunk than its peers and sets the pace of the ring).
 // At the end of a row-tile segment the fp32 partial H tile goes TMEM -> plain vector stores into the
 // segment's own 128 x r_t slot of the workspace (slot = CTA index + row tile: unique, and the slots of
-// one row tile are consecutive).  After a grid-wide barrier (all CTAs are co-resident: cooperative
-// launch) every CTA completes an equal share of the rows: it sums the row tile's slots in CTA order
-// and writes bf16 H and Hs = H * (1 / alpha) -- no second kernel, no atomics on the data, a fixed
-// summation order.  Measured and dropped: fp32 reductions into one accumulator (REDG issues at ~1.3
-// cycles per lane and word: 10 k cycles per 128 x 64 tile) and a last-arriver CTA finishing a whole
-// row tile alone (a 9-17 k-cycle tail on 36 of 296 CTAs).
+// one row tile are consecutive).  Once every slot is written, each row's slots are summed in CTA order
+// and leave as bf16 H and Hs = H * (1 / alpha): no atomics on the data, a fixed summation order.
+// Measured and dropped: fp32 reductions into one accumulator (REDG issues at ~1.3 cycles per lane and
+// word: 10 k cycles per 128 x 64 tile) and a last-arriver CTA finishing a whole row tile alone (a
+// 9-17 k-cycle tail on 36 of 296 CTAs).
 //
-// Two modes, one kernel:
-//   streaming (amax known): chunks stream through a 4-deep ring, two CTAs per SM;
-//   single pass (amax not known, tensor <= 12 chunks per SM = 29 MB on 148 SMs): every chunk of
-//     the CTA stays resident in shared memory; phase 1 finds the tensor amax (and runs the
-//     projection MMAs) as the chunks land, a grid-wide barrier publishes it, phase 2 quantizes
-//     from shared memory.  The tensor is read from HBM exactly once and the separate amax kernel
-//     (a0) disappears.  Launched cooperatively (all CTAs co-resident).
+// Two modes, one kernel template:
+//   streaming (amax known): chunks stream through a 4-deep ring, two CTAs per SM (48 registers: 18
+//     warps put 10 on one SM sub-partition, 10 x 32 x 48 fits its 16 K registers); the slot sums are
+//     done by k_finalize_h, launched behind it with a programmatic edge.  A grid barrier inside the
+//     kernel would need a cooperative launch, and the runtime admits one CTA per SM of a kernel that
+//     allocates tensor memory.
+//   single pass (amax not known, tensor <= 12 chunks per SM = 29 MB on 148 SMs): one CTA per SM, every
+//     chunk stays resident in shared memory; phase 1 finds the tensor amax (and runs the projection
+//     MMAs) as the chunks land, a grid-wide barrier publishes it, phase 2 quantizes from shared
+//     memory, a second grid barrier precedes the slot sums (each CTA an equal share of the rows).
+//     The tensor is read from HBM exactly once and the separate amax kernel (a0) disappears.
+//     Launched cooperatively (all CTAs co-resident); the barrier spin traps after 2 s instead of hanging.
 #include <cstdio>
 #include <cstdlib>
 
@@ -64,29 +68,11 @@ struct QFParams {
   int nx, nd;                   // ring depths (single pass: nx = max chunks per CTA)
   int chunks_per_tile;          // C = cols / 64
   int64_t total_chunks;         // TC = row tiles * C
-#ifdef FT_QF_TIMING
-  long long* dbg;               // [grid x 8] clock64 stamps (debug builds only)
-#endif
 };
-#ifdef FT_QF_TIMING
-#define QF_STAMP(k) do { if (p.dbg && threadIdx.x == 0) p.dbg[blockIdx.x * 8 + (k)] = clock64(); } while (0)
-#else
-#define QF_STAMP(k) do { } while (0)
-#endif
 
-__device__ __forceinline__ void red_add_v4_f32(float* addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(__uint_as_float(a)),
-               "f"(__uint_as_float(b)), "f"(__uint_as_float(c)), "f"(__uint_as_float(d))
-               : "memory");
-}
 __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t* p) {
   uint32_t v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ float2 ld_cg_f32x2(const float* p) {
-  float2 v;
-  asm volatile("ld.global.cg.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p) : "memory");
   return v;
 }
 __device__ __forceinline__ uint64_t globaltimer_ns() {
@@ -96,14 +82,18 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
 }
 
 // R_T: width of the projection (0 = quantize only).  NG = 64-column groups of D.
+// Registers: 18 warps land 5/5/4/4 on the four SM sub-partitions (16 K registers each), so two resident
+// CTAs put 10 warps on one of them: 10 x 32 x 48 = 15 360 fits, 56 per thread (what
+// __launch_bounds__(576, 2) would allow) does not, and the streaming kernel would silently run one
+// CTA per SM.
 template <int R_T, bool SINGLE>
-__global__ void __launch_bounds__(QF_THREADS, SINGLE ? 1 : 2)
+__global__ void __launch_bounds__(QF_THREADS) __maxnreg__(SINGLE ? 96 : 48)
 k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constant__ CUtensorMap map_d,
                  const QFParams p) {
   constexpr int NG = (R_T + 63) / 64;
   constexpr uint32_t ACC_COLS = R_T <= 32 ? 32 : (R_T <= 64 ? 64 : 128);
   constexpr int D_BYTES = NG * QF_DG_BYTES;
-  constexpr int NXS = NG == 2 ? 3 : 4;     // streaming mode: ring depth of X and of D
+  constexpr int NXS = NG == 2 ? 3 : 4;     // streaming mode: ring depth (X chunk + D slice per stage)
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   // 1024-byte alignment for the 128-byte swizzle atoms
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -138,11 +128,9 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
     tmem_alloc(&tmem_base_s, 2 * ACC_COLS);
     tmem_relinquish();
   }
-  QF_STAMP(0);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  QF_STAMP(1);
   pdl_trigger();   // the GEMM that follows may set itself up while this kernel runs (it waits for our end)
 
   // chunk `it` of this CTA is global chunk c_begin + it = (row tile t, column chunk kc)
@@ -203,11 +191,22 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
                  : "=r"(v1.x), "=r"(v1.y), "=r"(v1.z), "=r"(v1.w) : "r"(x_u + q_off1));
   };
-  auto quantize_chunk = [&](uint32_t x_u, float g_enc) {
+  const uint32_t enc_u = smem_u32(enc_tab), full_u = smem_u32(full_x), empty_u = smem_u32(empty_x);
+  // release_u: shared address of the slot's empty barrier, or 0 (single-pass mode: nothing to release).
+  // The slot is handed back as soon as the block is in registers (the amax tree consumes all eight
+  // loaded words, so the loads have completed), not after the ~100 instructions of arithmetic and the
+  // stores: the ring looks deeper to the producer.
+  auto quantize_chunk = [&](uint32_t x_u, float g_enc, uint32_t release_u) {
     uint4 v0, v1;
     load_block(x_u, v0, v1);
-    const uint32_t sf8 = block_sf8(amax_block16(v0, v1), g_enc);
-    const float enc = enc_tab[sf8];
+    const float amax_b = amax_block16(v0, v1);
+    if (release_u != 0) {
+      __syncwarp();
+      if (lane == 0) mbar_arrive_u32(release_u);
+    }
+    const uint32_t sf8 = block_sf8(amax_b, g_enc);
+    float enc;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(enc) : "r"(enc_u + sf8 * 4));
     uint2 c;
     c.x = quant_bf16x8_fast(v0, enc);
     c.y = quant_bf16x8_fast(v1, enc);
@@ -318,25 +317,16 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
     auto issue_stage = [&](int it, int slot) {
       const int64_t c = c_begin + it;
       const int t = (int)(c / C), kc = (int)(c % C);
-#ifdef QF_EXP_NO_D
-      mbar_expect_tx(&full_x[slot], QF_X_BYTES);
-#else
       mbar_expect_tx(&full_x[slot], QF_X_BYTES + (R_T > 0 ? D_BYTES : 0));
-#endif
       tma_load_2d(smem + slot * QF_X_BYTES, &map_x, &full_x[slot], kc * QF_KC, t * QF_ROWS);
-#ifndef QF_EXP_NO_D
       if constexpr (R_T > 0) {
 #pragma unroll
         for (int g = 0; g < NG; ++g)
           tma_load_2d(smem + NXS * QF_X_BYTES + slot * D_BYTES + g * QF_DG_BYTES, &map_d, &full_x[slot], g * 64,
                       kc * QF_KC);
       }
-#endif
     };
     const TensorScale ts = tensor_scale(__ldg(p.amax_in));
-    // Hs = bf16(H * (1 / alpha)), alpha = g_dec(this) * g_dec(other): one IEEE divide per CTA
-    float inv_alpha = 1.0f;
-    if (R_T > 0 && p.hs_out != nullptr) inv_alpha = __fdiv_rn(1.0f, __fmul_rn(ts.g_dec, __ldg(p.other_dec_scale)));
     if (blockIdx.x == 0 && tid == 0) *p.g_dec_out = ts.g_dec;
     if (tid < 128) enc_tab[tid] = enc_of_sf8((uint32_t)tid, ts.g_dec);
     __syncthreads();
@@ -390,10 +380,8 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       int sx = 0;            // ring slot of chunk `it`
       uint32_t phx = 0;      // and its barrier parity
       for (int it = 0; it < n; ++it) {
-        mbar_wait(&full_x[sx], phx);
-        quantize_chunk(xs_u + sx * QF_X_BYTES, ts.g_enc);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty_x[sx]);  // this warp is done with the slot
+        mbar_wait_u32(full_u + sx * 8, phx);
+        quantize_chunk(xs_u + sx * QF_X_BYTES, ts.g_enc, empty_u + sx * 8);
         if constexpr (R_T > 0) {
           if ((o_kc == C - 1) || (it == n - 1)) {   // end of a row-tile segment
             drain_segment(o_t, seg);
@@ -406,13 +394,9 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
           phx ^= 1;
         }
       }
-      QF_STAMP(2);
-      if constexpr (R_T > 0) {
-        grid_barrier(p.grid_bar + 1);
-        QF_STAMP(3);
-        finalize_share(inv_alpha);
-      }
-      QF_STAMP(4);
+      // the partial H tiles are in their slots; k_finalize_h (next launch) sums them.  A grid barrier
+      // here would need a cooperative launch, and the runtime admits only ONE CTA per SM of a kernel
+      // that allocates tensor memory (it cannot see that two 128-column allocations fit).
     }
   } else {
     // =========================================================== single-pass mode
@@ -468,7 +452,6 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       m2 = absmax2_bf16(m2, absmax2_bf16(absmax2_bf16(absmax2_bf16(v0.x, v0.y), absmax2_bf16(v0.z, v0.w)),
                                          absmax2_bf16(absmax2_bf16(v1.x, v1.y), absmax2_bf16(v1.z, v1.w))));
     }
-    QF_STAMP(2);
     m2 &= 0x7FFF7FFFu;
     uint32_t best = max(m2 & 0xFFFFu, m2 >> 16);
 #pragma unroll
@@ -486,7 +469,6 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       drain_segment(o_t, 0);
       if (n > n0) drain_segment(o_t + 1, 1);
     }
-    QF_STAMP(3);
     // ---- grid-wide barrier: every CTA has published its amax
     if (tid == 0) {
       const uint64_t t0 = globaltimer_ns();
@@ -502,18 +484,15 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
     if (blockIdx.x == 0 && tid == 0) *p.g_dec_out = ts.g_dec;
     if (tid < 128) enc_tab[tid] = enc_of_sf8((uint32_t)tid, ts.g_dec);
     qsync();
-    QF_STAMP(4);
     // ---- phase 2: quantize from shared memory
     for (int it = 0; it < n; ++it) {
-      quantize_chunk(xs_u + it * QF_X_BYTES, ts.g_enc);
+      quantize_chunk(xs_u + it * QF_X_BYTES, ts.g_enc, 0);
       advance_out();
     }
-    QF_STAMP(5);
     if constexpr (R_T > 0) {
       grid_barrier(p.grid_bar + 1);   // every CTA's slots are written
       finalize_share(inv_alpha);
     }
-    QF_STAMP(6);
     }
   }
 
@@ -527,12 +506,56 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
   }
 }
 
+// Streaming mode's second step: H[row] = sum of the row tile's slots, in CTA order, -> bf16 H and
+// Hs = H * (1 / alpha).  One thread per (row, column quad); neighbouring threads read neighbouring rows
+// of a slot (layout [quad][row][4]).  G = grid size of the quantize launch that filled the slots.
+template <int R_T>
+__global__ void __launch_bounds__(256) k_finalize_h(const QFParams p, int G) {
+  constexpr int QUADS = R_T / 4;
+  constexpr int SLOT_F4 = QF_ROWS * R_T / 4;
+  pdl_wait();      // the slots and g_dec come from the quantize kernel before us
+  pdl_trigger();
+  float inv_alpha = 1.0f;   // Hs = bf16(H * (1 / alpha)), alpha = g_dec(this) * g_dec(other)
+  if (p.hs_out != nullptr) inv_alpha = __fdiv_rn(1.0f, __fmul_rn(__ldcg(p.g_dec_out), __ldg(p.other_dec_scale)));
+  const int C = p.chunks_per_tile;
+  const int64_t TC = p.total_chunks;
+  // thread -> (tile t, quad q, row r) with r fastest
+  const int64_t e = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  const int r = (int)(e % QF_ROWS);
+  const int q = (int)((e / QF_ROWS) % QUADS);
+  const int64_t t = e / (QF_ROWS * QUADS);
+  const int64_t gr = t * QF_ROWS + r;
+  if (gr >= p.rows) return;
+  // the CTAs whose ranges meet row tile t: owner(c) = floor(((c + 1) * G - 1) / TC)
+  const int i_lo = (int)(((t * C + 1) * G - 1) / TC);
+  const int i_hi = (int)((((t + 1) * C) * G - 1) / TC);
+  const float4* src = reinterpret_cast<const float4*>(p.slots) + (i_lo + t) * SLOT_F4 + q * QF_ROWS + r;
+  float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+  constexpr int BATCH = 12;   // loads in flight; a row tile rarely has more contributors than that
+  for (int i = i_lo; i <= i_hi; i += BATCH) {   // added in CTA order whatever the batching
+    float4 v[BATCH];
+#pragma unroll
+    for (int j = 0; j < BATCH; ++j)
+      v[j] = (i + j <= i_hi) ? __ldcg(src + (int64_t)j * SLOT_F4) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int j = 0; j < BATCH; ++j) {
+      acc.x += v[j].x;
+      acc.y += v[j].y;
+      acc.z += v[j].z;
+      acc.w += v[j].w;
+    }
+    src += BATCH * (int64_t)SLOT_F4;
+  }
+  if (p.h_out != nullptr)
+    *reinterpret_cast<uint2*>(p.h_out + gr * R_T + q * 4) = make_uint2(pack_bf16x2(acc.x, acc.y), pack_bf16x2(acc.z, acc.w));
+  if (p.hs_out != nullptr)
+    *reinterpret_cast<uint2*>(p.hs_out + gr * R_T + q * 4) =
+        make_uint2(pack_bf16x2(__fmul_rn(acc.x, inv_alpha), __fmul_rn(acc.y, inv_alpha)),
+                   pack_bf16x2(__fmul_rn(acc.z, inv_alpha), __fmul_rn(acc.w, inv_alpha)));
+}
+
 int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first);
 
-#ifdef FT_QF_TIMING
-static long long* g_qf_dbg = nullptr;
-extern "C" void ft_debug_set_timing_buffer(void* b) { g_qf_dbg = reinterpret_cast<long long*>(b); }
-#endif
 static int g_qf_mode = 0;   // 0 auto, 1 never single pass, 2 (= auto; single pass whenever it fits)
 void set_quantize_mode(int mode) { g_qf_mode = mode; }
 
@@ -594,25 +617,25 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
   p.nx = NG == 2 ? 3 : 4;   // = NXS of the kernel
   p.nd = p.nx;
   const int smem = p.nx * QF_X_BYTES + (R_T == 0 ? 0 : p.nd * D_BYTES) + 1024;
-  static int occ = 0;       // resident CTAs per SM of this instantiation (the grid barrier needs co-residency)
-  if (occ == 0) {
-    FT_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_quantize_fused<R_T, false>, QF_THREADS, smem));
-    if (occ < 1) return FT_ERR_CUDA;
-    if (occ > 2) occ = 2;
-  }
-  int64_t cap = (int64_t)nsm * occ;
+  int64_t cap = (int64_t)nsm * 2;   // two CTAs per SM (48 registers, <= 97 KB, 128 TMEM columns each)
   if (cap > QF_MAX_GRID) cap = QF_MAX_GRID;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3((unsigned)(TC < cap ? TC : cap), 1, 1);
-  cfg.blockDim = dim3(QF_THREADS, 1, 1);
-  cfg.dynamicSmemBytes = smem;
-  cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeCooperative;
-  attr[0].val.cooperative = R_T > 0 ? 1 : 0;   // only the projection ends in a grid barrier
-  cfg.attrs = attr;
-  cfg.numAttrs = 1;
-  FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_quantize_fused<R_T, false>, mx, md, p));
+  const int grid = (int)(TC < cap ? TC : cap);
+  k_quantize_fused<R_T, false><<<grid, QF_THREADS, smem, st>>>(mx, md, p);
+  FT_CUDA_TRY(cudaGetLastError());
+  if constexpr (R_T > 0) {
+    // partial H tiles -> H, Hs; programmatic edge: it sets itself up while the quantize kernel drains
+    const int64_t items = ceil_div(p.rows, QF_ROWS) * QF_ROWS * (R_T / 4);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)ceil_div(items, 256), 1, 1);
+    cfg.blockDim = dim3(256, 1, 1);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl_enabled() ? 1 : 0;
+    FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_finalize_h<(R_T > 0 ? R_T : 16)>, p, grid));
+  }
   return FT_OK;
 }
 
@@ -650,9 +673,6 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
   p.h_out = proj ? reinterpret_cast<__nv_bfloat16*>(proj->out) : nullptr;
   p.hs_out = proj ? reinterpret_cast<__nv_bfloat16*>(proj->out_scaled) : nullptr;
   p.other_dec_scale = proj ? proj->other_dec_scale : nullptr;
-#ifdef FT_QF_TIMING
-  p.dbg = g_qf_dbg;
-#endif
   p.chunks_per_tile = (int)(cols / QF_KC);
   p.total_chunks = ceil_div(rows, QF_ROWS) * (cols / QF_KC);
   if (!zero_region_cleared && (amax_t == nullptr || r_t > 0))

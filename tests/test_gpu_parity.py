@@ -223,8 +223,12 @@ def test_layer_fused_backward(B, seed, M, K, N, r_s, r):
     out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=True)
     check_layer(B, d, R, D_f, U_f, out, r_s, r)
     ref = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
-    assert np.array_equal(out["dx"], ref["dx"]) and np.array_equal(out["p"], ref["p"])
+    # same amax -> identical codes; P (and through Ps, dX) may differ in the last bf16 bit of a few
+    # elements: the two schedules run the quantize kernel with different grids, i.e. a different (each
+    # time fixed) association of the fp32 partial sums of P
     assert np.array_equal(out["qg"].codes.cpu().numpy(), ref["qg"].codes.cpu().numpy())
+    for k in ("p", "dx"):
+        assert (out[k] == ref[k]).mean() >= 0.999 and rel(out[k], ref[k]) < 1e-3
     assert rel(out["dA"], ref["dA"]) < 1e-5 and rel(out["dBt"], ref["dBt"]) < 1e-5
 
 
