@@ -12,6 +12,7 @@ thread_local int g_last_cuda_error = 0;
 // kernels' host launchers (quantize.cu, quantize_fused.cu, gemm.cu, wgrad.cu)
 int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first);
 void set_quantize_mode(int mode);
+bool quantize_single_pass_fits(int64_t rows, int64_t cols, int r_t);
 int launch_quantize_generic(const void* x, int64_t rows, int64_t cols, const float* amax_t,
                             ft_qtensor* out, cudaStream_t st);
 int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t,
@@ -335,6 +336,16 @@ int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   if (!workspace || !aligned16(workspace)) return FT_ERR_INVALID_ARG;
   if (workspace_bytes < ft_workspace_bytes(M, L->N, L->K, L->r_s + L->r)) return FT_ERR_WORKSPACE_TOO_SMALL;
   const int r_t = L->r_s + L->r;
+  // G small enough for the single-pass quantizer (<= ~29 MB: it finds the amax itself and reads G once):
+  // quantize, GEMM, one wgrad launch for both gradients -- G is read twice either way, with two
+  // launches fewer than the schedule below
+  if (quantize_single_pass_fits(M, L->N, r_t)) {
+    rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
+                     workspace, workspace_bytes, nullptr, st);
+    if (rc != FT_OK) return rc;
+    return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
+                        accumulate, nullptr, nullptr, 0, st);
+  }
   // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0).  One memset
   //    clears the workspace's control words (the amax word among them); the kernel also zero-fills dA
   //    for step 3, so the call enqueues two memset nodes (control words, dBt) instead of four.

@@ -556,6 +556,9 @@ __global__ void __launch_bounds__(256) k_finalize_h(const QFParams p, int G) {
 
 int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first);
 
+// true if launch_quantize_fused would take the single-pass route (amax inside the kernel) for this tensor
+bool quantize_single_pass_fits(int64_t rows, int64_t cols, int r_t);
+
 static int g_qf_mode = 0;   // 0 auto, 1 never single pass, 2 (= auto; single pass whenever it fits)
 void set_quantize_mode(int mode) { g_qf_mode = mode; }
 
@@ -637,6 +640,18 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
     FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_finalize_h<(R_T > 0 ? R_T : 16)>, p, grid));
   }
   return FT_OK;
+}
+
+bool quantize_single_pass_fits(int64_t rows, int64_t cols, int r_t) {
+  if (g_qf_mode == 1) return false;
+  const int nsm = sm_count();
+  const int64_t C = cols / QF_KC, TC = ceil_div(rows, QF_ROWS) * C;
+  const int64_t G = TC < nsm ? TC : (nsm < QF_MAX_GRID ? nsm : QF_MAX_GRID);
+  const int64_t n_max = ceil_div(TC, G);
+  const int NG = (r_t + 63) / 64;
+  const int nd = r_t == 0 ? 0 : (NG == 2 ? 2 : 3);
+  const int64_t smem = n_max * QF_X_BYTES + (int64_t)nd * NG * QF_DG_BYTES + 1024;
+  return n_max <= QF_MAX_NX && smem <= 227 * 1024 - 2048 && (r_t == 0 || n_max <= C);
 }
 
 // Workspace use (offsets from ws_layout, common.cuh): the zero region holds the amax word and the two

@@ -217,8 +217,10 @@ def test_layer_small(B, seed, M, K, N, r_s, r, bn):
 
 @pytest.mark.parametrize("seed,M,K,N,r_s,r", [(21, 130, 320, 192, 16, 16), (22, 300, 1024, 768, 32, 32),
                                                (23, 1000, 512, 2048, 0, 16), (24, 64, 2048, 640, 32, 64)])
-def test_layer_fused_backward(B, seed, M, K, N, r_s, r):
-    """ft_linear_bwd = ft_linear_bwd_dgrad + ft_lora_wgrad with the amax of G found by the dB pass."""
+def test_layer_fused_backward(B, qmode, seed, M, K, N, r_s, r):
+    """ft_linear_bwd = ft_linear_bwd_dgrad + ft_lora_wgrad.  Both of its schedules: G small enough for
+    the single-pass quantizer (qmode 0 at these sizes) and the dB^T pass that also finds the amax of G
+    (forced by qmode 1, which switches the single-pass route off)."""
     d, R, D_f, U_f, L = make_layer(B, seed, M, K, N, r_s, r)
     out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=True)
     check_layer(B, d, R, D_f, U_f, out, r_s, r)
@@ -311,7 +313,9 @@ def test_layer_full_size_sampled(B, name):
     D_f = np.concatenate([L1, d["A"]], 1).astype(np.float32)
     U_f = np.concatenate([L2, d["B"]], 0).astype(np.float32)
     L = B.Layer(t16(R), t16(D_f), t16(U_f.T), r_s, r)
-    out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
+    # the schedule bench.py times: ft_linear_fwd + ft_linear_bwd (C2, C3u: G is too large for the
+    # single-pass quantizer -> dB^T pass with the amax of G first; C3d: G fits -> quantize, GEMM, one wgrad)
+    out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=True)
     rows = np.array(sorted({0, 1, 127, 128, 129, 1000, 2047, 2048, 3333, M - 129, M - 2, M - 1}))
     check_layer(B, d, R, D_f, U_f, out, r_s, r, rows=rows)
     # wgrad on sampled output rows: dA[k, :] = X[:, k]^T P_lora, dB[:, n] = H_lora^T G[:, n]
