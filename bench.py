@@ -468,6 +468,7 @@ def sweep(B, prepare, dev, timed, peaks, full=False):
         base = a.elapsed_time(b) / 5 * 1e3
         return ours, base
 
+    out["fusion_ablation_C2"] = fusion_ablation(B, dev, acts, g)
     cfgs = {"C1": (256, 3072, 3072, 32, 16), "C3u": (4608, 3072, 12288, 32, 64), "C3d": (4608, 12288, 3072, 32, 64)}
     out["configs"] = {}
     for name, (M, K, N, r_s, r) in cfgs.items():
@@ -493,6 +494,72 @@ def sweep(B, prepare, dev, timed, peaks, full=False):
                                    "bf16_lora_ms": round(tot_base / 1e3, 2),
                                    "speedup_vs_bf16_lora": round(tot_base / tot_ours, 2)}
     return out
+
+
+def fusion_ablation(B, dev, acts, g):
+    """The shape of the paper's kernel-fusion experiment (Fig. 9) on this GPU, C2 shapes:
+    the same 4-bit GEMM kernels with NOTHING fused around them -- separate amax and quantize launches, the
+    down- and up-projections as cuBLAS bf16 GEMMs, the branch sum as an elementwise add, the two LoRA
+    gradients as one launch -- against the fused path bench.py times.  Timing only (the unfused arm does
+    not pre-scale H, so its numbers are not the library's)."""
+    import torch
+    M, K, N, r_s, r = 4608, 3072, 9216, 32, 32
+    r_t = r_s + r
+    X, G = acts(M, K), acts(M, N, grad=True)
+    W = (torch.randn(N, K, device=dev, generator=g) * 0.02).to(torch.bfloat16)
+    D_f = (torch.randn(K, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
+    U_t = (torch.randn(N, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
+    layer = B.Layer(W, D_f, U_t, r_s, r)
+    y = torch.empty(M, N, dtype=torch.bfloat16, device=dev)
+    dx = torch.empty(M, K, dtype=torch.bfloat16, device=dev)
+    h = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
+    p = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
+    ws = torch.empty(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_t), dtype=torch.uint8, device=dev)
+    qx, qg = B.QTensor(M, K, device=dev), B.QTensor(M, N, device=dev)
+    dA = torch.empty(K, r, dtype=torch.float32, device=dev)
+    dBt = torch.empty(N, r, dtype=torch.float32, device=dev)
+    ax, ag = torch.empty(1, device=dev), torch.empty(1, device=dev)
+    U_f, D_t = U_t.t().contiguous(), D_f.t().contiguous()
+
+    def unfused():
+        B.ft_tensor_amax(X, ax)
+        B.ft_quantize_blockwise(X, qx, tensor_amax=ax, workspace=ws)
+        hh = X @ D_f
+        B.ft_gemm4(qx, layer.r_kmajor, None, None, y)
+        y.add_(hh @ U_f)
+        B.ft_tensor_amax(G, ag)
+        B.ft_quantize_blockwise(G, qg, tensor_amax=ag, workspace=ws)
+        pp = G @ U_t
+        B.ft_gemm4(qg, layer.r_nmajor, None, None, dx)
+        dx.add_(pp @ D_t)
+        B.ft_lora_wgrad(layer, X, G, hh, pp, dA, dBt)
+
+    def fused():
+        B.ft_linear_fwd(layer, X, y, h, qx, ws)
+        B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws)
+
+    res = {}
+    for name, fn in (("unfused_4bit_us", unfused), ("fused_us", fused)):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        gr = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(gr):
+            fn()
+        for _ in range(3):
+            gr.replay()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(20):
+            gr.replay()
+        b.record()
+        torch.cuda.synchronize()
+        res[name] = round(a.elapsed_time(b) / 20 * 1e3, 1)
+    res["fusion_speedup"] = round(res["unfused_4bit_us"] / res["fused_us"], 2)
+    res["note"] = ("both arms as CUDA graphs; unfused = k_amax, quantize without projection, cuBLAS bf16 down-/up-"
+                   "projections, elementwise adds, the same 4-bit GEMM kernel; paper (other GPUs, whole DiT): LoRA "
+                   "fusion 1.82x (PAPER.md:245)")
+    return res
 
 
 def main():
