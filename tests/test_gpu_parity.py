@@ -287,6 +287,26 @@ def test_wgrad_accumulate(B):
     assert rel(dA.cpu().numpy(), 2 * o["dA"]) <= 1e-5 and rel(dBt.cpu().numpy(), 2 * o["dBt"]) <= 1e-5
 
 
+def test_fused_backward_accumulate_and_errors(B, qmode):
+    """ft_linear_bwd with accumulate=1 adds to dA / dB^T (both schedules); a short workspace is refused
+    before anything is enqueued."""
+    M, K, N, r_s, r = 300, 256, 320, 16, 32
+    d, R, D_f, U_f, L = make_layer(B, 43, M, K, N, r_s, r)
+    o = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
+    dA = torch.from_numpy(o["dA"]).cuda().clone(); dBt = torch.from_numpy(o["dBt"]).cuda().clone()
+    dx = torch.zeros(M, K, dtype=torch.bfloat16, device="cuda")
+    p = torch.zeros(M, r_s + r, dtype=torch.bfloat16, device="cuda")
+    ws = torch.zeros(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_s + r), dtype=torch.uint8, device="cuda")
+    B.ft_linear_bwd(L, o["xt"], o["gt"], o["ht"], dx, p, dA, dBt, o["qg"], ws, accumulate=True)
+    assert rel(dA.cpu().numpy(), 2 * o["dA"]) <= 1e-5 and rel(dBt.cpu().numpy(), 2 * o["dBt"]) <= 1e-5
+    assert (npf(dx) == o["dx"]).mean() >= 0.999
+    before = dA.clone()
+    with pytest.raises(B.FtError, match="workspace too small"):
+        B.ft_linear_bwd(L, o["xt"], o["gt"], o["ht"], dx, p, dA, dBt, o["qg"], ws[:1024])
+    torch.cuda.synchronize()
+    assert torch.equal(before, dA)
+
+
 def test_layer_c1_full(B):
     """BASELINE.json configs[0] in full: M=256, K=N=3072, r_s=32, r=16, seed 0."""
     seed, M, K, N, r_s, r, kind = synth.CONFIGS["C1"]
