@@ -243,20 +243,54 @@ def run_ours(args):
     dAh = torch.empty(K, r, dtype=torch.float32).pin_memory()
     dBh = torch.empty(N, r, dtype=torch.float32).pin_memory()
 
-    def e2e_step():
-        X.copy_(Xh, non_blocking=True)
-        G.copy_(Gh, non_blocking=True)
-        step()
-        yh.copy_(y, non_blocking=True)
-        dxh.copy_(dx, non_blocking=True)
-        dAh.copy_(dA, non_blocking=True)
-        dBh.copy_(dBt, non_blocking=True)
-    e2e_step()
+    # Every step copies its inputs from pinned host memory and its results back; the three legs run on
+    # three streams with double-buffered device tensors, so the H2D of step i+1 and the D2H of step i-1
+    # overlap the kernels of step i (PCIe is full duplex).  The timed region still contains every copy.
+    s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+    Xd, Gd = [X, torch.empty_like(X)], [G, torch.empty_like(G)]
+    yd, dxd = [y, torch.empty_like(y)], [dx, torch.empty_like(dx)]
+    dAd, dBd = [dA, torch.empty_like(dA)], [dBt, torch.empty_like(dBt)]
+    ev_in = [torch.cuda.Event() for _ in range(2)]      # inputs of buffer b are on the device
+    ev_comp = [torch.cuda.Event() for _ in range(2)]    # kernels of buffer b are done
+    ev_out = [torch.cuda.Event() for _ in range(2)]     # results of buffer b are on the host
+    for b in range(2):
+        ev_comp[b].record(stream)
+        ev_out[b].record(stream)
+
+    def e2e_step(i):
+        b = i & 1
+        with torch.cuda.stream(s_in):
+            s_in.wait_event(ev_comp[b])                 # the kernels that last read this buffer are done
+            Xd[b].copy_(Xh, non_blocking=True)
+            Gd[b].copy_(Gh, non_blocking=True)
+            ev_in[b].record(s_in)
+        stream.wait_event(ev_in[b])
+        stream.wait_event(ev_out[b])                    # the previous results in this buffer have left
+        B.ft_linear_fwd(layer, Xd[b], yd[b], h, qx, ws)
+        B.ft_linear_bwd(layer, Xd[b], Gd[b], h, dxd[b], p, dAd[b], dBd[b], qg, ws)
+        if world > 1:
+            parallel.allreduce_lora_grads(dAd[b], dBd[b])
+        ev_comp[b].record(stream)
+        with torch.cuda.stream(s_out):
+            s_out.wait_event(ev_comp[b])
+            yh.copy_(yd[b], non_blocking=True)
+            dxh.copy_(dxd[b], non_blocking=True)
+            dAh.copy_(dAd[b], non_blocking=True)
+            dBh.copy_(dBd[b], non_blocking=True)
+            ev_out[b].record(s_out)
+
+    def e2e_drain():
+        stream.wait_stream(s_in)
+        stream.wait_stream(s_out)
+    e2e_step(0)
+    e2e_step(1)
+    e2e_drain()
     barrier()
-    n_e2e = max(3, min(args.steps, 20))
+    n_e2e = max(4, min(args.steps, 20))
     e0.record()
-    for _ in range(n_e2e):
-        e2e_step()
+    for i in range(n_e2e):
+        e2e_step(i)
+    e2e_drain()                                         # the last results are on the host inside the timed region
     e1.record()
     barrier()
     te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
@@ -339,7 +373,10 @@ def run_ours(args):
                        "peaks": peaks["source"]},
             "clocks": clocks,
             "e2e": {"value": world * flops_step / (e2e_ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms,
-                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                    "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "how": "ft_linear_fwd + ft_linear_bwd per step with X, G copied from pinned host memory and Y, dX, dA, "
+                           "dB^T copied back every step; copies on two side streams with double-buffered device tensors "
+                           "(H2D of step i+1 and D2H of step i-1 overlap the kernels of step i); PCIe-bound"},
             "gpu_launches": KERNELS_PER_STEP * args.steps,
             "roofline": {"kernel": "k_gemm4 (mean of fwd and dgrad launches)", "bound": "tensor",
                          "achieved": gemm_tflops, "peak": fp4_peak, "unit": "TFLOP/s", "frac": gemm_tflops / fp4_peak,
