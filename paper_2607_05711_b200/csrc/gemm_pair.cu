@@ -12,8 +12,12 @@
 //   warp 2   : TMEM allocator (cta_group::2, both CTAs)
 //   warps 4-11: epilogue of this CTA's 128 rows, two groups of four warps (one per 128-column half):
 //              tcgen05.ld, * alpha, bf16, swizzled smem, TMA store
-// TMEM: one 256-column fp32 accumulator + 48 columns of scale factors.  The accumulator is
-// single-buffered; while the epilogue drains it the producer keeps refilling the 4-stage ring.
+// TMEM: TWO 256-column fp32 accumulators (all 512 columns), used alternately, so the epilogue of tile i
+// overlaps the MMAs of tile i+1.  The block scales need 16 more columns (one K=64 step: 4 for A, 8 for
+// B): they live in the first 16 columns of the accumulator that is NOT being accumulated into -- the one
+// the epilogue is draining -- which the epilogue reads first and hands over at once (sf_free).  The
+// scale copies are issued per K=64 step, three tcgen05.cp in front of each MMA (same rate as copying a
+// whole stage up front: probe_fp4_peak.cu mode 2).
 #include "common.cuh"
 
 namespace ft {
@@ -29,7 +33,6 @@ constexpr int P_STAGE_BYTES = P_A_BYTES + P_B_BYTES + P_SFA_BYTES + P_SFB_BYTES;
 constexpr int P_STAGES = 4;
 constexpr int P_OUT_BYTES = 128 * 128;     // one staged output box: 128 rows x 64 bf16
 constexpr int P_SMEM = P_STAGES * P_STAGE_BYTES + 4 * P_OUT_BYTES + 1024;
-constexpr int P_SF_COL = 256;
 
 struct PairParams {
   int64_t M, N, K;
@@ -47,7 +50,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   __shared__ uint64_t full_bar[P_STAGES], empty_bar[P_STAGES];
-  __shared__ uint64_t acc_full, acc_empty;
+  __shared__ uint64_t acc_full[2], acc_empty[2], sf_free[2];
   __shared__ uint32_t tmem_base_s;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -70,8 +73,11 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
       mbar_init(&full_bar[s], 1);   // leader's producer arrives once (with the pair's byte count)
       mbar_init(&empty_bar[s], 1);  // one multicast commit per use
     }
-    mbar_init(&acc_full, 1);
-    mbar_init(&acc_empty, 16);      // 8 epilogue warps x 2 CTAs (used in the leader only)
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(&acc_full[a], 1);
+      mbar_init(&acc_empty[a], 16);   // 8 epilogue warps x 2 CTAs (used in the leader only)
+      mbar_init(&sf_free[a], 8);      // the 4 warps of column half 0 x 2 CTAs: first 16 columns read
+    }
     fence_mbar_init();
   }
   if (warp == 2) {
@@ -127,12 +133,16 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
     if (elect_one()) {
       constexpr uint32_t idesc4 = idesc_nvf4(P_BM, P_BN);
       constexpr uint32_t idesc16 = idesc_bf16(P_BM, P_BN);
-      const uint32_t sfa_t = tmem_base + P_SF_COL;       // 16 columns
-      const uint32_t sfb_t = tmem_base + P_SF_COL + 16;  // 32 columns
       int stage = 0;
-      uint32_t phase = 0, acc_phase = 0;
-      for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs) {
-        mbar_wait(&acc_empty, acc_phase ^ 1);
+      uint32_t phase = 0;
+      int i = 0;   // local tile index: accumulator i & 1, scales in the first 16 columns of the other one
+      for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs, ++i) {
+        const int a = i & 1;
+        const uint32_t acc_t = tmem_base + a * 256;
+        const uint32_t sfa_t = tmem_base + (a ^ 1) * 256;   // 4 columns
+        const uint32_t sfb_t = sfa_t + 8;                   // 8 columns
+        mbar_wait(&acc_empty[a], (((uint32_t)i >> 1) & 1) ^ 1);              // tile i-2 drained
+        if (i > 0) mbar_wait(&sf_free[a ^ 1], (((uint32_t)(i - 1)) >> 1) & 1);  // tile i-1: columns 0-15 read
         tc_fence_after();
         for (int kt = 0; kt < kiters; ++kt) {
           mbar_wait(&full_bar[stage], phase);
@@ -143,28 +153,25 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
             const int nk = (int)min((int64_t)4, sf_tiles_k - (int64_t)kt * 4);
             const uint32_t ssfa = sb + P_B_BYTES, ssfb = ssfa + P_SFA_BYTES;
             for (int k = 0; k < nk; ++k) {
-              tc_cp_sf_pair(sfa_t + 4 * k, make_smem_desc(ssfa + k * 512, 128, 0, 0));
-              tc_cp_sf_pair(sfb_t + 8 * k, make_smem_desc(ssfb + k * 512, 128, 0, 0));
-              tc_cp_sf_pair(sfb_t + 8 * k + 4, make_smem_desc(ssfb + 2048 + k * 512, 128, 0, 0));
+              tc_cp_sf_pair(sfa_t, make_smem_desc(ssfa + k * 512, 128, 0, 0));
+              tc_cp_sf_pair(sfb_t, make_smem_desc(ssfb + k * 512, 128, 0, 0));
+              tc_cp_sf_pair(sfb_t + 4, make_smem_desc(ssfb + 2048 + k * 512, 128, 0, 0));
+              mma_nvf4_pair(acc_t, make_smem_desc(sa + k * 32, 1024, 0, 2), make_smem_desc(sb + k * 32, 1024, 0, 2),
+                            idesc4, sfa_t, sfb_t, (kt | k) != 0);
             }
-            for (int k = 0; k < nk; ++k)
-              mma_nvf4_pair(tmem_base, make_smem_desc(sa + k * 32, 1024, 0, 2),
-                            make_smem_desc(sb + k * 32, 1024, 0, 2), idesc4, sfa_t + 4 * k, sfb_t + 8 * k,
-                            (kt | k) != 0);
           } else {
             const int cols = min(64, p.r_t - (kt - k4) * 64);
             for (int k = 0; k < cols / 16; ++k)
-              mma_bf16_pair(tmem_base, make_smem_desc(sa + k * 32, 1024, 0, 2),
+              mma_bf16_pair(acc_t, make_smem_desc(sa + k * 32, 1024, 0, 2),
                             make_smem_desc(sb + k * 32, 1024, 0, 2), idesc16, 1u);
           }
           tc_commit_pair(&empty_bar[stage], 3);            // frees the slot in both CTAs
-          if (kt == kiters - 1) tc_commit_pair(&acc_full, 3);
+          if (kt == kiters - 1) tc_commit_pair(&acc_full[a], 3);
           if (++stage == P_STAGES) {
             stage = 0;
             phase ^= 1;
           }
         }
-        acc_phase ^= 1;
       }
     }
   } else if (warp >= 4) {
@@ -177,26 +184,37 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
     const int half = (warp - 4) >> 2;
     const int et = (threadIdx.x - 128) & 127;  // 0..127 = row of this CTA's half tile
     const float alpha = __fmul_rn(__ldg(p.g_dec_a), __ldg(p.g_dec_b));
-    const uint32_t leader_acc_empty = map_to_cta(smem_u32(&acc_empty), 0);
     uint8_t* stage_out = smem + P_STAGES * P_STAGE_BYTES + half * 2 * P_OUT_BYTES;
-    uint32_t acc_phase = 0;
-    for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs) {
+    int i = 0;   // local tile index, as in the MMA issuer
+    for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs, ++i) {
+      const int a = i & 1;
       const int64_t mt = tile % tiles_m, nt = tile / tiles_m;
       const int32_t row0 = (int32_t)(mt * P_BM + rank * 128);
       const int32_t n0 = (int32_t)(nt * P_BN) + half * 128;
-      mbar_wait(&acc_full, acc_phase);
+      mbar_wait(&acc_full[a], ((uint32_t)i >> 1) & 1);
       tc_fence_after();
-      const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + half * 128;
+      const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + a * 256 + half * 128;
 #pragma unroll 1
       for (int c = 0; c < 2; ++c) {
         uint32_t v[64];
-        tmem_ld32(t0 + c * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
+        if (c == 0 && half == 0) {
+          // columns 0-15 of this accumulator are the next tile's scale-factor buffer: read them first and
+          // hand them over, so the next tile's MMAs (other accumulator) start while the rest drains
+          tmem_ld16(t0, *reinterpret_cast<uint32_t(*)[16]>(&v[0]));
+          tmem_ld_wait();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(map_to_cta(smem_u32(&sf_free[a]), 0));
+          tmem_ld16(t0 + 16, *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
+        } else {
+          tmem_ld32(t0 + c * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
+        }
         tmem_ld32(t0 + c * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
         tmem_ld_wait();
         if (c == 1) {   // this warp's part of the accumulator is in registers: hand it back
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive_cluster(leader_acc_empty);
+          if (lane == 0) mbar_arrive_cluster(map_to_cta(smem_u32(&acc_empty[a]), 0));
         }
         uint8_t* buf = stage_out + c * P_OUT_BYTES;
         if (et == 0) tma_store_wait_read<1>();   // the store that last used this box has read it
@@ -220,7 +238,6 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
           tma_store_commit();
         }
       }
-      acc_phase ^= 1;
     }
     if (et == 0) tma_store_wait<0>();
   }
