@@ -1,10 +1,11 @@
 // gemm_pair.cu -- a2 / a4 on CTA pairs: the same computation as gemm.cu,
 //     out = bf16( alpha * ( GEMM4(a, b) + Hs * U^T ) ),
 // with tcgen05.mma.cta_group::2: the two CTAs of a cluster (2,1,1) own one 256 x 256 output
-// tile.  Each CTA stages its own 128 rows of A and its own 128-row half of B, so a CTA pulls
-// 256 operand rows from L2 per 128 x 256 of output (the 1-CTA kernel pulls 256 rows per
-// 128 x 128) -- the kernel is bound by L2 -> SM bandwidth, not by the tensor pipe (DESIGN.md
-// section 6), and this halves the bytes per MAC.
+// tile.  Each CTA stages its own 128 rows of A and its own 128-row half of B, so a CTA moves
+// 256 operand rows through its shared memory per 128 x 256 of output (the 1-CTA kernel moves 256
+// rows per 128 x 128): the main loop is bound by shared-memory traffic, not by the tensor pipe
+// (DESIGN.md section 6), and the pair halves the bytes per MAC.  Ring: 5 stages of 38 KB; the
+// epilogue stages through one 16 KB box per column half.
 //
 //   warp 0   : TMA producer (both CTAs; completion bytes land on the LEADER's full barrier)
 //   warp 1   : tcgen05 issuer (leader CTA only): tcgen05.cp of the scale tiles, MMAs, commits
@@ -30,9 +31,9 @@ constexpr int P_B_BYTES = 128 * 128;
 constexpr int P_SFA_BYTES = 4 * 512;   // this CTA's 128 rows, four K=64 steps
 constexpr int P_SFB_BYTES = 2 * 4 * 512;  // all 256 columns of the tile
 constexpr int P_STAGE_BYTES = P_A_BYTES + P_B_BYTES + P_SFA_BYTES + P_SFB_BYTES;  // 38 KB
-constexpr int P_STAGES = 4;
+constexpr int P_STAGES = 5;
 constexpr int P_OUT_BYTES = 128 * 128;     // one staged output box: 128 rows x 64 bf16
-constexpr int P_SMEM = P_STAGES * P_STAGE_BYTES + 4 * P_OUT_BYTES + 1024;
+constexpr int P_SMEM = P_STAGES * P_STAGE_BYTES + 2 * P_OUT_BYTES + 1024;
 
 struct PairParams {
   int64_t M, N, K;
@@ -184,7 +185,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
     const int half = (warp - 4) >> 2;
     const int et = (threadIdx.x - 128) & 127;  // 0..127 = row of this CTA's half tile
     const float alpha = __fmul_rn(__ldg(p.g_dec_a), __ldg(p.g_dec_b));
-    uint8_t* stage_out = smem + P_STAGES * P_STAGE_BYTES + half * 2 * P_OUT_BYTES;
+    uint8_t* stage_out = smem + P_STAGES * P_STAGE_BYTES + half * P_OUT_BYTES;
     int i = 0;   // local tile index, as in the MMA issuer
     for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs, ++i) {
       const int a = i & 1;
@@ -216,8 +217,8 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster(map_to_cta(smem_u32(&acc_empty[a]), 0));
         }
-        uint8_t* buf = stage_out + c * P_OUT_BYTES;
-        if (et == 0) tma_store_wait_read<1>();   // the store that last used this box has read it
+        uint8_t* buf = stage_out;                // one 16 KB staging box per column half: the ring has the
+        if (et == 0) tma_store_wait_read<0>();   // fifth stage instead; the store that last used the box has read it   // the store that last used this box has read it
         if (half == 0) asm volatile("bar.sync 1, 128;" ::: "memory");
         else asm volatile("bar.sync 2, 128;" ::: "memory");
         uint8_t* rowp = buf + et * 128;
