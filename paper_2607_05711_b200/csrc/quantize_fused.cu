@@ -131,7 +131,8 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  pdl_trigger();   // the GEMM that follows may set itself up while this kernel runs (it waits for our end)
+  pdl_wait();      // streaming mode inside ft_linear_bwd: the amax comes from the dB^T kernel before us
+  pdl_trigger();   // the kernel that follows may set itself up while this one runs (it waits for our end)
 
   // chunk `it` of this CTA is global chunk c_begin + it = (row tile t, column chunk kc)
   auto issue_x = [&](int it, int slot) {
@@ -564,7 +565,7 @@ void set_quantize_mode(int mode) { g_qf_mode = mode; }
 
 template <int R_T>
 static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, const void* x, const float* amax_t,
-                     cudaStream_t st) {
+                     bool after_kernel, cudaStream_t st) {
   constexpr int NG = (R_T + 63) / 64;
   constexpr int D_BYTES = NG * QF_DG_BYTES;
   constexpr int SMEM_MAX = 227 * 1024 - 2048;   // minus the static shared memory (barriers, table)
@@ -623,8 +624,19 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
   int64_t cap = (int64_t)nsm * 2;   // two CTAs per SM (48 registers, <= 97 KB, 128 TMEM columns each)
   if (cap > QF_MAX_GRID) cap = QF_MAX_GRID;
   const int grid = (int)(TC < cap ? TC : cap);
-  k_quantize_fused<R_T, false><<<grid, QF_THREADS, smem, st>>>(mx, md, p);
-  FT_CUDA_TRY(cudaGetLastError());
+  {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid, 1, 1);
+    cfg.blockDim = dim3(QF_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = (after_kernel && pdl_enabled()) ? 1 : 0;   // directly behind the dB^T kernel: no memset between
+    FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_quantize_fused<R_T, false>, mx, md, p));
+  }
   if constexpr (R_T > 0) {
     // partial H tiles -> H, Hs; programmatic edge: it sets itself up while the quantize kernel drains
     const int64_t items = ceil_div(p.rows, QF_ROWS) * QF_ROWS * (R_T / 4);
@@ -697,16 +709,18 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
     const int64_t tiles_c = ceil_div(cols / 16, 4);
     FT_CUDA_TRY(cudaMemsetAsync(out->sf + (rows / 128) * tiles_c * 512, 0, tiles_c * 512, st));
   }
+  // no memset of ours in front of the kernel: it directly follows the caller's previous launch
+  const bool after_kernel = zero_region_cleared && !(out->sf_layout == FT_SF_TILE128x4 && rows % 128 != 0);
   switch (r_t) {
-    case 0: return launch_qf<0>(mx, md, p, x, amax_t, st);
-    case 16: return launch_qf<16>(mx, md, p, x, amax_t, st);
-    case 32: return launch_qf<32>(mx, md, p, x, amax_t, st);
-    case 48: return launch_qf<48>(mx, md, p, x, amax_t, st);
-    case 64: return launch_qf<64>(mx, md, p, x, amax_t, st);
-    case 80: return launch_qf<80>(mx, md, p, x, amax_t, st);
-    case 96: return launch_qf<96>(mx, md, p, x, amax_t, st);
-    case 112: return launch_qf<112>(mx, md, p, x, amax_t, st);
-    case 128: return launch_qf<128>(mx, md, p, x, amax_t, st);
+    case 0: return launch_qf<0>(mx, md, p, x, amax_t, after_kernel, st);
+    case 16: return launch_qf<16>(mx, md, p, x, amax_t, after_kernel, st);
+    case 32: return launch_qf<32>(mx, md, p, x, amax_t, after_kernel, st);
+    case 48: return launch_qf<48>(mx, md, p, x, amax_t, after_kernel, st);
+    case 64: return launch_qf<64>(mx, md, p, x, amax_t, after_kernel, st);
+    case 80: return launch_qf<80>(mx, md, p, x, amax_t, after_kernel, st);
+    case 96: return launch_qf<96>(mx, md, p, x, amax_t, after_kernel, st);
+    case 112: return launch_qf<112>(mx, md, p, x, amax_t, after_kernel, st);
+    case 128: return launch_qf<128>(mx, md, p, x, amax_t, after_kernel, st);
     default: return FT_ERR_UNSUPPORTED_SHAPE;
   }
 }
