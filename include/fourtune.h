@@ -80,7 +80,7 @@ typedef struct {
 typedef struct {
   const void* down;          /* bf16 [cols x r_t]                                        */
   void* out;                 /* bf16 [rows x r_t] = bf16(H); may be NULL                 */
-  void* out_scaled;          /* bf16 [rows x r_t] = bf16(H / alpha), alpha = g_dec(this
+  void* out_scaled;          /* bf16 [rows x r_t] = bf16(H * fl(1 / alpha)), alpha = g_dec(this
                                 tensor) * *other_dec_scale (O-10'); may be NULL */
   const float* other_dec_scale; /* g_dec of the operand this tensor will meet in GEMM4;
                                 required iff out_scaled != NULL                          */
@@ -148,7 +148,7 @@ int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* 
 /* ---- a2 / a4 alone: out[M x N] = bf16( alpha * ( GEMM4(a, b) + lr_a_scaled * lr_b^T ) ),
  * alpha = *a->tensor_dec_scale * *b->tensor_dec_scale.
  * a: Q(X) [M x K] (block_rows 1), b: Q(R) [N x K]; both sf TILE128x4, K % 64 == 0, N % 64 == 0.
- * lr_a_scaled: bf16 [M x r_t] = bf16(H / alpha) as written by ft_quantize_blockwise's
+ * lr_a_scaled: bf16 [M x r_t] = bf16(H * fl(1 / alpha)) as written by ft_quantize_blockwise's
  * out_scaled; lr_b: bf16 [N x r_t]; r_t = 0 (both may be NULL) skips the low-rank term.
  * ft_linear_fwd / ft_linear_bwd_dgrad are ft_tensor_amax + ft_quantize_blockwise + this. */
 int ft_gemm4(const ft_qtensor* a, const ft_qtensor* b, const void* lr_a_scaled, const void* lr_b,

@@ -4,7 +4,7 @@
 //     out[m, n] = bf16( alpha * ( sum_k e_a[m,k] sf_a[m,k/16] e_b[n,k] sf_b[n,k/16]
 //                                 + sum_j Hs[m,j] U[n,j] ) ),   alpha = g_dec_a * g_dec_b
 //
-// a: Q(X) or Q(G) [M x K], b: Q(R) [N x K] (K-major both), Hs = bf16(H / alpha) [M x r_t],
+// a: Q(X) or Q(G) [M x K], b: Q(R) [N x K] (K-major both), Hs = bf16(H * fl(1 / alpha)) [M x r_t],
 // U [N x r_t] (O-10').  One persistent CTA per SM, warp-specialised:
 //   warp 0   : TMA producer (codes by tensor map, scale tiles by 1-D bulk copy)
 //   warp 1   : tcgen05 issuer -- tcgen05.cp (scales -> TMEM), tcgen05.mma
