@@ -158,6 +158,35 @@ def test_fused_projection(B, qmode, rows, cols, r_t, kind):
         assert np.all(np.abs(got - want) <= np.abs(want) * 2.0 ** -7 + 1e-5 * np.abs(want).max())
 
 
+def test_fused_projection_random_shapes(B, qmode):
+    """Seeded sweep over ragged shapes: every way a CTA's chunk range can cut the row tiles (one chunk per
+    row tile, ranges spanning several tiles, more CTAs than chunks, ...) against the oracle."""
+    rng = synth.make_rng(2024)
+    for case in range(36):
+        rows = int(rng.integers(1, 900))
+        cols = 64 * int(rng.integers(1, 40))
+        r_t = 16 * int(rng.integers(0, 9))
+        x = synth.outlier_normal(rng, rows, cols) if case % 2 else synth.student_t_grad(rng, rows, cols)
+        out = B.QTensor(rows, cols, 1, B.FT_SF_TILE128x4 if case % 3 else B.FT_SF_ROWMAJOR)
+        q = nvfp4.quantize_blockwise(x, 1)
+        if r_t == 0:
+            B.ft_quantize_blockwise(t16(x), out)
+            assert_q_equal(out, q, out.sf_layout, B)
+            continue
+        D = synth.normal(rng, (cols, r_t), 0.01)
+        h = torch.zeros(rows, r_t, dtype=torch.bfloat16, device="cuda")
+        hs = torch.zeros_like(h)
+        other = np.float32(1.3e-3)
+        B.ft_quantize_blockwise(t16(x), out, down=t16(D), h_out=h, hs_out=hs,
+                                other_dec_scale=torch.tensor([other], device="cuda"))
+        assert_q_equal(out, q, out.sf_layout, B), (rows, cols, r_t)
+        Hex = x.astype(np.float64) @ D.astype(np.float64)
+        alpha = np.float64(np.float32(q["g_dec"]) * other)
+        for got, want in ((npf(h), nvfp4.bf16_round_from_f64(Hex)), (npf(hs), nvfp4.bf16_round_from_f64(Hex / alpha))):
+            assert rel(got, want) <= 2e-3, (rows, cols, r_t)
+            assert (got == want).mean() >= 0.98, (rows, cols, r_t)
+
+
 # ------------------------------------------------------------------ a2 / a4 / a5: the layer
 def make_layer(B, seed, M, K, N, r_s, r, x_kind="outlier"):
     d = synth.layer_inputs(seed, M, K, N, max(r, 1), x_kind)
