@@ -316,6 +316,30 @@ def test_wgrad_accumulate(B):
     assert rel(dA.cpu().numpy(), 2 * o["dA"]) <= 1e-5 and rel(dBt.cpu().numpy(), 2 * o["dBt"]) <= 1e-5
 
 
+def test_forward_with_1x16_weight_blocks(B):
+    """The other arm of the paper's granularity ablation (Table 5): group-wise 1x16 weight
+    scales.  Forward only -- such scales do not transpose (oracle pin P-4), which is why the layer uses 16x16 --
+    composed from the two exported calls: ft_quantize_blockwise(block_rows=1) on the weight, then ft_gemm4."""
+    M, K, N = 200, 512, 384
+    rng = synth.make_rng(77)
+    X = synth.outlier_normal(rng, M, K)
+    W = synth.normal(rng, (N, K), 0.02)
+    qx, qw = B.QTensor(M, K), B.QTensor(N, K, 1, B.FT_SF_TILE128x4)
+    B.ft_quantize_blockwise(t16(X), qx)
+    B.ft_quantize_blockwise(t16(W), qw)
+    y = torch.zeros(M, N, dtype=torch.bfloat16, device="cuda")
+    B.ft_gemm4(qx, qw, None, None, y)
+    oX, oW = nvfp4.quantize_blockwise(X, 1), nvfp4.quantize_blockwise(W, 1)
+    assert_q_equal(qw, oW, B.FT_SF_TILE128x4, B)
+    want = nvfp4.bf16_round_from_f64(nvfp4.dequantize(oX) @ nvfp4.dequantize(oW).T)
+    got = npf(y)
+    assert rel(got, want) <= TOL and (got == want).mean() >= 0.95
+    # and it is the finer quantizer of the two (Table 5's direction) on these weights
+    e1 = rel(nvfp4.dequantize(oW), W)
+    e16 = rel(nvfp4.dequantize(nvfp4.quantize_blockwise(W, 16)), W)
+    assert e1 < e16
+
+
 def test_fused_backward_accumulate_and_errors(B, qmode):
     """ft_linear_bwd with accumulate=1 adds to dA / dB^T (both schedules); a short workspace is refused
     before anything is enqueued."""
