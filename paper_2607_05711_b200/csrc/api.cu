@@ -26,7 +26,8 @@ int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64
                       const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st);
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, cudaStream_t st);
+                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, cudaStream_t st);
+int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t st);
 
 // ------------------------------------------------------------- device queries
 static int g_sm_count = 0;
@@ -321,7 +322,7 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   int rc = check_wgrad(L, x_bf16, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt);
   if (rc != FT_OK) return rc;
   return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, L->r_s + L->r, L->r_s, L->r, dA,
-                      dBt, accumulate, nullptr, nullptr, 0, (cudaStream_t)stream);
+                      dBt, accumulate, nullptr, nullptr, 0, false, (cudaStream_t)stream);
 }
 
 int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
@@ -344,17 +345,19 @@ int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
                      workspace, workspace_bytes, nullptr, st);
     if (rc != FT_OK) return rc;
     return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                        accumulate, nullptr, nullptr, 0, st);
+                        accumulate, nullptr, nullptr, 0, false, st);
   }
-  // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0).  One memset
-  //    clears the workspace's control words (the amax word among them); the kernel also zero-fills dA
-  //    for step 3, so the call enqueues two memset nodes (control words, dBt) instead of four.
+  // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0).  The
+  //    workspace's control words (the amax word among them) and dB^T are cleared by ONE small kernel with
+  //    programmatic edges on both sides instead of two memset nodes; the dB^T kernel also zero-fills dA
+  //    for step 3.  (accumulate: dB^T keeps its contents, only the control words are cleared.)
   const WsLayout w = ws_layout(M, r_t);
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
-  FT_CUDA_TRY(cudaMemsetAsync(ws + w.zero_off, 0, w.zero_bytes, st));
+  rc = launch_clear2(ws + w.zero_off, w.zero_bytes, dBt, accumulate ? 0 : (size_t)L->N * L->r * sizeof(float), st);
+  if (rc != FT_OK) return rc;
   unsigned int* amax_g = reinterpret_cast<unsigned int*>(ws + w.amax_ext_off);
   rc = launch_wgrad(2, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                    accumulate, amax_g, accumulate ? nullptr : dA, accumulate ? 0 : L->K * (int64_t)L->r, st);
+                    1, amax_g, accumulate ? nullptr : dA, accumulate ? 0 : L->K * (int64_t)L->r, true, st);
   if (rc != FT_OK) return rc;
   // 2. a3 + a4 with that amax: Q(G), P = G U_t, dX
   rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
@@ -362,7 +365,7 @@ int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   if (rc != FT_OK) return rc;
   // 3. dA = X^T (G B^T) needs P; its buffer was cleared by step 1 (accumulate == 1: nothing to clear)
   return launch_wgrad(1, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                      1, nullptr, nullptr, 0, st);
+                      1, nullptr, nullptr, 0, true, st);
 }
 
 }  // extern "C"

@@ -60,6 +60,36 @@ int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st,
   return FT_OK;
 }
 
+// ------------------------------------------------ clears with a programmatic edge
+// Two buffers zeroed by one kernel launched with the programmatic-stream-serialization attribute: in
+// a CUDA graph a memset node is a full dependency on both sides, this is a kernel that sets itself up
+// while its predecessor drains and lets its successor do the same.  Sizes in bytes, multiples of 16.
+__global__ void __launch_bounds__(256) k_clear2(uint4* a, int64_t na, uint4* b, int64_t nb) {
+  pdl_wait();
+  pdl_trigger();
+  const int64_t nthr = (int64_t)gridDim.x * 256, me = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  for (int64_t i = me; i < na; i += nthr) a[i] = make_uint4(0, 0, 0, 0);
+  for (int64_t i = me; i < nb; i += nthr) b[i] = make_uint4(0, 0, 0, 0);
+}
+
+int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t st) {
+  const int64_t na = (int64_t)(a_bytes / 16), nb = (int64_t)(b_bytes / 16);
+  int64_t blocks = ceil_div(na + nb, 256 * 4);
+  if (blocks > 2 * sm_count()) blocks = 2 * sm_count();
+  if (blocks < 1) blocks = 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)blocks, 1, 1);
+  cfg.blockDim = dim3(256, 1, 1);
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl_enabled() ? 1 : 0;
+  FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_clear2, reinterpret_cast<uint4*>(a), na, reinterpret_cast<uint4*>(b), nb));
+  return FT_OK;
+}
+
 // ------------------------------------------- generic quantizer (a6, offline path)
 // One thread per 16-element row segment.  BR = 16: the 16 lanes of a half-warp own
 // the 16 rows of one 16x16 block and share its amax by shuffles.  BR = 1: 1x16 blocks.

@@ -42,6 +42,7 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
         const WgParams p) {
   const int z = blockIdx.z;
   if (p.zero_fill != nullptr) {   // grid-stride clear, every CTA of the launch (before any early return)
+    pdl_wait();                   // launched with a programmatic edge: nothing is written before the predecessor ends
     const int64_t nthr = (int64_t)gridDim.x * gridDim.y * gridDim.z * WG_THREADS;
     const int64_t me = ((int64_t)(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * WG_THREADS + threadIdx.x;
     for (int64_t i = me; i < p.zero_fill_n4; i += nthr) p.zero_fill[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -206,7 +207,7 @@ static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, bool
 // amax_g (which & 2 only): pre-zeroed word that receives the bit pattern of max |G|.
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, cudaStream_t st) {
+                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, cudaStream_t st) {
   CUtensorMap maps[4];
   const void* in_all[2] = {x, g};
   const void* lr_all[2] = {p_saved, h_saved};
@@ -253,9 +254,9 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
     if (sl > gy) gy = sl;
   }
   const dim3 grid(gx, gy, (unsigned)nz);
-  // a dA-only launch directly follows the dgrad GEMM in ft_linear_bwd and enqueues no memset of its own
-  // (accumulate): it may start while the GEMM drains
-  const bool pdl = which == 1 && accumulate != 0;
+  // after_kernel: the launch directly follows a kernel of the same call and enqueues no memset of its own
+  // (accumulate): it may set itself up while that kernel drains
+  const bool pdl = after_kernel && accumulate != 0;
   switch (r) {
     case 16: return launch_wg<16>(maps, p, grid, pdl, st);
     case 32: return launch_wg<32>(maps, p, grid, pdl, st);
