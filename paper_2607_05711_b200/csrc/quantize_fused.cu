@@ -556,6 +556,7 @@ __global__ void __launch_bounds__(256) k_finalize_h(const QFParams p, int G) {
 }
 
 int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first);
+int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t st);
 
 // true if launch_quantize_fused would take the single-pass route (amax inside the kernel) for this tensor
 bool quantize_single_pass_fits(int64_t rows, int64_t cols, int r_t);
@@ -596,12 +597,21 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
       cfg.blockDim = dim3(QF_THREADS, 1, 1);
       cfg.dynamicSmemBytes = smem;
       cfg.stream = st;
-      cudaLaunchAttribute attr[1];
+      cudaLaunchAttribute attr[2];
       attr[0].id = cudaLaunchAttributeCooperative;   // the grid barrier needs every CTA resident
       attr[0].val.cooperative = 1;
+      attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+      attr[1].val.programmaticStreamSerializationAllowed = 1;
       cfg.attrs = attr;
-      cfg.numAttrs = 1;
-      const cudaError_t e = cudaLaunchKernelEx(&cfg, k_quantize_fused<R_T, true>, mx, md, p);
+      static bool coop_pdl_ok = true;   // cooperative + programmatic edge: tried once, dropped if refused
+      cfg.numAttrs = (after_kernel && pdl_enabled() && coop_pdl_ok) ? 2 : 1;
+      cudaError_t e = cudaLaunchKernelEx(&cfg, k_quantize_fused<R_T, true>, mx, md, p);
+      if (e != cudaSuccess && cfg.numAttrs == 2) {
+        (void)cudaGetLastError();
+        coop_pdl_ok = false;
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, k_quantize_fused<R_T, true>, mx, md, p);
+      }
       if (e == cudaSuccess) return FT_OK;
       if (e != cudaErrorCooperativeLaunchTooLarge && e != cudaErrorNotSupported) {
         g_last_cuda_error = (int)e;
@@ -702,15 +712,20 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
   p.other_dec_scale = proj ? proj->other_dec_scale : nullptr;
   p.chunks_per_tile = (int)(cols / QF_KC);
   p.total_chunks = ceil_div(rows, QF_ROWS) * (cols / QF_KC);
-  if (!zero_region_cleared && (amax_t == nullptr || r_t > 0))
-    FT_CUDA_TRY(cudaMemsetAsync(ws + w.zero_off, 0, w.zero_bytes, st));
+  bool after_kernel = zero_region_cleared;   // a kernel of ours directly precedes the quantize launch
+  if (!zero_region_cleared && (amax_t == nullptr || r_t > 0)) {
+    // the control words are cleared by a small kernel with programmatic edges, not a memset node
+    rc = launch_clear2(ws + w.zero_off, w.zero_bytes, nullptr, 0, st);
+    if (rc != FT_OK) return rc;
+    after_kernel = true;
+  }
   // padding rows of the last 128-row scale tile must read as zero
   if (out->sf_layout == FT_SF_TILE128x4 && rows % 128 != 0) {
     const int64_t tiles_c = ceil_div(cols / 16, 4);
     FT_CUDA_TRY(cudaMemsetAsync(out->sf + (rows / 128) * tiles_c * 512, 0, tiles_c * 512, st));
   }
-  // no memset of ours in front of the kernel: it directly follows the caller's previous launch
-  const bool after_kernel = zero_region_cleared && !(out->sf_layout == FT_SF_TILE128x4 && rows % 128 != 0);
+  // a memset of ours in front of the kernel (below) breaks the programmatic chain
+  if (out->sf_layout == FT_SF_TILE128x4 && rows % 128 != 0) after_kernel = false;
   switch (r_t) {
     case 0: return launch_qf<0>(mx, md, p, x, amax_t, after_kernel, st);
     case 16: return launch_qf<16>(mx, md, p, x, amax_t, after_kernel, st);
