@@ -11,6 +11,8 @@
 
 namespace ft {
 
+int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t st);
+
 constexpr int WG_F = 128;
 constexpr int WG_MC = 64;
 constexpr int WG_STAGES = 4;
@@ -232,6 +234,9 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
   if (slices > chunks / 8) slices = chunks / 8;
   if (slices < 1) slices = 1;
   unsigned gx = 0, gy = 0;
+  void* clr[2] = {nullptr, nullptr};
+  size_t clr_bytes[2] = {0, 0};
+  int nclr = 0;
   for (int i = 0; i < 2; ++i) {
     const int z = i < nz ? sel[i] : sel[0];
     int rc = make_tensor_map_2d(&maps[2 * i], in_all[z], 2, (uint64_t)F_all[z], (uint64_t)M, (uint64_t)F_all[z] * 2, 64,
@@ -247,16 +252,23 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
     p.out[i] = out_all[z];
     p.amax_bits[i] = z == 1 ? amax_g : nullptr;
     if (i >= nz) continue;
-    if (!accumulate && !p.direct[i])
-      FT_CUDA_TRY(cudaMemsetAsync(out_all[z], 0, (size_t)F_all[z] * r * sizeof(float), st));
+    if (!accumulate && !p.direct[i]) {   // cleared below by one kernel with programmatic edges
+      clr[nclr] = out_all[z];
+      clr_bytes[nclr++] = (size_t)F_all[z] * r * sizeof(float);
+    }
     const unsigned ft = (unsigned)ceil_div(F_all[z], WG_F);
     if (ft > gx) gx = ft;
     if (sl > gy) gy = sl;
   }
   const dim3 grid(gx, gy, (unsigned)nz);
-  // after_kernel: the launch directly follows a kernel of the same call and enqueues no memset of its own
-  // (accumulate): it may set itself up while that kernel drains
-  const bool pdl = after_kernel && accumulate != 0;
+  if (nclr > 0) {
+    int rc = launch_clear2(clr[0], clr_bytes[0], clr[1], clr_bytes[1], st);
+    if (rc != FT_OK) return rc;
+    after_kernel = true;
+  }
+  // after_kernel: the launch directly follows a kernel of the same call (the clear above, or the caller's
+  // previous launch with accumulate set): it may set itself up while that kernel drains
+  const bool pdl = after_kernel && (accumulate != 0 || nclr > 0 || (p.direct[0] && (nz == 1 || p.direct[1])));
   switch (r) {
     case 16: return launch_wg<16>(maps, p, grid, pdl, st);
     case 32: return launch_wg<32>(maps, p, grid, pdl, st);
