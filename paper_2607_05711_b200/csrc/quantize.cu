@@ -12,6 +12,8 @@ namespace ft {
 __global__ void __launch_bounds__(256) k_amax(const uint4* __restrict__ x, int64_t n_vec,
                                               const uint16_t* __restrict__ tail, int n_tail,
                                               unsigned int* __restrict__ out_bits) {
+  pdl_wait();      // behind the clear kernel of the quantize call (no-op without a programmatic edge)
+  pdl_trigger();
   const uint32_t m = 0x7FFF7FFFu;
   uint32_t acc = 0;  // two 15-bit maxima packed; compared per half with vmax
   // a CTA walks 32 KB tiles (256 threads x 8 x 16 bytes); the 8 loads of a thread are issued
@@ -53,10 +55,18 @@ int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st,
   const int64_t cap = (int64_t)sm_count() * 6;
   if (blocks > cap) blocks = cap;
   if (blocks < 1) blocks = 1;
-  k_amax<<<(unsigned)blocks, 256, 0, st>>>(reinterpret_cast<const uint4*>(x_bf16), n_vec,
-                                           reinterpret_cast<const uint16_t*>(x_bf16) + n_vec * 8,
-                                           n_tail, reinterpret_cast<unsigned int*>(amax_out));
-  FT_CUDA_TRY(cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)blocks, 1, 1);
+  cfg.blockDim = dim3(256, 1, 1);
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = (!zero_first && pdl_enabled()) ? 1 : 0;   // directly behind the caller's clear kernel
+  FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_amax, reinterpret_cast<const uint4*>(x_bf16), n_vec,
+                                 reinterpret_cast<const uint16_t*>(x_bf16) + n_vec * 8, n_tail,
+                                 reinterpret_cast<unsigned int*>(amax_out)));
   return FT_OK;
 }
 
