@@ -126,3 +126,14 @@ def wgrad(X, G, H, P, r_s):
     dB = (H_l.T @ G).astype(np.float32)
     dA = (X.T @ P_l).astype(np.float32)
     return {"dA": dA, "dB": dB}
+
+
+def wgrad_saved4(qX, G, H, P, r_s):
+    """W with 4-bit saved activations (reading O-12' in DESIGN.md): Eq. 4
+     with the X of `dA = X^T (G B^T)` taken as dequant(Q(X)) -- the codes and scales
+    the forward pass produced anyway -- instead of the bf16 X, so that the layer keeps 0.5625
+    instead of 2 bytes per activation element between forward and backward (the activation side
+    of the memory figures at PAPER.md:197-207; the paper does not say which X its Eq. 4 uses).
+        dA[k,j] = sum_m (E2M1(code[m,k]) * sf[m,k/16] * g_dec) * P[m, r_s+j]
+    dB is unchanged (it never touches X).  float64 sums, float32 results."""
+    return wgrad(nvfp4.dequantize(qX), G, H, P, r_s)

@@ -234,3 +234,51 @@ def test_qrt_is_permuted_qr_in_dgrad():
     out = layer.dgrad(G, qR, D_f, U_f, out_bf16=False)
     ref = nvfp4.dequantize(out["qG"]) @ nvfp4.dequantize(qRt).T
     assert np.allclose(out["dX"], ref, rtol=1e-10, atol=1e-14 * np.abs(ref).max())   # summation order only
+
+
+# ------------------------------------------- NEXT-2 / O-12': dA from the saved 4-bit activations
+def test_wgrad_saved4_bruteforce_and_special_cases():
+    X, G, R, D_f, U_f, _ = _tiny_layer(31, 5, 32, 16, 2, 2)
+    M, K = X.shape
+    r_s = 2
+    qR = layer.quantize_weight(R)
+    fw = layer.forward(X, qR, D_f, U_f)
+    P = layer.dgrad(G, qR, D_f, U_f)["P"]
+    qX = fw["qX"]
+    w4 = layer.wgrad_saved4(qX, G, fw["H"], P, r_s)
+    w = layer.wgrad(X, G, fw["H"], P, r_s)
+    # brute force from the codes, the scale bytes and g_dec, decoded by hand (not through dequantize):
+    # E2M1 magnitudes by table, E4M3 by its bit fields
+    mag = [0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0]
+    def e4m3(b):
+        e, m = (int(b) >> 3) & 15, int(b) & 7
+        return (m / 8.0) * 2.0 ** -6 if e == 0 else (1 + m / 8.0) * 2.0 ** (e - 7)
+    g_dec = float(np.float32(qX["g_dec"]))
+    for k in range(K):
+        for j in range(2):
+            s = 0.0
+            for m in range(M):
+                c = int(qX["codes"][m, k])
+                v = (-1.0 if c & 8 else 1.0) * mag[c & 7] * e4m3(qX["sf"][m, k // 16]) * g_dec
+                s += v * float(P[m, r_s + j])
+            assert abs(w4["dA"][k, j] - s) <= 1e-6 * max(1e-6, abs(s))
+    # dB never touches X
+    assert np.array_equal(w4["dB"], w["dB"])
+    # the two readings of Eq. 4 differ by exactly the quantization error of X against P
+    err = (nvfp4.dequantize(qX) - X.astype(np.float64)).T @ P[:, r_s:].astype(np.float64)
+    assert np.allclose(w4["dA"] - w["dA"], err, rtol=0, atol=1e-6 * np.abs(w["dA"]).max() + 1e-12)
+    assert np.any(w4["dA"] != w["dA"])
+    # on data Q(.) represents exactly the two readings coincide: grid values times a power-of-two
+    # block scale, tensor amax 42 = 2688 / 64 so that g_enc = 64 exactly, a +-6 in every block
+    rng = synth.make_rng(5)
+    grid = np.array(mag + [-v for v in mag], np.float32)
+    Xe = grid[rng.integers(0, 16, (M, K))].reshape(M, K // 16, 16)
+    Xe[:, :, 0] = 6.0 * np.where(rng.integers(0, 2, (M, K // 16)) == 1, 1.0, -1.0)
+    sfe = (2.0 ** rng.integers(-3, 4, (M, K // 16))).astype(np.float32)
+    sfe[0, 0] = 448.0
+    Xe = (Xe * sfe[:, :, None] / 64.0).reshape(M, K).astype(np.float32)
+    assert np.abs(Xe).max() == 42.0
+    qXe = nvfp4.quantize_blockwise(Xe, 1)
+    assert np.array_equal(nvfp4.dequantize(qXe), Xe.astype(np.float64))
+    assert np.array_equal(layer.wgrad_saved4(qXe, G, fw["H"], P, r_s)["dA"],
+                          layer.wgrad(Xe, G, fw["H"], P, r_s)["dA"])
