@@ -163,6 +163,19 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
                   const void* h_saved_bf16, const void* p_saved_bf16, float* dA,
                   float* dBt, int32_t accumulate, void* stream);
 
+/* ---- a5 with 4-bit saved activations (O-12'): Eq. 4
+ * with the X of dA = X^T (G B^T) taken as dequant(Q(X)) = E2M1(code) * sf * g_dec -- the qx_scratch
+ * that ft_linear_fwd filled -- so the caller keeps 0.5625 instead of 2 bytes per activation element
+ * between forward and backward (the activation side of PAPER.md:197-207) and may free or reuse x_bf16
+ * as soon as ft_linear_fwd has run.
+ * qx: Q(X) [M x K], block_rows 1, sf FT_SF_TILE128x4, all three pointers device memory.
+ * dBt = G^T * H[:, r_s:] exactly as in ft_lora_wgrad (it never reads X).  Everything else as there.
+ * The dequantized operand is exact in bf16 (E2M1 x E4M3 has six significant bits); g_dec multiplies
+ * the fp32 sums. */
+int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16, int64_t M,
+                     const void* h_saved_bf16, const void* p_saved_bf16, float* dA,
+                     float* dBt, int32_t accumulate, void* stream);
+
 /* ---- a0+a3+a4+a5 in one call: the whole backward of the layer (Eq. 3 and Eq. 4).
  * Same results as ft_linear_bwd_dgrad followed by ft_lora_wgrad, different schedule: the pass
  * over G that computes dBt = G^T (X A) also finds max |G|, so the separate amax pass of the

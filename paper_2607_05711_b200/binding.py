@@ -55,6 +55,7 @@ def lib():
         L.ft_linear_bwd_dgrad.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
         L.ft_gemm4.argtypes = [C.POINTER(_QT), C.POINTER(_QT), vp, vp, i32, vp, vp]
         L.ft_lora_wgrad.argtypes = [C.POINTER(_Layer), vp, vp, i64, vp, vp, vp, vp, i32, vp]
+        L.ft_lora_wgrad_q4.argtypes = [C.POINTER(_Layer), C.POINTER(_QT), vp, i64, vp, vp, vp, vp, i32, vp]
         L.ft_linear_bwd.argtypes = [C.POINTER(_Layer), vp, vp, i64, vp, vp, vp, vp, vp, i32, C.POINTER(_QT), vp, sz, vp]
         L.ft_sf_bytes.argtypes = [i64, i64, i32, i32]
         L.ft_sf_bytes.restype = sz
@@ -201,6 +202,14 @@ def ft_lora_wgrad(layer, x, g, h_saved, p_saved, dA, dBt, accumulate=False, stre
     L = layer.c()
     _check(lib().ft_lora_wgrad(C.byref(L), _ptr(x), _ptr(g), x.shape[0], _ptr(h_saved), _ptr(p_saved),
                                _ptr(dA), _ptr(dBt), 1 if accumulate else 0, _stream(stream)))
+    return dA, dBt
+
+
+def ft_lora_wgrad_q4(layer, qx, g, h_saved, p_saved, dA, dBt, accumulate=False, stream=None):
+    """ft_lora_wgrad with dequant(Q(X)) -- the QTensor ft_linear_fwd filled -- in place of the bf16 X."""
+    L, q = layer.c(), qx.c()
+    _check(lib().ft_lora_wgrad_q4(C.byref(L), C.byref(q), _ptr(g), g.shape[0], _ptr(h_saved), _ptr(p_saved),
+                                  _ptr(dA), _ptr(dBt), 1 if accumulate else 0, _stream(stream)))
     return dA, dBt
 
 

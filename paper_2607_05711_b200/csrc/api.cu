@@ -28,6 +28,8 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
                  unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, cudaStream_t st);
 int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t st);
+int launch_wgrad_q4(const uint8_t* codes, const uint8_t* sf, const float* g_dec, int64_t M, int64_t K,
+                    const void* p_saved, int r_t, int r_s, int r, float* dA, int accumulate, cudaStream_t st);
 
 // ------------------------------------------------------------- device queries
 static int g_sm_count = 0;
@@ -323,6 +325,25 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   if (rc != FT_OK) return rc;
   return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, L->r_s + L->r, L->r_s, L->r, dA,
                       dBt, accumulate, nullptr, nullptr, 0, false, (cudaStream_t)stream);
+}
+
+int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16, int64_t M,
+                     const void* h_saved_bf16, const void* p_saved_bf16, float* dA, float* dBt,
+                     int32_t accumulate, void* stream) {
+  if (!qx || !qx->codes || !qx->sf || !qx->tensor_dec_scale) return FT_ERR_INVALID_ARG;
+  int rc = check_wgrad(L, qx->codes, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt);
+  if (rc != FT_OK) return rc;
+  if (qx->rows != M || qx->cols != L->K || qx->block_rows != 1 || qx->sf_layout != FT_SF_TILE128x4 ||
+      !aligned16(qx->sf))
+    return FT_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int r_t = L->r_s + L->r;
+  // dB^T never reads X: the bf16 kernel, problem 2 only
+  rc = launch_wgrad(2, nullptr, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
+                    accumulate, nullptr, nullptr, 0, false, st);
+  if (rc != FT_OK) return rc;
+  return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA,
+                         accumulate, st);
 }
 
 int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,

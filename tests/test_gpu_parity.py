@@ -316,6 +316,42 @@ def test_wgrad_accumulate(B):
     assert rel(dA.cpu().numpy(), 2 * o["dA"]) <= 1e-5 and rel(dBt.cpu().numpy(), 2 * o["dBt"]) <= 1e-5
 
 
+@pytest.mark.parametrize("seed,M,K,N,r_s,r", [(51, 1, 64, 64, 0, 16), (52, 130, 320, 192, 16, 16),
+                                               (53, 300, 576, 448, 32, 32), (54, 1100, 512, 256, 32, 64),
+                                               (55, 2049, 1024, 128, 0, 128), (56, 64, 2048, 640, 16, 48)])
+def test_wgrad_saved4(B, seed, M, K, N, r_s, r):
+    """NEXT-2 / O-12': ft_lora_wgrad_q4 = Eq. 4 with dequant(Q(X)) as the saved activation, against
+    oracle.layer.wgrad_saved4 on the ORACLE's own Q(X).  Ragged M, K % 128 == 64 (half feature tile),
+    one and several M slices (M >= 1024: fp32 reductions), every r group count; then accumulate."""
+    d, R, D_f, U_f, L = make_layer(B, seed, M, K, N, r_s, r)
+    o = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
+    qX = nvfp4.quantize_blockwise(d["X"], 1)
+    assert_q_equal(o["qx"], qX, B.FT_SF_TILE128x4, B)
+    w = olayer.wgrad_saved4(qX, d["dY"], o["h"], o["p"], r_s)
+    dA = torch.full((K, r), 7.0, dtype=torch.float32, device="cuda")
+    dBt = torch.full((N, r), 7.0, dtype=torch.float32, device="cuda")
+    B.ft_lora_wgrad_q4(L, o["qx"], o["gt"], o["ht"], o["pt"], dA, dBt)
+    torch.cuda.synchronize()
+    assert rel(dA.cpu().numpy(), w["dA"]) <= 1e-5, "dA from 4-bit saved activations"
+    assert rel(dBt.cpu().numpy().T, w["dB"]) <= TOL
+    assert rel(dBt.cpu().numpy(), o["dBt"]) <= 1e-5            # the same kernel as ft_lora_wgrad
+    # the two readings of Eq. 4 differ by the quantization error of X, far above the kernel's own error
+    assert rel(dA.cpu().numpy(), o["dA"]) > 1e-3
+    once = dA.cpu().numpy().copy()
+    B.ft_lora_wgrad_q4(L, o["qx"], o["gt"], o["ht"], o["pt"], dA, dBt, accumulate=True)
+    torch.cuda.synchronize()
+    assert rel(dA.cpu().numpy(), 2 * once) <= 1e-5 and rel(dBt.cpu().numpy(), 2 * o["dBt"]) <= 1e-5
+
+
+def test_wgrad_saved4_errors(B):
+    M, K, N, r_s, r = 128, 256, 128, 16, 16
+    d, R, D_f, U_f, L = make_layer(B, 57, M, K, N, r_s, r)
+    o = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
+    dA = torch.zeros(K, r, dtype=torch.float32, device="cuda"); dBt = torch.zeros(N, r, dtype=torch.float32, device="cuda")
+    with pytest.raises(B.FtError):      # Q(G) has the wrong column count for the X operand
+        B.ft_lora_wgrad_q4(L, o["qg"] if N != K else B.QTensor(M, K + 64), o["gt"], o["ht"], o["pt"], dA, dBt)
+
+
 def test_forward_with_1x16_weight_blocks(B):
     """The other arm of the paper's granularity ablation (Table 5): group-wise 1x16 weight
     scales.  Forward only -- such scales do not transpose (oracle pin P-4), which is why the layer uses 16x16 --
@@ -396,3 +432,10 @@ def test_layer_full_size_sampled(B, name):
     Pl = out["p"][:, r_s:].astype(np.float64); Hl = out["h"][:, r_s:].astype(np.float64)
     assert rel(out["dA"][ks], d["X"][:, ks].astype(np.float64).T @ Pl) <= TOL
     assert rel(out["dBt"][ns], d["dY"][:, ns].astype(np.float64).T @ Hl) <= TOL
+    # the same with 4-bit saved activations (NEXT-2): dA[k, :] = dequant(Q(X))[:, k]^T P_lora
+    dA4 = torch.zeros(K, r, dtype=torch.float32, device="cuda"); dBt4 = torch.zeros(N, r, dtype=torch.float32, device="cuda")
+    B.ft_lora_wgrad_q4(L, out["qx"], out["gt"], out["ht"], out["pt"], dA4, dBt4)
+    torch.cuda.synchronize()
+    Xq = nvfp4.dequantize(nvfp4.quantize_blockwise(d["X"], 1))
+    assert rel(dA4.cpu().numpy()[ks], Xq[:, ks].T @ Pl) <= 1e-5
+    assert rel(dBt4.cpu().numpy()[ns], d["dY"][:, ns].astype(np.float64).T @ Hl) <= TOL
