@@ -336,6 +336,7 @@ def run_ours(args):
         workspace=ws))
     kern["gemm_dgrad_us"] = timed(lambda: B.ft_gemm4(qg, layer.r_nmajor, hs, D_f, dx))
     kern["wgrad_us"] = timed(lambda: B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt))
+    kern["wgrad_saved4_us"] = timed(lambda: B.ft_lora_wgrad_q4(layer, qx, G, h, p, dA, dBt))
     kern["bwd_fused_us"] = timed(lambda: B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws))
     kern["fwd_us"] = timed(lambda: B.ft_linear_fwd(layer, X, y, h, qx, ws))
 
@@ -394,6 +395,12 @@ def run_ours(args):
                                  "each figure is launch overhead"},
             "bf16_lora_baseline": {"us_per_step": bf16_us, "speedup": bf16_us / (ms_per_step * 1e3),
                                    "how": "torch.matmul (cuBLAS) bf16, frozen W, same shapes, same GPU"},
+            "saved4_activations": {
+                "wgrad_bf16_x_us": round(kern["wgrad_us"], 2), "wgrad_saved4_us": round(kern["wgrad_saved4_us"], 2),
+                "saved_bytes_per_layer_bf16": 2 * M * K, "saved_bytes_per_layer_4bit": int(0.5625 * M * K),
+                "note": "NEXT-2: ft_lora_wgrad_q4 takes dA = dequant(Q(X))^T (G B^T) from the codes and scales the "
+                        "forward pass wrote, so the bf16 X need not be kept for backward (3.56x fewer saved bytes); "
+                        "not part of the timed step, which follows Eq. 4 literally (O-12)"},
             **extra,
             "paper_context": "2.27x step time / 2.25x memory vs BF16 LoRA on RTX 5090 (PAPER.md:7,207); not the target",
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle",

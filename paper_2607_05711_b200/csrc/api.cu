@@ -26,10 +26,12 @@ int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64
                       const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st);
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, cudaStream_t st);
+                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, bool beside_prev,
+                 cudaStream_t st);
 int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t st);
 int launch_wgrad_q4(const uint8_t* codes, const uint8_t* sf, const float* g_dec, int64_t M, int64_t K,
-                    const void* p_saved, int r_t, int r_s, int r, float* dA, int accumulate, cudaStream_t st);
+                    const void* p_saved, int r_t, int r_s, int r, float* dA, int accumulate, bool beside_prev,
+                    cudaStream_t st);
 
 // ------------------------------------------------------------- device queries
 static int g_sm_count = 0;
@@ -324,7 +326,7 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   int rc = check_wgrad(L, x_bf16, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt);
   if (rc != FT_OK) return rc;
   return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, L->r_s + L->r, L->r_s, L->r, dA,
-                      dBt, accumulate, nullptr, nullptr, 0, false, (cudaStream_t)stream);
+                      dBt, accumulate, nullptr, nullptr, 0, false, false, (cudaStream_t)stream);
 }
 
 int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16, int64_t M,
@@ -338,12 +340,20 @@ int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
     return FT_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   const int r_t = L->r_s + L->r;
-  // dB^T never reads X: the bf16 kernel, problem 2 only
+  // one clear for both gradients, then dB^T (it never reads X: the bf16 kernel, problem 2 only) and dA
+  // from the codes, both accumulating, both behind programmatic edges; the dA kernel does not wait for the
+  // dB^T kernel (they share nothing) and takes over the SMs as its CTAs retire
+  bool chained = false;
+  if (!accumulate) {
+    rc = launch_clear2(dA, (size_t)L->K * L->r * sizeof(float), dBt, (size_t)L->N * L->r * sizeof(float), st);
+    if (rc != FT_OK) return rc;
+    chained = true;
+  }
   rc = launch_wgrad(2, nullptr, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                    accumulate, nullptr, nullptr, 0, false, st);
+                    1, nullptr, nullptr, 0, chained, false, st);
   if (rc != FT_OK) return rc;
   return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA,
-                         accumulate, st);
+                         1, chained, st);
 }
 
 int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
@@ -366,7 +376,7 @@ int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
                      workspace, workspace_bytes, nullptr, st);
     if (rc != FT_OK) return rc;
     return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                        accumulate, nullptr, nullptr, 0, false, st);
+                        accumulate, nullptr, nullptr, 0, false, false, st);
   }
   // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0).  The
   //    workspace's control words (the amax word among them) and dB^T are cleared by ONE small kernel with
@@ -378,15 +388,18 @@ int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   if (rc != FT_OK) return rc;
   unsigned int* amax_g = reinterpret_cast<unsigned int*>(ws + w.amax_ext_off);
   rc = launch_wgrad(2, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                    1, amax_g, accumulate ? nullptr : dA, accumulate ? 0 : L->K * (int64_t)L->r, true, st);
+                    1, amax_g, accumulate ? nullptr : dA, accumulate ? 0 : L->K * (int64_t)L->r, true, false, st);
   if (rc != FT_OK) return rc;
   // 2. a3 + a4 with that amax: Q(G), P = G U_t, dX
   rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
                    workspace, workspace_bytes, reinterpret_cast<const float*>(amax_g), st);
   if (rc != FT_OK) return rc;
-  // 3. dA = X^T (G B^T) needs P; its buffer was cleared by step 1 (accumulate == 1: nothing to clear)
+  // 3. dA = X^T (G B^T) needs P; its buffer was cleared by step 1 (accumulate == 1: nothing to clear).
+  //    Nothing it touches depends on the GEMM in front of it (X, P in; dA out), and every CTA of the GEMM
+  //    passes its own wait -- P complete -- before triggering: dA starts in the GEMM's tail and waits for
+  //    the GEMM only before it exits.
   return launch_wgrad(1, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                      1, nullptr, nullptr, 0, true, st);
+                      1, nullptr, nullptr, 0, true, true, st);
 }
 
 }  // extern "C"

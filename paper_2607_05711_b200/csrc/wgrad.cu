@@ -28,6 +28,9 @@ struct WgParams {      // two problems in one launch: [0] dA = X^T P_lora, [1] d
   int direct[2];       // 1: a single M slice owns the output, plain stores (no zero-fill needed)
   float* out[2];
   unsigned int* amax_bits[2];   // non-null: atomicMax target for max |In| (bf16 bits << 16), pre-zeroed
+  int late_wait;                // 1: nothing this launch touches depends on its predecessor, which passes
+                                //    griddepcontrol.wait in every CTA before triggering: start beside it and
+                                //    wait for it at the END (completion stays transitive for the next launch)
   float4* zero_fill;            // non-null: buffer this launch clears for a LATER launch (zero_fill_n4 float4s)
   int64_t zero_fill_n4;
 };
@@ -87,7 +90,7 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
-  pdl_wait();      // dA reads P, written by the kernels before it (no-op without a programmatic edge)
+  if (!p.late_wait) pdl_wait();   // dA reads P, written by the kernels before it (no-op without a programmatic edge)
   pdl_trigger();
 
   if (warp == 0) {
@@ -182,6 +185,7 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
     tc_fence_after();
     tmem_dealloc(tmem_base, TMEM_COLS);
   }
+  if (p.late_wait) pdl_wait();
 }
 
 template <int R>
@@ -209,7 +213,8 @@ static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, bool
 // amax_g (which & 2 only): pre-zeroed word that receives the bit pattern of max |G|.
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, cudaStream_t st) {
+                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, bool beside_prev,
+                 cudaStream_t st) {
   CUtensorMap maps[4];
   const void* in_all[2] = {x, g};
   const void* lr_all[2] = {p_saved, h_saved};
@@ -269,6 +274,9 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
   // after_kernel: the launch directly follows a kernel of the same call (the clear above, or the caller's
   // previous launch with accumulate set): it may set itself up while that kernel drains
   const bool pdl = after_kernel && (accumulate != 0 || nclr > 0 || (p.direct[0] && (nz == 1 || p.direct[1])));
+  // beside_prev (caller's promise, see WgParams::late_wait): only without a clear kernel in between and
+  // without a zero-fill job, whose wait comes first
+  p.late_wait = (beside_prev && pdl && nclr == 0 && zero_fill == nullptr) ? 1 : 0;
   switch (r) {
     case 16: return launch_wg<16>(maps, p, grid, pdl, st);
     case 32: return launch_wg<32>(maps, p, grid, pdl, st);

@@ -6,7 +6,7 @@
 // a CTA owns 128 features x one slice of M, walks it in 64-row chunks, one thread issues four
 // tcgen05.mma kind::f16 per chunk with both operands MN-major into a TMEM accumulator.  The difference is
 // where the A operand comes from: TMA stages the chunk's codes (64 rows x 64 bytes) and its two 512-byte
-// scale tiles; four warps expand them to bf16 in the swizzled layout the MMA reads.  E2M1 x E4M3 has at
+// scale tiles; eight warps expand them to bf16 in the swizzled layout the MMA reads.  E2M1 x E4M3 has at
 // most six significant bits, so e2m1 * sf is EXACT in f16 and in bf16: the dequantizer rounds nothing,
 // and the tensor scale g_dec is one fp32 multiply on the drained accumulator.
 #include <cuda_fp16.h>
@@ -20,7 +20,7 @@ int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t
 constexpr int WQ_F = 128;
 constexpr int WQ_MC = 64;
 constexpr int WQ_STAGES = 3;
-constexpr int WQ_THREADS = 256;                // warp 0 TMA, 1 MMA, 2 TMEM owner, 4-7 dequantize
+constexpr int WQ_THREADS = 384;                // warp 0 TMA, 1 MMA, 2 TMEM owner, 4-11 dequantize
 constexpr int WQ_IN_BYTES = 2 * WQ_MC * 128;   // two 64-feature boxes of bf16
 constexpr int WQ_LG_BYTES = WQ_MC * 128;       // one 64-column group of P
 constexpr int WQ_CODE_BYTES = WQ_MC * 64;      // 64 rows x 128 fp4
@@ -31,6 +31,10 @@ struct WqParams {
   int r_s;
   int chunks_per_cta;
   int direct;
+  int late_wait;              // 1: everything this kernel reads or clears was complete before its predecessor
+                              //    triggered (see launch_wgrad_q4): run beside the predecessor and wait for
+                              //    it at the END, so that "this kernel is complete" still implies "everything
+                              //    before it in the stream is complete" for whatever is launched next
   int64_t sf_tiles_per_row;   // ceil(F / 64)
   const uint8_t* sf;          // FT_SF_TILE128x4
   const float* g_dec;
@@ -94,7 +98,7 @@ k_wgrad_q4(const __grid_constant__ CUtensorMap map_codes, const __grid_constant_
     prefetch_tmap(&map_l);
     for (int s = 0; s < WQ_STAGES; ++s) {
       mbar_init(&raw_bar[s], 1);
-      mbar_init(&cvt_bar[s], 4);     // one arrival per dequantizer warp
+      mbar_init(&cvt_bar[s], 8);     // one arrival per dequantizer warp
       mbar_init(&empty_bar[s], 1);   // MMA commit
     }
     mbar_init(&acc_bar, 1);
@@ -108,7 +112,7 @@ k_wgrad_q4(const __grid_constant__ CUtensorMap map_codes, const __grid_constant_
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
-  pdl_wait();      // P and Q(X) come from kernels before this one (no-op without a programmatic edge)
+  if (!p.late_wait) pdl_wait();   // P and Q(X) come from kernels before this one (no-op without a programmatic edge)
   pdl_trigger();
 
   if (warp == 0) {
@@ -147,7 +151,7 @@ k_wgrad_q4(const __grid_constant__ CUtensorMap map_codes, const __grid_constant_
       tc_commit(&acc_bar);
     }
   } else if (warp >= 4) {
-    // ---- dequantizer: thread = one 1x16 block at a time, four per chunk.  Eight consecutive threads
+    // ---- dequantizer: thread = one 1x16 block at a time, two per chunk.  Eight consecutive threads
     // cover one row's 128 features, a warp four rows.
     const int t = tid - 128;
     for (int it = 0; it < n_chunks; ++it) {
@@ -159,8 +163,8 @@ k_wgrad_q4(const __grid_constant__ CUtensorMap map_codes, const __grid_constant_
       const int64_t m0 = (c_begin + it) * WQ_MC;
       const int half = (int)((m0 >> 6) & 1);   // which 64 rows of the 128-row scale tile
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int q = i * 128 + t;
+      for (int i = 0; i < 2; ++i) {
+        const int q = i * 256 + t;
         const int row = q >> 3, b = q & 7;
         uint32_t w[8];
         // rows beyond M and features beyond F: zeros (their scale bytes are not defined)
@@ -231,6 +235,7 @@ k_wgrad_q4(const __grid_constant__ CUtensorMap map_codes, const __grid_constant_
     tc_fence_after();
     tmem_dealloc(tmem_base, TMEM_COLS);
   }
+  if (p.late_wait) pdl_wait();
 }
 
 template <int R>
@@ -255,8 +260,14 @@ static int launch_wq(const CUtensorMap* maps, const WqParams& p, dim3 grid, bool
 // dA [K x r] (+)= dequant(Q(X))^T P[:, r_s:].  codes [M x K/2], sf FT_SF_TILE128x4 over [M x K/16],
 // g_dec device float.  accumulate == 0 and a single M slice: plain stores; otherwise dA is cleared by
 // a small kernel first (accumulate == 0) and the slices combine with fp32 reductions.
+// beside_prev: the launch directly follows a kernel of the same call that (a) neither writes anything
+// this kernel touches nor reads dA and (b) passes griddepcontrol.wait in every CTA before it triggers its
+// dependents -- then all earlier work of the stream is complete when this kernel starts; it fills the SMs as
+// that kernel's CTAs retire and waits for it only before it exits (every CTA of the predecessor is
+// resident by then, so the wait cannot deadlock).
 int launch_wgrad_q4(const uint8_t* codes, const uint8_t* sf, const float* g_dec, int64_t M, int64_t K,
-                    const void* p_saved, int r_t, int r_s, int r, float* dA, int accumulate, cudaStream_t st) {
+                    const void* p_saved, int r_t, int r_s, int r, float* dA, int accumulate, bool beside_prev,
+                    cudaStream_t st) {
   CUtensorMap maps[2];
   int rc = make_tensor_map_2d(&maps[0], codes, 1, (uint64_t)K / 2, (uint64_t)M, (uint64_t)K / 2, 64, WQ_MC,
                               Swizzle::None);
@@ -267,7 +278,7 @@ int launch_wgrad_q4(const uint8_t* codes, const uint8_t* sf, const float* g_dec,
   const int64_t chunks = ceil_div(M, WQ_MC);
   const int64_t f_tiles = ceil_div(K, WQ_F);
   int64_t slices = (int64_t)2 * sm_count() / f_tiles;   // one wave of two resident CTAs per SM
-  if (slices > chunks / 8) slices = chunks / 8;
+  if (slices > chunks / 4) slices = chunks / 4;   // at least 4 chunks (256 rows) per slice
   if (slices < 1) slices = 1;
   WqParams p;
   p.M = M;
@@ -280,7 +291,8 @@ int launch_wgrad_q4(const uint8_t* codes, const uint8_t* sf, const float* g_dec,
   p.sf = sf;
   p.g_dec = g_dec;
   p.out = dA;
-  bool pdl = false;
+  bool pdl = beside_prev && accumulate != 0;
+  p.late_wait = pdl ? 1 : 0;
   if (!accumulate && !p.direct) {
     rc = launch_clear2(dA, (size_t)K * r * sizeof(float), nullptr, 0, st);
     if (rc != FT_OK) return rc;
