@@ -186,6 +186,13 @@ int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
                   int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
                   void* stream);
 
+/* ---- ft_linear_bwd with 4-bit saved activations: the same schedule, dA taken from qx = Q(X) as in
+ * ft_lora_wgrad_q4 (O-12').  qx and qg_scratch must be different buffers. */
+int ft_linear_bwd_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16, int64_t M,
+                     const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
+                     int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
+                     void* stream);
+
 /* ---- sizes and diagnostics (host only, no CUDA calls) */
 size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout);
 size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t);

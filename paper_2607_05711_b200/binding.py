@@ -57,6 +57,7 @@ def lib():
         L.ft_lora_wgrad.argtypes = [C.POINTER(_Layer), vp, vp, i64, vp, vp, vp, vp, i32, vp]
         L.ft_lora_wgrad_q4.argtypes = [C.POINTER(_Layer), C.POINTER(_QT), vp, i64, vp, vp, vp, vp, i32, vp]
         L.ft_linear_bwd.argtypes = [C.POINTER(_Layer), vp, vp, i64, vp, vp, vp, vp, vp, i32, C.POINTER(_QT), vp, sz, vp]
+        L.ft_linear_bwd_q4.argtypes = [C.POINTER(_Layer), C.POINTER(_QT), vp, i64, vp, vp, vp, vp, vp, i32, C.POINTER(_QT), vp, sz, vp]
         L.ft_sf_bytes.argtypes = [i64, i64, i32, i32]
         L.ft_sf_bytes.restype = sz
         L.ft_workspace_bytes.argtypes = [i64, i64, i64, i32]
@@ -220,6 +221,17 @@ def ft_linear_bwd(layer, x, g, h_saved, dx, p_saved, dA, dBt, qg, workspace, acc
     _check(lib().ft_linear_bwd(C.byref(L), _ptr(x), _ptr(g), g.shape[0], _ptr(h_saved), _ptr(dx), _ptr(p_saved),
                                _ptr(dA), _ptr(dBt), 1 if accumulate else 0, C.byref(q), _ptr(workspace),
                                workspace.numel(), _stream(stream)))
+    qg.sync_from(q)
+    return dx, dA, dBt
+
+
+def ft_linear_bwd_q4(layer, qx, g, h_saved, dx, p_saved, dA, dBt, qg, workspace, accumulate=False, stream=None):
+    """ft_linear_bwd with dA taken from the saved Q(X) instead of the bf16 X."""
+    _bf16(g)
+    L, qi, q = layer.c(), qx.c(), qg.c()
+    _check(lib().ft_linear_bwd_q4(C.byref(L), C.byref(qi), _ptr(g), g.shape[0], _ptr(h_saved), _ptr(dx), _ptr(p_saved),
+                                  _ptr(dA), _ptr(dBt), 1 if accumulate else 0, C.byref(q), _ptr(workspace),
+                                  workspace.numel(), _stream(stream)))
     qg.sync_from(q)
     return dx, dA, dBt
 

@@ -356,13 +356,21 @@ int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
                          1, chained, st);
 }
 
-int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
-                  const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
-                  int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
-                  void* stream) {
+// the whole backward; qx != NULL: dA from the saved 4-bit activations (x_bf16 unused)
+static int linear_bwd(const ft_layer* L, const void* x_bf16, const ft_qtensor* qx, const void* g_bf16, int64_t M,
+                      const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
+                      int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
+                      void* stream) {
   cudaStream_t st = (cudaStream_t)stream;
   int rc = check_layer(L);
   if (rc != FT_OK) return rc;
+  if (qx != nullptr) {
+    if (!qx->codes || !qx->sf || !qx->tensor_dec_scale) return FT_ERR_INVALID_ARG;
+    if (qx->rows != M || qx->cols != L->K || qx->block_rows != 1 || qx->sf_layout != FT_SF_TILE128x4 ||
+        !aligned16(qx->sf))
+      return FT_ERR_INVALID_ARG;
+    x_bf16 = qx->codes;   // for the pointer checks below; never read as bf16
+  }
   rc = check_wgrad(L, x_bf16, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt);
   if (rc != FT_OK) return rc;
   if (!workspace || !aligned16(workspace)) return FT_ERR_INVALID_ARG;
@@ -375,8 +383,10 @@ int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
     rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
                      workspace, workspace_bytes, nullptr, st);
     if (rc != FT_OK) return rc;
-    return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                        accumulate, nullptr, nullptr, 0, false, false, st);
+    if (qx == nullptr)
+      return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
+                          accumulate, nullptr, nullptr, 0, false, false, st);
+    return ft_lora_wgrad_q4(L, qx, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt, accumulate, stream);
   }
   // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0).  The
   //    workspace's control words (the amax word among them) and dB^T are cleared by ONE small kernel with
@@ -398,8 +408,29 @@ int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   //    Nothing it touches depends on the GEMM in front of it (X, P in; dA out), and every CTA of the GEMM
   //    passes its own wait -- P complete -- before triggering: dA starts in the GEMM's tail and waits for
   //    the GEMM only before it exits.
-  return launch_wgrad(1, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                      1, nullptr, nullptr, 0, true, true, st);
+  if (qx == nullptr)
+    return launch_wgrad(1, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
+                        1, nullptr, nullptr, 0, true, true, st);
+  return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA, 1,
+                         true, st);
+}
+
+int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
+                  const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
+                  int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
+                  void* stream) {
+  if (!x_bf16) return FT_ERR_INVALID_ARG;
+  return linear_bwd(L, x_bf16, nullptr, g_bf16, M, h_saved_bf16, dx_bf16, p_saved_bf16, dA, dBt, accumulate,
+                    qg_scratch, workspace, workspace_bytes, stream);
+}
+
+int ft_linear_bwd_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16, int64_t M,
+                     const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
+                     int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
+                     void* stream) {
+  if (!qx) return FT_ERR_INVALID_ARG;
+  return linear_bwd(L, nullptr, qx, g_bf16, M, h_saved_bf16, dx_bf16, p_saved_bf16, dA, dBt, accumulate,
+                    qg_scratch, workspace, workspace_bytes, stream);
 }
 
 }  // extern "C"

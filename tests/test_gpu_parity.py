@@ -343,6 +343,28 @@ def test_wgrad_saved4(B, seed, M, K, N, r_s, r):
     assert rel(dA.cpu().numpy(), 2 * once) <= 1e-5 and rel(dBt.cpu().numpy(), 2 * o["dBt"]) <= 1e-5
 
 
+@pytest.mark.parametrize("seed,M,K,N,r_s,r", [(58, 300, 576, 448, 32, 32), (59, 1100, 512, 2048, 16, 16)])
+def test_fused_backward_saved4(B, qmode, seed, M, K, N, r_s, r):
+    """ft_linear_bwd_q4 (both schedules, see test_layer_fused_backward) = ft_linear_bwd with dA from Q(X)."""
+    d, R, D_f, U_f, L = make_layer(B, seed, M, K, N, r_s, r)
+    o = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=True)
+    dx = torch.zeros(M, K, dtype=torch.bfloat16, device="cuda")
+    p = torch.zeros_like(o["pt"])
+    dA = torch.full((K, r), 7.0, dtype=torch.float32, device="cuda")
+    dBt = torch.full((N, r), 7.0, dtype=torch.float32, device="cuda")
+    ws = torch.zeros(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_s + r), dtype=torch.uint8, device="cuda")
+    qg = B.QTensor(M, N)
+    B.ft_linear_bwd_q4(L, o["qx"], o["gt"], o["ht"], dx, p, dA, dBt, qg, ws)
+    torch.cuda.synchronize()
+    assert torch.equal(qg.codes, o["qg"].codes) and np.array_equal(npf(dx), o["dx"]) and np.array_equal(npf(p), o["p"])
+    assert rel(dBt.cpu().numpy(), o["dBt"]) <= 1e-5
+    w = olayer.wgrad_saved4(nvfp4.quantize_blockwise(d["X"], 1), d["dY"], o["h"], o["p"], r_s)
+    assert rel(dA.cpu().numpy(), w["dA"]) <= 1e-5
+    B.ft_linear_bwd_q4(L, o["qx"], o["gt"], o["ht"], dx, p, dA, dBt, qg, ws, accumulate=True)
+    torch.cuda.synchronize()
+    assert rel(dA.cpu().numpy(), 2 * w["dA"]) <= 1e-5 and rel(dBt.cpu().numpy(), 2 * o["dBt"]) <= 1e-5
+
+
 def test_wgrad_saved4_errors(B):
     M, K, N, r_s, r = 128, 256, 128, 16, 16
     d, R, D_f, U_f, L = make_layer(B, 57, M, K, N, r_s, r)
