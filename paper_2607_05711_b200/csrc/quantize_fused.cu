@@ -30,7 +30,9 @@
 //   single pass (amax not known, tensor <= 12 chunks per SM = 29 MB on 148 SMs): one CTA per SM, every
 //     chunk stays resident in shared memory; phase 1 finds the tensor amax (and runs the projection
 //     MMAs) as the chunks land, a grid-wide barrier publishes it, phase 2 quantizes from shared
-//     memory, a second grid barrier precedes the slot sums (each CTA an equal share of the rows).
+//     memory, a second grid barrier precedes the slot sums (each CTA an equal share of the rows); it is
+//     split-phase: a CTA arrives as soon as its slots are written (before phase 2) and waits after
+//     phase 2, when every CTA has long arrived.
 //     The tensor is read from HBM exactly once and the separate amax kernel (a0) disappears.
 //     Launched cooperatively (all CTAs co-resident); the barrier spin traps after 2 s instead of hanging.
 #include <cstdio>
@@ -256,19 +258,6 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       if (lane == 0) mbar_arrive(&acc_free[a]);   // the accumulator may be overwritten
     }
   };
-  // grid-wide barrier on a zeroed counter (every CTA of the launch is resident: cooperative launch).
-  // Quantizer warps only; release / acquire at gpu scope, cumulative through the CTA barrier.
-  auto grid_barrier = [&](uint32_t* counter) {
-    qsync();
-    if (tid == 0) {
-      asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
-      const uint64_t t0 = globaltimer_ns();
-      while (ld_acquire_u32(counter) < gridDim.x) {
-        if (globaltimer_ns() - t0 > 2000000000ull) __trap();   // co-residency broken: fail, do not hang
-      }
-    }
-    qsync();
-  };
   // After the grid barrier every partial H tile is in its slot.  CTA i completes rows
   // [i * rows / G, (i + 1) * rows / G): fp32 sum of the row tile's slots in CTA order (fixed order:
   // the result does not depend on timing) -> bf16 H and Hs = H * (1 / alpha).
@@ -469,6 +458,12 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
     if constexpr (R_T > 0) {
       drain_segment(o_t, 0);
       if (n > n0) drain_segment(o_t + 1, 1);
+      // split-phase second barrier: ARRIVE now (this CTA's slots are written), wait only after phase 2 --
+      // by then every CTA has long arrived and the wait costs one poll instead of a barrier round trip
+      if (warp < 4) {
+        asm volatile("bar.sync 2, 128;" ::: "memory");   // the four draining warps
+        if (tid == 0) asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p.grid_bar + 1) : "memory");
+      }
     }
     // ---- grid-wide barrier: every CTA has published its amax
     if (tid == 0) {
@@ -491,7 +486,13 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       advance_out();
     }
     if constexpr (R_T > 0) {
-      grid_barrier(p.grid_bar + 1);   // every CTA's slots are written
+      if (tid == 0) {   // every CTA's slots are written (they arrived before their phase 2)
+        const uint64_t t0 = globaltimer_ns();
+        while (ld_acquire_u32(p.grid_bar + 1) < gridDim.x) {
+          if (globaltimer_ns() - t0 > 2000000000ull) __trap();
+        }
+      }
+      qsync();
       finalize_share(inv_alpha);
     }
     }
