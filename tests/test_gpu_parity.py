@@ -433,7 +433,19 @@ def test_layer_full_size_sampled(B, name):
     (rows of Y / dX depend only on their own row of X / G and the tensor amax).  The weight
     split uses a cheap randomized range finder instead of a full SVD: any L1, L2 is a valid
     stabilizer for parity purposes (the oracle receives the same R, L1, L2)."""
-    seed, M, K, N, r_s, r, kind = synth.CONFIGS[name]
+    _full_size_sampled(B, *synth.CONFIGS[name])
+
+
+@pytest.mark.parametrize("name", ["single.lin1", "single.lin2", "dual.txt.mlp_down", "dual.img.proj"])
+def test_layer_c5_shapes_sampled(B, name):
+    """BASELINE.json configs[4]: the extreme shapes of the FLUX.1-dev-shaped layer list (widest N = 21504,
+    deepest K = 15360, the 512-token text stream, the square 4096-token projection), r_s = r = 32, seed 4,
+    same sampled comparison as above."""
+    _, _, M, K, N = next(l for l in synth.C5_LAYERS if l[0] == name)
+    _full_size_sampled(B, 4, M, K, N, 32, 32, "outlier")
+
+
+def _full_size_sampled(B, seed, M, K, N, r_s, r, kind):
     d = synth.layer_inputs(seed, M, K, N, r, kind)
     rng = synth.make_rng(seed + 100)
     W = d["W"].astype(np.float64)
@@ -447,7 +459,7 @@ def test_layer_full_size_sampled(B, name):
     # the schedule bench.py times: ft_linear_fwd + ft_linear_bwd (C2, C3u: G is too large for the
     # single-pass quantizer -> dB^T pass with the amax of G first; C3d: G fits -> quantize, GEMM, one wgrad)
     out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=True)
-    rows = np.array(sorted({0, 1, 127, 128, 129, 1000, 2047, 2048, 3333, M - 129, M - 2, M - 1}))
+    rows = np.array(sorted({0, 1, 127, 128, 129, 1000 % M, 2047 % M, 2048 % M, 3333 % M, M - 129, M - 2, M - 1}))
     check_layer(B, d, R, D_f, U_f, out, r_s, r, rows=rows)
     # wgrad on sampled output rows: dA[k, :] = X[:, k]^T P_lora, dB[:, n] = H_lora^T G[:, n]
     ks = np.array([0, 1, 63, 64, 777, K - 1]); ns = np.array([0, 5, 127, 128, 2000, N - 1])
