@@ -304,11 +304,14 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
   if constexpr (!SINGLE) {
     // =========================================================== streaming mode (amax known)
     // a stage = the X chunk and its D slice; both land on full_x[slot] (issue_d is given that barrier)
+    const uint64_t pol_stream = l2_policy_evict_first();
     auto issue_stage = [&](int it, int slot) {
       const int64_t c = c_begin + it;
       const int t = (int)(c / C), kc = (int)(c % C);
       mbar_expect_tx(&full_x[slot], QF_X_BYTES + (R_T > 0 ? D_BYTES : 0));
-      tma_load_2d(smem + slot * QF_X_BYTES, &map_x, &full_x[slot], kc * QF_KC, t * QF_ROWS);
+      // streaming mode reads its tensor for the last time: evict-first, so that what the pass before left
+      // in L2 (the dB^T pass over the same G) is not displaced by lines nobody reads again
+      tma_load_2d_hint(smem + slot * QF_X_BYTES, &map_x, &full_x[slot], kc * QF_KC, t * QF_ROWS, pol_stream);
       if constexpr (R_T > 0) {
 #pragma unroll
         for (int g = 0; g < NG; ++g)

@@ -95,14 +95,22 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
 
   if (warp == 0) {
     if (elect_one()) {   // ---- TMA producer
+      // the pass that also finds max |G| is followed by the quantize pass over the same G: ask L2 to keep it
+      const bool keep = p.amax_bits[z] != nullptr;
+      const uint64_t pol = l2_policy_evict_last();
       for (int it = 0; it < n_chunks; ++it) {
         const int s = it % WG_STAGES;
         mbar_wait(&empty_bar[s], ((it / WG_STAGES) & 1) ^ 1);
         uint8_t* base = smem + s * STAGE_BYTES;
         const int32_t m0 = (int32_t)((c_begin + it) * WG_MC);
         mbar_expect_tx(&full_bar[s], STAGE_BYTES);
-        tma_load_2d(base, &map_in, &full_bar[s], f0, m0);
-        tma_load_2d(base + WG_MC * 128, &map_in, &full_bar[s], f0 + 64, m0);
+        if (keep) {
+          tma_load_2d_hint(base, &map_in, &full_bar[s], f0, m0, pol);
+          tma_load_2d_hint(base + WG_MC * 128, &map_in, &full_bar[s], f0 + 64, m0, pol);
+        } else {
+          tma_load_2d(base, &map_in, &full_bar[s], f0, m0);
+          tma_load_2d(base + WG_MC * 128, &map_in, &full_bar[s], f0 + 64, m0);
+        }
 #pragma unroll
         for (int g = 0; g < NG; ++g)
           tma_load_2d(base + WG_IN_BYTES + g * WG_LG_BYTES, &map_l, &full_bar[s], p.r_s + g * 64, m0);
