@@ -17,13 +17,11 @@ int launch_quantize_generic(const void* x, int64_t rows, int64_t cols, const flo
                             ft_qtensor* out, cudaStream_t st);
 int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t,
                           const ft_proj* proj, ft_qtensor* out, void* workspace, bool zero_region_cleared,
-                          cudaStream_t st);
+                          bool* finalize_last, cudaStream_t st);
 int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, cudaStream_t st);
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
-                 const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16,
+                 const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, bool lr_late,
                  cudaStream_t st);
-int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
-                      const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st);
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
                  unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, bool beside_prev,
@@ -137,9 +135,11 @@ static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_
   pr.r_t = r_t;
   // a0 + a1/a3: the tensor amax is found inside the quantize pass when the tensor fits the SMs'
   // shared memory (single pass), by a preceding k_amax launch otherwise
-  rc = launch_quantize_fused(act, M, Kd, act_amax, r_t > 0 ? &pr : nullptr, q, workspace, act_amax != nullptr, st);
+  bool finalize_last = false;   // streaming route: k_finalize_h (which writes only H and Hs) is the last launch
+  rc = launch_quantize_fused(act, M, Kd, act_amax, r_t > 0 ? &pr : nullptr, q, workspace, act_amax != nullptr,
+                             &finalize_last, st);
   if (rc != FT_OK) return rc;
-  return launch_gemm4(q, w, M, Nd, Kd, r_t > 0 ? hs : nullptr, lr_up, r_t, out, st);
+  return launch_gemm4(q, w, M, Nd, Kd, r_t > 0 ? hs : nullptr, lr_up, r_t, out, finalize_last, st);
 }
 
 static int check_layer(const ft_layer* L) {
@@ -244,7 +244,7 @@ int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols, const 
     }
     return launch_quantize_generic(x_bf16, rows, cols, amax, out, st);
   }
-  return launch_quantize_fused(x_bf16, rows, cols, tensor_amax, proj, out, workspace, false, st);
+  return launch_quantize_fused(x_bf16, rows, cols, tensor_amax, proj, out, workspace, false, nullptr, st);
 }
 
 int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, void* stream) {
@@ -285,7 +285,7 @@ int ft_gemm4(const ft_qtensor* a, const ft_qtensor* b, const void* lr_a_scaled, 
     return FT_ERR_INVALID_ARG;
   int rc = device_check();
   if (rc != FT_OK) return rc;
-  return launch_gemm4(a, b, a->rows, b->rows, a->cols, lr_a_scaled, lr_b, r_t, out_bf16,
+  return launch_gemm4(a, b, a->rows, b->rows, a->cols, lr_a_scaled, lr_b, r_t, out_bf16, false,
                       (cudaStream_t)stream);
 }
 

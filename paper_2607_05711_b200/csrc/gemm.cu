@@ -247,7 +247,7 @@ static int launch_gemm4_bn(const CUtensorMap& ma, const CUtensorMap& mb, const C
 }
 
 int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
-                      const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st);
+                      const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, bool lr_late, cudaStream_t st);
 int g_force_bn = 0;  // test/bench hook: 0 = CTA-pair kernel (default), else 1-CTA kernel with this N tile
 
 template <int BN>
@@ -282,10 +282,12 @@ static int setup_and_launch(const ft_qtensor* a, const ft_qtensor* b, int64_t M,
   return launch_gemm4_bn<BN>(ma, mb, mh, mu, p, st);
 }
 
+// lr_late: the launch directly follows k_finalize_h of the same call, which writes nothing the GEMM reads
+// except lr_a_scaled: the pair kernel may start beside it (gemm_pair.cu); the 1-CTA kernels ignore it
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
-                 const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, cudaStream_t st) {
+                 const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, bool lr_late, cudaStream_t st) {
   const int bn = g_force_bn;
-  if (bn == 0) return launch_gemm4_pair(a, b, M, N, K, lr_a_scaled, lr_b, r_t, out_bf16, st);
+  if (bn == 0) return launch_gemm4_pair(a, b, M, N, K, lr_a_scaled, lr_b, r_t, out_bf16, lr_late, st);
   if (bn == 256) return setup_and_launch<256>(a, b, M, N, K, lr_a_scaled, lr_b, r_t, out_bf16, st);
   if (bn == 192) return setup_and_launch<192>(a, b, M, N, K, lr_a_scaled, lr_b, r_t, out_bf16, st);
   return setup_and_launch<128>(a, b, M, N, K, lr_a_scaled, lr_b, r_t, out_bf16, st);

@@ -38,6 +38,7 @@ constexpr int P_SMEM = P_STAGES * P_STAGE_BYTES + 2 * P_OUT_BYTES + 1024;
 struct PairParams {
   int64_t M, N, K;
   int r_t;
+  int lr_late;   // 1: only the low-rank operand Hs depends on the kernel in front (k_finalize_h), see below
   const float* g_dec_a;
   const float* g_dec_b;
   __nv_bfloat16* out;
@@ -89,14 +90,23 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
   cluster_sync();
   tc_fence_after();
   const uint32_t tmem_base = tmem_base_s;
-  pdl_wait();      // the operands (codes, scales, Hs, tensor scales) come from the preceding quantize kernel
-  pdl_trigger();   // the next kernel may set itself up while this one runs
+  // Programmatic edge to the kernel in front.  Normally everything this kernel reads comes from it: wait, then
+  // let the next kernel set itself up.  lr_late: the kernel in front is k_finalize_h, which writes only the
+  // low-rank operand Hs (and H), and every one of ITS CTAs has passed its own wait before this grid could
+  // start -- so the codes, scales and tensor scales (quantize kernel) are complete already.  The 4-bit stages
+  // of the first tile then run beside k_finalize_h; each producer waits just before its first Hs load and
+  // triggers the dependents only there (the dA kernel behind us reads P, also written by k_finalize_h).
+  if (!p.lr_late) {
+    pdl_wait();
+    pdl_trigger();
+  }
 
   if (warp == 0) {
     // ===================================================== TMA producer (both CTAs)
     if (elect_one()) {
       int stage = 0;
       uint32_t phase = 0;
+      bool lr_waited = !p.lr_late;
       for (int64_t tile = pair_id; tile < n_tiles; tile += n_pairs) {
         const int64_t mt = tile % tiles_m, nt = tile / tiles_m;
         const int32_t m0 = (int32_t)(mt * P_BM + rank * 128);   // this CTA's rows of A
@@ -117,6 +127,11 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
             tma_load_2d_pair(ssfb, &map_sfb, bar, 0, (int32_t)(sfb_rt * sf_tiles_k + kt * 4));
             tma_load_2d_pair(ssfb + 2048, &map_sfb, bar, 0, (int32_t)((sfb_rt + 1) * sf_tiles_k + kt * 4));
           } else {
+            if (!lr_waited) {   // first Hs load of this CTA: k_finalize_h must be complete
+              pdl_wait();
+              pdl_trigger();
+              lr_waited = true;
+            }
             const int c0 = (kt - k4) * 64;
             if (leader) mbar_expect_tx(&full_bar[stage], 2 * (P_A_BYTES + P_B_BYTES));
             tma_load_2d_pair(sa, &map_h, bar, c0, m0);
@@ -243,6 +258,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
     if (et == 0) tma_store_wait<0>();
   }
 
+  if (p.lr_late) pdl_wait();   // every thread: "this grid complete" implies "k_finalize_h complete" (no-op if passed)
   tc_fence_before();
   cluster_sync();   // no CTA of the pair exits (or frees TMEM) while its peer still uses it
   if (warp == 2) {
@@ -252,7 +268,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
 }
 
 int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
-                      const void* lr_a, const void* lr_b, int r_t, void* out, cudaStream_t st) {
+                      const void* lr_a, const void* lr_b, int r_t, void* out, bool lr_late, cudaStream_t st) {
   CUtensorMap ma, mb, msa, msb, mh, mu, mo;
   int rc = make_tensor_map_2d(&ma, a->codes, 1, (uint64_t)K / 2, (uint64_t)M, (uint64_t)K / 2, 128, 128,
                               Swizzle::B128);
@@ -281,6 +297,7 @@ int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64
   p.N = N;
   p.K = K;
   p.r_t = r_t;
+  p.lr_late = (lr_late && r_t > 0 && pdl_enabled()) ? 1 : 0;
   p.g_dec_a = a->tensor_dec_scale;
   p.g_dec_b = b->tensor_dec_scale;
   p.out = reinterpret_cast<__nv_bfloat16*>(out);

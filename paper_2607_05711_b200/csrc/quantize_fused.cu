@@ -570,7 +570,7 @@ void set_quantize_mode(int mode) { g_qf_mode = mode; }
 
 template <int R_T>
 static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, const void* x, const float* amax_t,
-                     bool after_kernel, cudaStream_t st) {
+                     bool after_kernel, bool* finalize_last, cudaStream_t st) {
   constexpr int NG = (R_T + 63) / 64;
   constexpr int D_BYTES = NG * QF_DG_BYTES;
   constexpr int SMEM_MAX = 227 * 1024 - 2048;   // minus the static shared memory (barriers, table)
@@ -664,6 +664,7 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
     cfg.attrs = attr;
     cfg.numAttrs = pdl_enabled() ? 1 : 0;
     FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_finalize_h<(R_T > 0 ? R_T : 16)>, p, grid));
+    if (finalize_last != nullptr) *finalize_last = true;   // the caller's GEMM may start beside it (gemm_pair.cu)
   }
   return FT_OK;
 }
@@ -684,8 +685,10 @@ bool quantize_single_pass_fits(int64_t rows, int64_t cols, int r_t) {
 // grid-barrier counters; it is cleared here with one 256-byte memset node.  The partial-H slots behind
 // it need no clearing.
 int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t, const ft_proj* proj,
-                          ft_qtensor* out, void* workspace, bool zero_region_cleared, cudaStream_t st) {
+                          ft_qtensor* out, void* workspace, bool zero_region_cleared, bool* finalize_last,
+                          cudaStream_t st) {
   const int r_t = proj ? proj->r_t : 0;
+  if (finalize_last != nullptr) *finalize_last = false;
   CUtensorMap mx, md;
   int rc = make_tensor_map_2d(&mx, x, 2, (uint64_t)cols, (uint64_t)rows, (uint64_t)cols * 2, QF_KC, QF_ROWS,
                               Swizzle::B128);
@@ -731,15 +734,15 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
   // a memset of ours in front of the kernel (below) breaks the programmatic chain
   if (out->sf_layout == FT_SF_TILE128x4 && rows % 128 != 0) after_kernel = false;
   switch (r_t) {
-    case 0: return launch_qf<0>(mx, md, p, x, amax_t, after_kernel, st);
-    case 16: return launch_qf<16>(mx, md, p, x, amax_t, after_kernel, st);
-    case 32: return launch_qf<32>(mx, md, p, x, amax_t, after_kernel, st);
-    case 48: return launch_qf<48>(mx, md, p, x, amax_t, after_kernel, st);
-    case 64: return launch_qf<64>(mx, md, p, x, amax_t, after_kernel, st);
-    case 80: return launch_qf<80>(mx, md, p, x, amax_t, after_kernel, st);
-    case 96: return launch_qf<96>(mx, md, p, x, amax_t, after_kernel, st);
-    case 112: return launch_qf<112>(mx, md, p, x, amax_t, after_kernel, st);
-    case 128: return launch_qf<128>(mx, md, p, x, amax_t, after_kernel, st);
+    case 0: return launch_qf<0>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
+    case 16: return launch_qf<16>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
+    case 32: return launch_qf<32>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
+    case 48: return launch_qf<48>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
+    case 64: return launch_qf<64>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
+    case 80: return launch_qf<80>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
+    case 96: return launch_qf<96>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
+    case 112: return launch_qf<112>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
+    case 128: return launch_qf<128>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
     default: return FT_ERR_UNSUPPORTED_SHAPE;
   }
 }
