@@ -29,8 +29,8 @@ METRIC = "W4A4G4 linear fwd+bwd TFLOPS (4*M*N*K per step / step time)"
 UNIT = "TFLOP/s"
 FP4_OVER_BF16 = 4.0   # nominal dense ratio 9 / 2.25 PFLOP/s (B200_PROFILING.md)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_gemm4 launch (C2 forward), from the
-# ncu --set full capture summarised in profiles/r01f_full_summary.md (ncu flushes caches per launch).
-GEMM_DRAM_TRAFFIC_BYTES = 57137664   # 25.70 MB read + 31.44 MB written, profiles/r01f_full_summary.md
+# ncu --set full capture summarised in profiles/r01g_full_summary.md (ncu flushes caches per launch).
+GEMM_DRAM_TRAFFIC_BYTES = 57590000   # 25.70 MB read + 31.89 MB written, profiles/r01g_full_summary.md
 
 
 def load_peaks():

@@ -473,3 +473,16 @@ def _full_size_sampled(B, seed, M, K, N, r_s, r, kind):
     Xq = nvfp4.dequantize(nvfp4.quantize_blockwise(d["X"], 1))
     assert rel(dA4.cpu().numpy()[ks], Xq[:, ks].T @ Pl) <= 1e-5
     assert rel(dBt4.cpu().numpy()[ns], d["dY"][:, ns].astype(np.float64).T @ Hl) <= TOL
+
+
+def test_without_programmatic_launch():
+    """FT_PDL=0 switches every programmatic edge (and with it the late-wait modes of the dA kernels and of the
+    dgrad GEMM) off: the plain stream-ordered schedule must give the same answers.  Re-runs the fused-backward,
+    saved-activation and small-layer parity tests in a fresh process, since the switch is read once per process."""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, FT_PDL="0")
+    r = subprocess.run([sys.executable, "-m", "pytest", "tests/test_gpu_parity.py", "-x", "-q", "-m", "gpu", "-k",
+                        "fused_backward or saved4 or layer_small"], cwd=root, env=env, capture_output=True, text=True,
+                       timeout=900)
+    assert r.returncode == 0 and " passed" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
