@@ -168,12 +168,23 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
           if (kt < k4) {
             const int nk = (int)min((int64_t)4, sf_tiles_k - (int64_t)kt * 4);
             const uint32_t ssfa = sb + P_B_BYTES, ssfb = ssfa + P_SFA_BYTES;
-            for (int k = 0; k < nk; ++k) {
-              tc_cp_sf_pair(sfa_t, make_smem_desc(ssfa + k * 512, 128, 0, 0));
-              tc_cp_sf_pair(sfb_t, make_smem_desc(ssfb + k * 512, 128, 0, 0));
-              tc_cp_sf_pair(sfb_t + 4, make_smem_desc(ssfb + 2048 + k * 512, 128, 0, 0));
-              mma_nvf4_pair(acc_t, make_smem_desc(sa + k * 32, 1024, 0, 2), make_smem_desc(sb + k * 32, 1024, 0, 2),
-                            idesc4, sfa_t, sfb_t, (kt | k) != 0);
+            // one descriptor per operand and stage; the K=64 steps advance the 16-byte address field by a
+            // constant (the stage buffers are 1024-byte aligned, the field cannot carry)
+            const uint64_t da = make_smem_desc(sa, 1024, 0, 2), db = make_smem_desc(sb, 1024, 0, 2);
+            const uint64_t dfa = make_smem_desc(ssfa, 128, 0, 0), dfb = make_smem_desc(ssfb, 128, 0, 0);
+            auto step = [&](int k) {
+              tc_cp_sf_pair(sfa_t, dfa + (uint64_t)(k * 32));
+              tc_cp_sf_pair(sfb_t, dfb + (uint64_t)(k * 32));
+              tc_cp_sf_pair(sfb_t + 4, dfb + (uint64_t)(128 + k * 32));
+              mma_nvf4_pair(acc_t, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc4, sfa_t, sfb_t, (kt | k) != 0);
+            };
+            if (nk == 4) {   // every stage but a ragged last one: straight-line code
+              step(0);
+              step(1);
+              step(2);
+              step(3);
+            } else {
+              for (int k = 0; k < nk; ++k) step(k);
             }
           } else {
             const int cols = min(64, p.r_t - (kt - k4) * 64);
