@@ -29,8 +29,8 @@ METRIC = "W4A4G4 linear fwd+bwd TFLOPS (4*M*N*K per step / step time)"
 UNIT = "TFLOP/s"
 FP4_OVER_BF16 = 4.0   # nominal dense ratio 9 / 2.25 PFLOP/s (B200_PROFILING.md)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_gemm4 launch (C2 forward), from the
-# ncu --set full capture summarised in profiles/r01g_full_summary.md (ncu flushes caches per launch).
-GEMM_DRAM_TRAFFIC_BYTES = 57590000   # 25.70 MB read + 31.89 MB written, profiles/r01g_full_summary.md
+# ncu --set full capture summarised in profiles/r01h_launches.md (ncu flushes caches per launch).
+GEMM_DRAM_TRAFFIC_BYTES = 57846272   # 25.69 MB read + 32.15 MB written, profiles/r01h_launches.md
 
 
 def load_peaks():
