@@ -189,8 +189,9 @@ def run_ours(args):
         if world > 1:
             parallel.allreduce_lora_grads(dA, dBt)
     # fwd: k_quantize_fused (single pass, amax inside) + k_gemm4_pair; bwd (ft_linear_bwd): k_wgrad (dB^T + amax
-    # of G) + k_quantize_fused (streaming) + k_finalize_h + k_gemm4_pair + k_wgrad (dA); memsets not counted
-    KERNELS_PER_STEP = 7
+    # of G) + k_quantize_fused (streaming) + k_finalize_h + k_gemm4_pair + k_wgrad (dA)
+    # plus the two k_clear2 launches (control words; the backward's also clears dB^T): 9 kernels, no memset node
+    KERNELS_PER_STEP = 9
 
     def barrier():
         if world > 1:
