@@ -107,8 +107,9 @@ int ft_tensor_amax(const void* x_bf16, int64_t n, float* amax_out, void* stream)
  * x_bf16 [rows x cols]; blocks are out->block_rows x 16 along cols.
  * tensor_amax: device float holding amax_t; NULL => the library computes it: inside the same
  *   kernel (one HBM read of x in total) when x is at most ~29 MB, by an extra pass otherwise.
- *   The fused projection accumulates H with fp32 reductions in the workspace (addition order not
- *   fixed).  workspace may be NULL only if tensor_amax != NULL and proj == NULL.
+ *   The fused projection keeps fp32 partial sums of H (one per CTA and 128-row tile) in the
+ *   workspace and adds them in a fixed order: the same bits on every run for a given shape.
+ *   workspace may be NULL only if tensor_amax != NULL and proj == NULL.
  * proj: NULL => quantize only.  Requires out->block_rows == 1 if non-NULL.
  * Requirements: cols % 64 == 0; rows % 16 == 0 if block_rows == 16; any rows >= 1
  *   otherwise.  out->rows/cols must equal rows/cols.  round_mode must be
