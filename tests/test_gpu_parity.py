@@ -486,3 +486,67 @@ def test_without_programmatic_launch():
                         "fused_backward or saved4 or layer_small"], cwd=root, env=env, capture_output=True, text=True,
                        timeout=900)
     assert r.returncode == 0 and " passed" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
+
+
+def test_back_to_back_steps_without_sync(B):
+    """The programmatic-launch shortcuts (dgrad GEMM started beside k_finalize_h, dA kernels started beside the
+    GEMM with their wait at the end, clear kernels with programmatic edges) must not let a step see a neighbour's
+    half-written buffers: 24 forward+backward steps enqueued back to back with no host sync, alternating two
+    inputs through the SAME output and scratch buffers, against the same two steps run alone.  G is large enough
+    (37 MB) for the streaming route, i.e. the schedule bench.py times."""
+    M, K, N, r_s, r = 4608, 512, 4096, 32, 32
+    r_t = r_s + r
+    d1, R, D_f, U_f, L = make_layer(B, 61, M, K, N, r_s, r)
+    d2 = synth.layer_inputs(62, M, K, N, r)
+    xs, gs = [t16(d1["X"]), t16(d2["X"])], [t16(d1["dY"]), t16(d2["dY"])]
+    y = torch.zeros(M, N, dtype=torch.bfloat16, device="cuda"); dx = torch.zeros(M, K, dtype=torch.bfloat16, device="cuda")
+    h = torch.zeros(M, r_t, dtype=torch.bfloat16, device="cuda"); p = torch.zeros_like(h)
+    ws = torch.zeros(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_t), dtype=torch.uint8, device="cuda")
+    qx, qg = B.QTensor(M, K), B.QTensor(M, N)
+    dA = torch.zeros(K, r, dtype=torch.float32, device="cuda"); dBt = torch.zeros(N, r, dtype=torch.float32, device="cuda")
+
+    def step(i, q4):
+        B.ft_linear_fwd(L, xs[i], y, h, qx, ws)
+        if q4:
+            B.ft_linear_bwd_q4(L, qx, gs[i], h, dx, p, dA, dBt, qg, ws)
+        else:
+            B.ft_linear_bwd(L, xs[i], gs[i], h, dx, p, dA, dBt, qg, ws)
+        return [t.clone() for t in (y, dx, h, p, qx.codes, qg.codes, dA, dBt)]   # stream-ordered copies
+
+    for q4 in (False, True):
+        ref = []
+        for i in (0, 1):
+            torch.cuda.synchronize()
+            ref.append(step(i, q4))
+            torch.cuda.synchronize()
+        got = [step(it & 1, q4) for it in range(24)]
+        torch.cuda.synchronize()
+        for it, out in enumerate(got):
+            want = ref[it & 1]
+            for j in range(6):      # Y, dX, H, P, codes: the same bits as the step run alone
+                assert torch.equal(out[j], want[j]), (q4, it, j)
+            for j in (6, 7):        # dA, dB^T: fp32 reductions in no fixed order
+                assert rel(out[j].cpu().numpy(), want[j].cpu().numpy()) <= 1e-5, (q4, it, j)
+        # the same with NOTHING between the calls (the clones above are kernels of their own): the last kernel of
+        # one step (dA, late wait) is directly followed by the first of the next (clear kernel, programmatic edge)
+        for n_steps in (2, 3, 8):
+            for it in range(n_steps):
+                B.ft_linear_fwd(L, xs[it & 1], y, h, qx, ws)
+                if q4:
+                    B.ft_linear_bwd_q4(L, qx, gs[it & 1], h, dx, p, dA, dBt, qg, ws)
+                else:
+                    B.ft_linear_bwd(L, xs[it & 1], gs[it & 1], h, dx, p, dA, dBt, qg, ws)
+            torch.cuda.synchronize()
+            want = ref[(n_steps - 1) & 1]
+            for j, t in enumerate((y, dx, h, p, qx.codes, qg.codes)):
+                assert torch.equal(t, want[j]), (q4, n_steps, j)
+            assert rel(dA.cpu().numpy(), want[6].cpu().numpy()) <= 1e-5 and rel(dBt.cpu().numpy(), want[7].cpu().numpy()) <= 1e-5
+    # and the forward of step 0 is right in the first place (sampled rows against the oracle)
+    rows = np.array([0, 127, 128, 2047, M - 1])
+    qR = olayer.quantize_weight(R)
+    torch.cuda.synchronize()
+    B.ft_linear_fwd(L, xs[0], y, h, qx, ws)
+    torch.cuda.synchronize()
+    hs = npf(ws[256:256 + M * r_t * 2].view(torch.bfloat16).reshape(M, r_t))
+    f = olayer.forward(d1["X"][rows], qR, D_f, U_f, prescale=True, x_amax=nvfp4.tensor_amax(d1["X"]), H_given=hs[rows])
+    assert rel(npf(y)[rows], f["Y"]) <= TOL
