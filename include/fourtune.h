@@ -197,16 +197,14 @@ int ft_linear_bwd_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
 /* ---- sizes and diagnostics (host only, no CUDA calls) */
 size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout);
 size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t);
+/* Byte offset, inside the workspace handed to ft_linear_fwd / ft_linear_bwd_dgrad / ft_linear_bwd, of the
+ * pre-scaled low-rank intermediate Hs = bf16(H * fl(1 / alpha)) [M x r_t] that the quantize pass leaves for
+ * the GEMM (O-10'); valid from the call's completion until the next call that uses the
+ * workspace.  Exported so that the staged comparison of DESIGN.md O-11 can read the bits the GEMM consumed. */
+size_t ft_workspace_hs_offset(int64_t M, int32_t r_t);
 const char* ft_error_string(int status);
 int ft_last_cuda_error(void); /* cudaError_t / CUresult of the last FT_ERR_CUDA, thread-local */
 int ft_version(void);
-/* test / bench hook: 0 = default (CTA-pair 256x256 kernel); 128, 192, 256 = the 1-CTA kernel
- * with that N tile */
-int ft_debug_set_gemm_tile_n(int bn);
-/* test / bench hook: 0 = default (single-pass amax + quantize when the tensor fits), 1 = always
- * the two-pass path (k_amax, then the streaming quantize kernel) */
-int ft_debug_set_quantize_mode(int mode);
-
 #ifdef __cplusplus
 }
 #endif

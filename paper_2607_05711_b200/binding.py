@@ -62,6 +62,8 @@ def lib():
         L.ft_sf_bytes.restype = sz
         L.ft_workspace_bytes.argtypes = [i64, i64, i64, i32]
         L.ft_workspace_bytes.restype = sz
+        L.ft_workspace_hs_offset.argtypes = [i64, i32]
+        L.ft_workspace_hs_offset.restype = sz
         L.ft_error_string.argtypes = [C.c_int]
         L.ft_error_string.restype = C.c_char_p
         L.ft_debug_set_gemm_tile_n.argtypes = [C.c_int]
@@ -97,6 +99,13 @@ def ft_sf_bytes(rows, cols, block_rows, layout):
 
 def ft_workspace_bytes(M, K, N, r_t):
     return lib().ft_workspace_bytes(M, K, N, r_t)
+
+
+def workspace_hs(workspace, M, r_t):
+    """View of the pre-scaled low-rank intermediate Hs [M x r_t] (bf16) that the last ft_linear_* call left in
+    `workspace` (ft_workspace_hs_offset of the header): what the GEMM consumed, for the staged comparison O-11."""
+    off = lib().ft_workspace_hs_offset(M, r_t)
+    return workspace[off:off + M * r_t * 2].view(torch.bfloat16).view(M, r_t)
 
 
 class QTensor:
@@ -236,6 +245,7 @@ def ft_linear_bwd_q4(layer, qx, g, h_saved, dx, p_saved, dA, dBt, qg, workspace,
     return dx, dA, dBt
 
 
+# test / bench hooks of include/fourtune_debug.h (not part of the product interface)
 def debug_set_gemm_tile_n(bn):
     _check(lib().ft_debug_set_gemm_tile_n(bn))
 

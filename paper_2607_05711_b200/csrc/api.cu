@@ -4,6 +4,7 @@
 #include <cstring>
 
 #include "common.cuh"
+#include "../../include/fourtune_debug.h"
 
 namespace ft {
 
@@ -32,17 +33,23 @@ int launch_wgrad_q4(const uint8_t* codes, const uint8_t* sf, const float* g_dec,
                     cudaStream_t st);
 
 // ------------------------------------------------------------- device queries
-static int g_sm_count = 0;
+// SM count of the CURRENT device, cached per device ordinal (a process may drive several GPUs)
+int current_device() {
+  int dev = 0;
+  return cudaGetDevice(&dev) == cudaSuccess ? dev : 0;
+}
 int sm_count() {
-  if (g_sm_count == 0) {
-    int dev = 0, n = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
-      g_sm_count = n;
+  static int cached[FT_MAX_DEVICES] = {};   // 0 = not queried yet; racing writers store the same value
+  const int dev = current_device();
+  if (dev < 0 || dev >= FT_MAX_DEVICES) return 148;
+  if (cached[dev] == 0) {
+    int n = 0;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+      cached[dev] = n;
     else
       return 148;
   }
-  return g_sm_count;
+  return cached[dev];
 }
 
 bool pdl_enabled() {
@@ -68,9 +75,55 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 static PFN_encodeTiled g_encode = nullptr;
 
+// cuTensorMapEncodeTiled is a pure function of its arguments (the descriptor holds the base address, the
+// extents, the box and the swizzle: nothing device- or context-specific), and an eager step calls it ~25
+// times with the same arguments every step.  A small per-thread memo turns the repeats into a 128-byte copy.
+struct TmapKey {
+  const void* base;
+  uint64_t inner, outer, pitch;
+  uint32_t box_inner, box_outer;
+  int elem_bytes, sw;
+  bool operator==(const TmapKey& o) const {
+    return base == o.base && inner == o.inner && outer == o.outer && pitch == o.pitch && box_inner == o.box_inner &&
+           box_outer == o.box_outer && elem_bytes == o.elem_bytes && sw == o.sw;
+  }
+};
+constexpr int TMAP_CACHE = 64;   // direct-mapped
+struct TmapEntry {
+  TmapKey key;
+  CUtensorMap map;
+  bool valid;
+};
+static thread_local TmapEntry g_tmap_cache[TMAP_CACHE];
+
+static int encode_tensor_map_2d(CUtensorMap* map, const void* base, int elem_bytes, uint64_t inner,
+                                uint64_t outer, uint64_t row_pitch_bytes, uint32_t box_inner,
+                                uint32_t box_outer, Swizzle sw);
+
 int make_tensor_map_2d(CUtensorMap* map, const void* base, int elem_bytes, uint64_t inner,
                        uint64_t outer, uint64_t row_pitch_bytes, uint32_t box_inner,
                        uint32_t box_outer, Swizzle sw) {
+  const TmapKey key = {base, inner, outer, row_pitch_bytes, box_inner, box_outer, elem_bytes, (int)sw};
+  uint64_t h = reinterpret_cast<uintptr_t>(base) >> 4;
+  h = (h ^ (h >> 17) ^ (inner * 0x9E3779B97F4A7C15ull) ^ (outer << 7) ^ ((uint64_t)box_outer << 3) ^ box_inner) *
+      0xD6E8FEB86659FD93ull;
+  TmapEntry& e = g_tmap_cache[(h >> 32) % TMAP_CACHE];
+  if (e.valid && e.key == key) {
+    *map = e.map;
+    return FT_OK;
+  }
+  const int rc = encode_tensor_map_2d(map, base, elem_bytes, inner, outer, row_pitch_bytes, box_inner, box_outer, sw);
+  if (rc == FT_OK) {
+    e.key = key;
+    e.map = *map;
+    e.valid = true;
+  }
+  return rc;
+}
+
+static int encode_tensor_map_2d(CUtensorMap* map, const void* base, int elem_bytes, uint64_t inner,
+                                uint64_t outer, uint64_t row_pitch_bytes, uint32_t box_inner,
+                                uint32_t box_outer, Swizzle sw) {
   if (g_encode == nullptr) {
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
@@ -198,6 +251,11 @@ size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t) {
   (void)N;
   if (M < 0 || r_t < 0) return 0;
   return ws_layout(M, r_t).total;
+}
+
+size_t ft_workspace_hs_offset(int64_t M, int32_t r_t) {
+  if (M < 0 || r_t < 0) return 0;
+  return ws_layout(M, r_t).hs_off;
 }
 
 int ft_tensor_amax(const void* x_bf16, int64_t n, float* amax_out, void* stream) {

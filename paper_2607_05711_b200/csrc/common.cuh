@@ -34,7 +34,9 @@ int make_tensor_map_2d(CUtensorMap* map, const void* base, int elem_bytes, uint6
                        uint64_t outer, uint64_t row_pitch_bytes, uint32_t box_inner,
                        uint32_t box_outer, Swizzle sw);
 int device_check();  // FT_OK if the current device is sm_100-class
-int sm_count();
+constexpr int FT_MAX_DEVICES = 64;   // per-device host-side caches are arrays of this size
+int current_device();                // ordinal of the calling thread's current device
+int sm_count();                      // of the current device
 bool pdl_enabled();  // programmatic dependent launch of the GEMM and dA kernels (FT_PDL=0 turns it off)
 
 // Caller-provided workspace of one quantize (+ GEMM) pass over an [M x *] activation with a rank-r_t

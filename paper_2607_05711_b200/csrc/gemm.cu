@@ -13,6 +13,7 @@
 //   warp 2   : TMEM allocator
 //   warps 4-7: epilogue -- tcgen05.ld, * alpha, bf16, global store
 #include "common.cuh"
+#include "../../include/fourtune_debug.h"
 
 namespace ft {
 

@@ -213,9 +213,7 @@ int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* r
   FT_CUDA_TRY(cudaMemsetAsync(rn->sf, 0, ft_sf_bytes(K, N, 16, FT_SF_TILE128x4), st));
   if (rk_tiled != nullptr)
     FT_CUDA_TRY(cudaMemsetAsync(rk_tiled->sf, 0, ft_sf_bytes(N, K, 16, FT_SF_TILE128x4), st));
-  const int64_t threads = (N > K ? N : K) * ((N > K ? K : N) / 16) ;
   const int64_t tmax = (N * (K / 16) > K * (N / 16)) ? N * (K / 16) : K * (N / 16);
-  (void)threads;
   k_expand_sf<<<(unsigned)ceil_div(tmax, 256), 256, 0, st>>>(
       rk->sf, N, K, rk_tiled ? rk_tiled->sf : nullptr, rn->sf);
   FT_CUDA_TRY(cudaGetLastError());

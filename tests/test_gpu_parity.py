@@ -75,7 +75,11 @@ def qmode(request, B):
     B.debug_set_quantize_mode(0)
 
 
-@pytest.mark.parametrize("rows,cols,kind,layout", QCASES + [(2304, 3072, "x", 1), (4608, 3072, "g", 1)])
+# BASELINE.json configs[3] (C4): the four tensors of the quantizer sweep at full size
+C4_CASES = [(rows, cols, "x", 1) for rows, cols in synth.C4_SHAPES]
+
+
+@pytest.mark.parametrize("rows,cols,kind,layout", QCASES + [(2304, 3072, "x", 1), (4608, 3072, "g", 1)] + C4_CASES)
 def test_quantize_1x16_bit_exact(B, qmode, rows, cols, kind, layout):
     rng = synth.make_rng(rows * 131 + cols)
     x = synth.outlier_normal(rng, rows, cols) if kind == "x" else synth.student_t_grad(rng, rows, cols)
@@ -133,7 +137,8 @@ def test_weight_quantize_16x16_and_pack(B, N, K):
 
 @pytest.mark.parametrize("rows,cols,r_t,kind", [(128, 512, 16, "x"), (200, 1024, 64, "x"), (256, 3072, 48, "x"),
                                                 (384, 2048, 96, "g"), (130, 4096, 128, "g"), (1, 64, 32, "x"),
-                                                (2000, 128, 64, "x"), (4608, 3072, 64, "x"), (2304, 3072, 128, "g")])
+                                                (2000, 128, 64, "x"), (4608, 3072, 64, "x"), (2304, 3072, 128, "g")] +
+                         [(rows, cols, 32, "x") for rows, cols in synth.C4_SHAPES])
 def test_fused_projection(B, qmode, rows, cols, r_t, kind):
     rng = synth.make_rng(rows + cols + r_t)
     x = synth.outlier_normal(rng, rows, cols) if kind == "x" else synth.student_t_grad(rng, rows, cols)
@@ -198,6 +203,33 @@ def make_layer(B, seed, M, K, N, r_s, r, x_kind="outlier"):
     return d, R, D_f, U_f, L
 
 
+def range_finder_split(W, r_s, seed):
+    """Eq. 1 with a cheap rank-r_s subspace (one randomized range-finder pass instead of a full SVD): still
+    W = R + (L1 L2)^T up to the bf16 rounding of R, and any L1, L2 is a valid stabilizer for parity purposes (the
+    oracle and the CUDA path receive the same R, L1, L2).  float64 numpy, input preparation only."""
+    N, K = W.shape
+    if r_s == 0:
+        return W.astype(np.float32), np.zeros((K, 0), np.float32), np.zeros((0, N), np.float32)
+    rng = synth.make_rng(seed + 100)
+    W64 = W.astype(np.float64)
+    Qb, _ = np.linalg.qr(W64 @ rng.standard_normal((K, r_s)))        # N x r_s
+    L2 = nvfp4.bf16_round_from_f64(Qb.T)                              # r_s x N
+    L1 = nvfp4.bf16_round_from_f64((Qb.T @ W64).T)                    # K x r_s
+    R = nvfp4.bf16_round_from_f64(W64 - (L1.astype(np.float64) @ L2.astype(np.float64)).T)
+    return R, L1, L2
+
+
+def make_layer_fast(B, seed, M, K, N, r_s, r, x_kind="outlier"):
+    """make_layer with the range-finder split: for shapes where the full SVD of W would dominate the test."""
+    d = synth.layer_inputs(seed, M, K, N, max(r, 1), x_kind)
+    R, L1, L2 = range_finder_split(d["W"], r_s, seed)
+    D_f = np.concatenate([L1, d["A"][:, :r]], 1).astype(np.float32)
+    U_f = np.concatenate([L2, d["B"][:r, :]], 0).astype(np.float32)
+    r_t = r_s + r
+    L = B.Layer(t16(R), t16(D_f) if r_t else None, t16(U_f.T) if r_t else None, r_s, r)
+    return d, R, D_f, U_f, L
+
+
 def run_layer(B, L, X, G, M, K, N, r_t, r, fused_bwd=False):
     y = torch.zeros(M, N, dtype=torch.bfloat16, device="cuda")
     dx = torch.zeros(M, K, dtype=torch.bfloat16, device="cuda")
@@ -206,7 +238,7 @@ def run_layer(B, L, X, G, M, K, N, r_t, r, fused_bwd=False):
     ws = torch.zeros(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_t), dtype=torch.uint8, device="cuda")
     qx, qg = B.QTensor(M, K), B.QTensor(M, N)
     xt, gt = t16(X), t16(G)
-    scaled = lambda: (npf(ws[256:256 + M * r_t * 2].view(torch.bfloat16).reshape(M, r_t)) if r_t else None)
+    scaled = lambda: (npf(B.workspace_hs(ws, M, r_t)) if r_t else None)
     B.ft_linear_fwd(L, xt, y, h, qx, ws)
     torch.cuda.synchronize()
     hs = scaled()
@@ -263,6 +295,17 @@ def test_layer_fused_backward(B, qmode, seed, M, K, N, r_s, r):
     assert rel(out["dA"], ref["dA"]) < 1e-5 and rel(out["dBt"], ref["dBt"]) < 1e-5
 
 
+def elementwise_ok(got, want, absdot, what):
+    """Every element of a bf16 GEMM output against the oracle's (O-11): both sides are one bf16 rounding
+    of nearly the same real number, so they differ by at most one bf16 ulp (<= 2^-7 |want|) -- plus the fp32
+    accumulation error of the tensor core, which only shows on elements that cancel: 2^-20 of the sum of the
+    absolute products (sixteen fp32 ulps of headroom over the 2^-24 of a single rounding)."""
+    bound = np.abs(want) * 2.0 ** -7 + absdot * 2.0 ** -20
+    bad = np.abs(got.astype(np.float64) - want.astype(np.float64)) > bound
+    assert not bad.any(), "%s: %d of %d elements out of bound, first at %s" % (
+        what, int(bad.sum()), bad.size, np.argwhere(bad)[0])
+
+
 def check_layer(B, d, R, D_f, U_f, out, r_s, r, rows=None):
     """Full comparison, or on a row sample (rows) for sizes the oracle cannot finish whole."""
     X, G = d["X"], d["dY"]
@@ -282,13 +325,61 @@ def check_layer(B, d, R, D_f, U_f, out, r_s, r, rows=None):
         for got, want in ((out["h"][sel], f["H"]), (out["hs"][sel], f["Hs"]), (out["p"][sel], b["P"]),
                           (out["ps"][sel], b["Ps"])):
             assert rel(got, want) <= 2e-3 and (got == want).mean() >= 0.99
-    # (iii) outputs, both cast to bf16
+    # (iii) outputs, both cast to bf16: norm, identical fraction, and a bound on EVERY element
     assert rel(out["y"][sel], f["Y"]) <= TOL
     assert rel(out["dx"][sel], b["dX"]) <= TOL
     assert (out["y"][sel] == f["Y"]).mean() >= 0.95 and (out["dx"][sel] == b["dX"]).mean() >= 0.95
+    aR = np.abs(nvfp4.dequantize_unscaled(qR))
+    absdot_f = np.abs(nvfp4.dequantize_unscaled(f["qX"])) @ aR.T
+    absdot_b = np.abs(nvfp4.dequantize_unscaled(b["qG"])) @ aR
+    if r_t:
+        absdot_f += np.abs(out["hs"][sel].astype(np.float64)) @ np.abs(U_f.astype(np.float64))
+        absdot_b += np.abs(out["ps"][sel].astype(np.float64)) @ np.abs(D_f.astype(np.float64)).T
+    elementwise_ok(out["y"][sel], f["Y"], f["alpha"] * absdot_f, "Y")
+    elementwise_ok(out["dx"][sel], b["dX"], b["alpha"] * absdot_b, "dX")
     if r > 0 and rows is None:
         w = olayer.wgrad(X, G, out["h"], out["p"], r_s)
         assert rel(out["dA"], w["dA"]) <= TOL and rel(out["dBt"].T, w["dB"]) <= TOL
+
+
+# Shapes whose tile count exceeds 2 x 74 in one GEMM direction, so that every CTA pair of the persistent kernel
+# runs three or more tiles there -- both accumulators, the hand-over of the scale columns, the barrier phase wrap
+# -- with EVERY output element compared (the full-size cases below only sample rows).  Ragged M.
+MULTI_TILE_CASES = [   # seed, M, K, N, r_s, r
+    (71, 1100, 512, 7936, 32, 32),     # forward: 5 x 31 = 155 tiles of 256 x 256
+    (72, 1100, 7936, 512, 32, 64),     # dgrad:   155 tiles, 31 K stages forward
+    (73, 2304, 4352, 4352, 32, 64),    # 9 x 17 = 153 tiles in both directions, r_t = 96
+    (74, 1300, 320, 6400, 0, 16),      # 6 x 25 = 150 tiles, a partial K stage, one low-rank group of 16
+    (75, 2304, 4352, 4352, 0, 0),      # no low-rank stage at all
+]
+
+
+@pytest.mark.parametrize("seed,M,K,N,r_s,r", MULTI_TILE_CASES)
+def test_layer_multi_tile_per_cta_pair(B, seed, M, K, N, r_s, r):
+    d, R, D_f, U_f, L = make_layer_fast(B, seed, M, K, N, r_s, r)
+    out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=r > 0)
+    check_layer(B, d, R, D_f, U_f, out, r_s, r)
+
+
+def test_gemm4_alone_multi_tile(B):
+    """ft_gemm4 by itself (no low-rank term) on 150 tiles, every element against the oracle's float64 product of the
+    dequantized operands (pin P-5: r_s = r = 0 reduces the layer to a plain block-scaled GEMM)."""
+    M, K, N = 1500, 576, 6400
+    rng = synth.make_rng(76)
+    X = synth.outlier_normal(rng, M, K)
+    W = synth.normal(rng, (N, K), 0.02)
+    qx = B.QTensor(M, K)
+    B.ft_quantize_blockwise(t16(X), qx)
+    L = B.Layer(t16(W), None, None, 0, 0)
+    y = torch.zeros(M, N, dtype=torch.bfloat16, device="cuda")
+    B.ft_gemm4(qx, L.r_kmajor, None, None, y)
+    oX, oW = nvfp4.quantize_blockwise(X, 1), nvfp4.quantize_blockwise(W, 16)
+    alpha = np.float64(np.float32(oX["g_dec"]) * np.float32(oW["g_dec"]))
+    uX, uW = nvfp4.dequantize_unscaled(oX), nvfp4.dequantize_unscaled(oW)
+    want = nvfp4.bf16_round_from_f64(alpha * (uX @ uW.T))
+    got = npf(y)
+    assert rel(got, want) <= TOL and (got == want).mean() >= 0.95
+    elementwise_ok(got, want, alpha * (np.abs(uX) @ np.abs(uW).T), "Y")
 
 
 def test_layer_degenerate_branches(B):
@@ -436,43 +527,45 @@ def test_layer_full_size_sampled(B, name):
     _full_size_sampled(B, *synth.CONFIGS[name])
 
 
-@pytest.mark.parametrize("name", ["single.lin1", "single.lin2", "dual.txt.mlp_down", "dual.img.proj"])
+@pytest.mark.parametrize("name", [l[0] for l in synth.C5_LAYERS])
 def test_layer_c5_shapes_sampled(B, name):
-    """BASELINE.json configs[4]: the extreme shapes of the FLUX.1-dev-shaped layer list (widest N = 21504,
-    deepest K = 15360, the 512-token text stream, the square 4096-token projection), r_s = r = 32, seed 4,
-    same sampled comparison as above."""
+    """BASELINE.json configs[4]: ALL ten distinct (M, K, N) of the FLUX.1-dev-shaped layer list (the shapes bench.py
+    times and sums into the C5 figure), r_s = r = 32, seed 4, same sampled comparison as above."""
     _, _, M, K, N = next(l for l in synth.C5_LAYERS if l[0] == name)
     _full_size_sampled(B, 4, M, K, N, 32, 32, "outlier")
 
 
+def sample_rows(M):
+    """Rows of a full-size output to compare: in EVERY 256-row tile of the CTA-pair GEMM two rows from each 32-lane
+    quarter of each of the two CTAs (rows 3, 40, 77, 110 of the first CTA's 128, 131 - 128 = 3, 42, 72, 122 of the
+    second's: TMEM lane quarters 0, 1, 2, 3 = epilogue warps q = 0..3), plus the tile edges and the ragged end."""
+    rows = set()
+    for t in range((M + 255) // 256):
+        rows.update(t * 256 + o for o in (3, 40, 77, 110, 131, 170, 200, 250))
+    rows.update((0, 1, 127, 128, 129, 255, 256, M - 129, M - 2, M - 1))
+    return np.array(sorted(r for r in rows if 0 <= r < M))
+
+
 def _full_size_sampled(B, seed, M, K, N, r_s, r, kind):
     d = synth.layer_inputs(seed, M, K, N, r, kind)
-    rng = synth.make_rng(seed + 100)
-    W = d["W"].astype(np.float64)
-    Qb, _ = np.linalg.qr(W @ rng.standard_normal((K, r_s)))          # N x r_s
-    L2 = nvfp4.bf16_round_from_f64(Qb.T)                              # r_s x N
-    L1 = nvfp4.bf16_round_from_f64((Qb.T @ W).T)                      # K x r_s
-    R = nvfp4.bf16_round_from_f64(W - (L1.astype(np.float64) @ L2.astype(np.float64)).T)
+    R, L1, L2 = range_finder_split(d["W"], r_s, seed)
     D_f = np.concatenate([L1, d["A"]], 1).astype(np.float32)
     U_f = np.concatenate([L2, d["B"]], 0).astype(np.float32)
     L = B.Layer(t16(R), t16(D_f), t16(U_f.T), r_s, r)
     # the schedule bench.py times: ft_linear_fwd + ft_linear_bwd (C2, C3u: G is too large for the
     # single-pass quantizer -> dB^T pass with the amax of G first; C3d: G fits -> quantize, GEMM, one wgrad)
     out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=True)
-    rows = np.array(sorted({0, 1, 127, 128, 129, 1000 % M, 2047 % M, 2048 % M, 3333 % M, M - 129, M - 2, M - 1}))
-    check_layer(B, d, R, D_f, U_f, out, r_s, r, rows=rows)
-    # wgrad on sampled output rows: dA[k, :] = X[:, k]^T P_lora, dB[:, n] = H_lora^T G[:, n]
-    ks = np.array([0, 1, 63, 64, 777, K - 1]); ns = np.array([0, 5, 127, 128, 2000, N - 1])
-    Pl = out["p"][:, r_s:].astype(np.float64); Hl = out["h"][:, r_s:].astype(np.float64)
-    assert rel(out["dA"][ks], d["X"][:, ks].astype(np.float64).T @ Pl) <= TOL
-    assert rel(out["dBt"][ns], d["dY"][:, ns].astype(np.float64).T @ Hl) <= TOL
-    # the same with 4-bit saved activations (NEXT-2): dA[k, :] = dequant(Q(X))[:, k]^T P_lora
+    check_layer(B, d, R, D_f, U_f, out, r_s, r, rows=sample_rows(M))
+    # wgrad in full (Eq. 4 is two skinny products: the oracle finishes them at any of these sizes)
+    w = olayer.wgrad(d["X"], d["dY"], out["h"], out["p"], r_s)
+    assert rel(out["dA"], w["dA"]) <= TOL and rel(out["dBt"].T, w["dB"]) <= TOL
+    # the same with 4-bit saved activations (NEXT-2): dA = dequant(Q(X))^T P_lora
     dA4 = torch.zeros(K, r, dtype=torch.float32, device="cuda"); dBt4 = torch.zeros(N, r, dtype=torch.float32, device="cuda")
     B.ft_lora_wgrad_q4(L, out["qx"], out["gt"], out["ht"], out["pt"], dA4, dBt4)
     torch.cuda.synchronize()
-    Xq = nvfp4.dequantize(nvfp4.quantize_blockwise(d["X"], 1))
-    assert rel(dA4.cpu().numpy()[ks], Xq[:, ks].T @ Pl) <= 1e-5
-    assert rel(dBt4.cpu().numpy()[ns], d["dY"][:, ns].astype(np.float64).T @ Hl) <= TOL
+    w4 = olayer.wgrad_saved4(nvfp4.quantize_blockwise(d["X"], 1), d["dY"], out["h"], out["p"], r_s)
+    assert rel(dA4.cpu().numpy(), w4["dA"]) <= 1e-5
+    assert rel(dBt4.cpu().numpy().T, w4["dB"]) <= TOL
 
 
 def test_without_programmatic_launch():
@@ -547,6 +640,6 @@ def test_back_to_back_steps_without_sync(B):
     torch.cuda.synchronize()
     B.ft_linear_fwd(L, xs[0], y, h, qx, ws)
     torch.cuda.synchronize()
-    hs = npf(ws[256:256 + M * r_t * 2].view(torch.bfloat16).reshape(M, r_t))
+    hs = npf(B.workspace_hs(ws, M, r_t))
     f = olayer.forward(d1["X"][rows], qR, D_f, U_f, prescale=True, x_amax=nvfp4.tensor_amax(d1["X"]), H_given=hs[rows])
     assert rel(npf(y)[rows], f["Y"]) <= TOL
