@@ -175,7 +175,7 @@ def run_ours(args):
     dx = torch.empty(M, K, dtype=torch.bfloat16, device=dev)
     h = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
     p = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
-    ws = torch.empty(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_t), dtype=torch.uint8, device=dev)
+    ws = B.new_workspace(M, max(K, N), max(K, N), r_t, dev)
     qx, qg = B.QTensor(M, K, device=dev), B.QTensor(M, N, device=dev)
     dA = torch.empty(K, r, dtype=torch.float32, device=dev)
     dBt = torch.empty(N, r, dtype=torch.float32, device=dev)
@@ -187,9 +187,9 @@ def run_ours(args):
         if world > 1:
             parallel.allreduce_lora_grads(dA, dBt)
     # fwd: k_quantize_fused (single pass, amax inside) + k_gemm4_pair; bwd (ft_linear_bwd): k_wgrad (dB^T + amax
-    # of G) + k_quantize_fused (streaming) + k_finalize_h + k_gemm4_pair + k_wgrad (dA)
-    # plus the two k_clear2 launches (control words; the backward's also clears dB^T): 9 kernels, no memset node
-    KERNELS_PER_STEP = 9
+    # of G) + k_quantize_fused (streaming, row sums inside) + k_gemm4_pair + k_wgrad (dA): 6 kernels, no clear
+    # kernel and no memset node (the workspace's control words are put back by the kernels that use them)
+    KERNELS_PER_STEP = 6
 
     def barrier():
         if world > 1:
@@ -464,7 +464,7 @@ def sweep(B, prepare, dev, timed, peaks, full=False):
     for rows, cols in ((4608, 3072), (4608, 12288), (4608, 15360), (9216, 3072)):
         x = acts(rows, cols)
         q = B.QTensor(rows, cols, device=dev)
-        ws = torch.empty(B.ft_workspace_bytes(rows, cols, 0, 32), dtype=torch.uint8, device=dev)
+        ws = B.new_workspace(rows, cols, 0, 32, dev)
         amax = B.ft_tensor_amax(x)
         d = (torch.randn(cols, 32, device=dev, generator=g) * 0.01).to(torch.bfloat16)
         h = torch.empty(rows, 32, dtype=torch.bfloat16, device=dev)
@@ -497,7 +497,7 @@ def sweep(B, prepare, dev, timed, peaks, full=False):
         dx = torch.empty(M, K, dtype=torch.bfloat16, device=dev)
         h = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
         p = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
-        ws = torch.empty(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_t), dtype=torch.uint8, device=dev)
+        ws = B.new_workspace(M, max(K, N), max(K, N), r_t, dev)
         qx, qg = B.QTensor(M, K, device=dev), B.QTensor(M, N, device=dev)
         dA = torch.empty(K, r, dtype=torch.float32, device=dev)
         dBt = torch.empty(N, r, dtype=torch.float32, device=dev)
@@ -587,7 +587,7 @@ def fusion_ablation(B, dev, acts, g):
     dx = torch.empty(M, K, dtype=torch.bfloat16, device=dev)
     h = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
     p = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
-    ws = torch.empty(B.ft_workspace_bytes(M, max(K, N), max(K, N), r_t), dtype=torch.uint8, device=dev)
+    ws = B.new_workspace(M, max(K, N), max(K, N), r_t, dev)
     qx, qg = B.QTensor(M, K, device=dev), B.QTensor(M, N, device=dev)
     dA = torch.empty(K, r, dtype=torch.float32, device=dev)
     dBt = torch.empty(N, r, dtype=torch.float32, device=dev)

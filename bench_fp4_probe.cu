@@ -1,13 +1,19 @@
-// probe_fp4_peak.cu -- measurement only: the rate of tcgen05.mma.cta_group::2.kind::mxf4nvf4
-// .block_scale (M=256, N=256, K=64) with operands fixed in shared memory, the accumulator in TMEM and
-// nothing else in the loop (no TMA, no epilogue); optionally with the 12 tcgen05.cp scale copies the
-// GEMM issues per K=256 stage.  Stand-alone executable: `python -m paper_2607_05711_b200.probe`.
-// On the B200 of this round: exactly 128.0 cycles per MMA in every variant (one CTA pair or all 74),
-// 8.3-8.4 PFLOP/s chip-wide by CUDA events over a 1.2 ms burst.
+// bench_fp4_probe.cu -- measurement only, built and run by bench.py: the rate of
+// tcgen05.mma.cta_group::2.kind::mxf4nvf4.block_scale (M=256, N=256, K=64) with operands fixed in shared memory,
+// the accumulator in TMEM and nothing else in the loop (no TMA, no epilogue); optionally with the 12 tcgen05.cp
+// scale copies the GEMM issues per K=256 stage.  Not part of the library (it only borrows the PTX wrappers of
+// paper_2607_05711_b200/csrc/common.cuh).
+//   bench_fp4_probe [iterations]            the round-1 table: 1 / 4 operand stages x with / without scale copies
+//   bench_fp4_probe --sustained SECONDS     all CTA pairs, 4 stages, scale copies on, back-to-back launches for
+//                                           SECONDS; prints one line "sustained ... TFLOP/s" (the FP4 ceiling
+//                                           under the power cap, next to which bench.py samples the SM clock)
+// Round 1 on B200: exactly 128.0 cycles per MMA in every variant, 8.3-8.4 PFLOP/s chip-wide over a 1.2 ms burst.
 #include <cstdio>
 #include <cstdlib>
 #include <vector>
-#include "common.cuh"
+#include <cstring>
+#include <chrono>
+#include "paper_2607_05711_b200/csrc/common.cuh"
 using namespace ft;
 thread_local int ft::g_last_cuda_error = 0;
 
@@ -79,11 +85,40 @@ k_probe(int iters, int mode, int nstages, long long* out) {
 }
 
 int main(int argc, char** argv) {
-  const int iters = argc > 1 ? atoi(argv[1]) : 2000;
   int nsm = 0;
   cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
   long long* d;
   cudaMalloc(&d, 1024 * 8);
+  if (argc > 2 && strcmp(argv[1], "--sustained") == 0) {
+    const double seconds = atof(argv[2]);
+    const int nstages = 4, mode = 1, iters = 20000;   // ~5 ms per launch
+    const int smem = nstages * STAGE + 1024;
+    cudaFuncSetAttribute(k_probe, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaMemset(d, 0, 1024 * 8);
+    k_probe<<<nsm, 128, smem>>>(iters, mode, nstages, d);   // warm
+    cudaDeviceSynchronize();
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const auto t0 = std::chrono::steady_clock::now();
+    long launches = 0;
+    cudaEventRecord(e0);
+    do {
+      for (int i = 0; i < 8; ++i) k_probe<<<nsm, 128, smem>>>(iters, mode, nstages, d);
+      launches += 8;
+      cudaStreamSynchronize(0);
+    } while (std::chrono::duration<double>(std::chrono::steady_clock::now() - t0).count() < seconds);
+    cudaEventRecord(e1);
+    cudaError_t e = cudaDeviceSynchronize();
+    float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+    std::vector<long long> h(nsm / 2);
+    cudaMemcpy(h.data(), d, nsm / 2 * 8, cudaMemcpyDeviceToHost);
+    double cyc = 0; for (auto v : h) cyc += (double)v; cyc /= (nsm / 2);
+    const double flop = 2.0 * 256 * 256 * 64 * 4.0 * iters * (nsm / 2) * launches;
+    printf("sustained %s %.3f s %ld launches: %.1f cycles per MMA (last launch), %.0f TFLOP/s\n", cudaGetErrorString(e),
+           ms * 1e-3, launches, cyc / (4.0 * iters), flop / (ms * 1e-3) / 1e12);
+    return e == cudaSuccess ? 0 : 1;
+  }
+  const int iters = argc > 1 ? atoi(argv[1]) : 2000;
   for (int nstages : {1, 4})
     for (int mode : {0, 1}) {
       const int smem = nstages * STAGE + 1024;

@@ -24,7 +24,11 @@
  *  - all data pointers are DEVICE pointers unless the comment says "host";
  *    the structs themselves are host memory, read during the call only.
  *  - the caller owns every buffer; the library never allocates, frees or keeps
- *    a pointer after the call returns.  Scratch comes from `workspace`.
+ *    a pointer after the call returns.  Scratch comes from `workspace`, a device buffer of at least
+ *    ft_workspace_bytes() bytes whose first 4 KB hold control words that must be ZERO when a call starts:
+ *    zero-fill the buffer once (or call ft_workspace_init); every call leaves them zero again (the kernels
+ *    put each word back when they are done with it), so no clearing runs per call.  One workspace serves any
+ *    number of stream-ordered calls of any shapes, but not two calls that run concurrently.
  *  - `stream` is a cudaStream_t passed as void*; all work is enqueued on it and
  *    the call returns without synchronising.  No device scalar is read by the
  *    host (tensor scales stay on the device).
@@ -73,6 +77,15 @@ typedef struct {
   int64_t rows, cols;
   int32_t block_rows;      /* 1 (activations, gradients) or 16 (weights, 16x16 blocks)  */
   int32_t sf_layout;       /* FT_SF_ROWMAJOR or FT_SF_TILE128x4                          */
+  /* optional, weights only (NULL / 0 otherwise): the same scales once more, cut to the GEMM's output-tile
+   * width `ntile` (224): for row tile nt = row / ntile and K=64 step ks two 512-byte groups -- rows
+   * nt*ntile + 0..127 and + 128..ntile-1 of the tile, each in the (r%32)*16 + (r/32)*4 + c%4 order of
+   * FT_SF_TILE128x4, rows past the tile or the tensor zero -- at ((nt * cols/64 + ks) * 2 + half) * 512.
+   * ft_sf_ntile_bytes() bytes, filled by ft_pack_weight.  With it ft_gemm4 / ft_linear_* may run 256 x ntile
+   * tiles, whose block scales have tensor-memory columns of their own. */
+  uint8_t* sf_ntile;
+  int32_t ntile;
+  int32_t reserved_;
 } ft_qtensor;
 
 /* Optional low-rank down-projection fused into the quantize pass (PAPER.md:110,
@@ -125,7 +138,8 @@ int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols,
  * Outputs: r_nmajor (codes [K x N/2], sf TILE128x4 over K rows, same tensor scale
  * value copied), and, if r_kmajor_tiled != NULL, the TILE128x4 expansion of the
  * forward operand's scales (its codes/tensor_dec_scale pointers are not written;
- * point them at r_kmajor's buffers). N % 64 == 0 and K % 64 == 0. */
+ * point them at r_kmajor's buffers).  For each of the two outputs whose sf_ntile is non-NULL and whose ntile
+ * is 224, the tile-cut copy of the scales as well.  N % 64 == 0 and K % 64 == 0. */
 int ft_pack_weight(const ft_qtensor* r_kmajor, ft_qtensor* r_kmajor_tiled,
                    ft_qtensor* r_nmajor, void* stream);
 
@@ -158,8 +172,9 @@ int ft_gemm4(const ft_qtensor* a, const ft_qtensor* b, const void* lr_a_scaled, 
 /* ---- a5: LoRA weight gradients (Eq. 4), fp32.
  * dA  [K x r]  = X^T  * P[:, r_s:]      dBt [N x r] = G^T * H[:, r_s:]  (= dB^T)
  * h_saved / p_saved are the [M x r_t] outputs of the two calls above.
- * accumulate: 0 overwrite, 1 add to the existing contents.  Sums over M are
- * accumulated with fp32 atomics: the order of additions is not fixed. */
+ * accumulate: 0 overwrite, 1 add to the existing contents.  This call has no workspace: partial sums over
+ * slices of M are combined with fp32 atomics, so the order of additions is not fixed (ft_linear_bwd combines
+ * them through its workspace in a fixed order instead). */
 int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
                   const void* h_saved_bf16, const void* p_saved_bf16, float* dA,
                   float* dBt, int32_t accumulate, void* stream);
@@ -181,7 +196,8 @@ int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
  * Same results as ft_linear_bwd_dgrad followed by ft_lora_wgrad, different schedule: the pass
  * over G that computes dBt = G^T (X A) also finds max |G|, so the separate amax pass of the
  * quantizer disappears (G is read twice instead of three times); dA = X^T (G B^T) runs last
- * because it needs P.  Arguments as in the two calls above. */
+ * because it needs P.  The partial sums of dA and dBt over slices of M go through the workspace and are added
+ * in a fixed order: the same bits on every run, no clear kernel.  Arguments as in the two calls above. */
 int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
                   const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
                   int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
@@ -196,7 +212,12 @@ int ft_linear_bwd_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
 
 /* ---- sizes and diagnostics (host only, no CUDA calls) */
 size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout);
+size_t ft_sf_ntile_bytes(int64_t rows, int64_t cols, int32_t ntile);   /* ft_qtensor::sf_ntile */
 size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t);
+/* Zero the control words at the head of a workspace (one 4 KB memset on `stream`).  Needed once per buffer,
+ * before its first use, unless the caller zero-filled it; never per call.  Also the way to recover a workspace
+ * after a call was aborted by a CUDA error. */
+int ft_workspace_init(void* workspace, size_t workspace_bytes, void* stream);
 /* Byte offset, inside the workspace handed to ft_linear_fwd / ft_linear_bwd_dgrad / ft_linear_bwd, of the
  * pre-scaled low-rank intermediate Hs = bf16(H * fl(1 / alpha)) [M x r_t] that the quantize pass leaves for
  * the GEMM (O-10'); valid from the call's completion until the next call that uses the

@@ -23,7 +23,8 @@ class FtError(RuntimeError):
 
 class _QT(C.Structure):
     _fields_ = [("codes", C.c_void_p), ("sf", C.c_void_p), ("tensor_dec_scale", C.c_void_p),
-                ("rows", C.c_int64), ("cols", C.c_int64), ("block_rows", C.c_int32), ("sf_layout", C.c_int32)]
+                ("rows", C.c_int64), ("cols", C.c_int64), ("block_rows", C.c_int32), ("sf_layout", C.c_int32),
+                ("sf_ntile", C.c_void_p), ("ntile", C.c_int32), ("reserved_", C.c_int32)]
 
 
 class _Proj(C.Structure):
@@ -60,8 +61,11 @@ def lib():
         L.ft_linear_bwd_q4.argtypes = [C.POINTER(_Layer), C.POINTER(_QT), vp, i64, vp, vp, vp, vp, vp, i32, C.POINTER(_QT), vp, sz, vp]
         L.ft_sf_bytes.argtypes = [i64, i64, i32, i32]
         L.ft_sf_bytes.restype = sz
+        L.ft_sf_ntile_bytes.argtypes = [i64, i64, i32]
+        L.ft_sf_ntile_bytes.restype = sz
         L.ft_workspace_bytes.argtypes = [i64, i64, i64, i32]
         L.ft_workspace_bytes.restype = sz
+        L.ft_workspace_init.argtypes = [vp, sz, vp]
         L.ft_workspace_hs_offset.argtypes = [i64, i32]
         L.ft_workspace_hs_offset.restype = sz
         L.ft_error_string.argtypes = [C.c_int]
@@ -101,6 +105,18 @@ def ft_workspace_bytes(M, K, N, r_t):
     return lib().ft_workspace_bytes(M, K, N, r_t)
 
 
+def ft_workspace_init(workspace, stream=None):
+    """Zero the control words at the head of a workspace (once per buffer; torch.zeros does the same)."""
+    _check(lib().ft_workspace_init(_ptr(workspace), workspace.numel(), _stream(stream)))
+    return workspace
+
+
+def new_workspace(M, K, N, r_t, device="cuda"):
+    """A workspace for one layer, control words initialised."""
+    ws = torch.empty(ft_workspace_bytes(M, K, N, r_t), dtype=torch.uint8, device=device)
+    return ft_workspace_init(ws)
+
+
 def workspace_hs(workspace, M, r_t):
     """View of the pre-scaled low-rank intermediate Hs [M x r_t] (bf16) that the last ft_linear_* call left in
     `workspace` (ft_workspace_hs_offset of the header): what the GEMM consumed, for the staged comparison O-11."""
@@ -116,10 +132,18 @@ class QTensor:
         self.codes = torch.empty((rows, cols // 2), dtype=torch.uint8, device=device)
         self.sf = torch.zeros(ft_sf_bytes(rows, cols, block_rows, sf_layout), dtype=torch.uint8, device=device)
         self.tensor_dec_scale = torch.zeros(1, dtype=torch.float32, device=device)
+        self.sf_ntile, self.ntile = None, 0      # weights only: scales cut to the GEMM's tile width
+
+    def with_ntile(self, ntile=224):
+        self.ntile = ntile
+        self.sf_ntile = torch.zeros(lib().ft_sf_ntile_bytes(self.rows, self.cols, ntile), dtype=torch.uint8,
+                                    device=self.codes.device)
+        return self
 
     def c(self):
         return _QT(self.codes.data_ptr(), self.sf.data_ptr(), self.tensor_dec_scale.data_ptr(),
-                   self.rows, self.cols, self.block_rows, self.sf_layout)
+                   self.rows, self.cols, self.block_rows, self.sf_layout,
+                   None if self.sf_ntile is None else self.sf_ntile.data_ptr(), self.ntile, 0)
 
     def sync_from(self, q):
         self.rows, self.cols, self.block_rows, self.sf_layout = q.rows, q.cols, q.block_rows, q.sf_layout
@@ -138,8 +162,7 @@ def ft_quantize_blockwise(x, out, tensor_amax=None, down=None, h_out=None, hs_ou
     _bf16(x)
     rows, cols = x.shape
     if workspace is None:
-        workspace = torch.empty(ft_workspace_bytes(rows, cols, 0, 0 if down is None else down.shape[1]),
-                                dtype=torch.uint8, device=x.device)
+        workspace = new_workspace(rows, cols, 0, 0 if down is None else down.shape[1], x.device)
     proj = None
     if down is not None:
         _bf16(down)
@@ -169,10 +192,10 @@ class Layer:
         # a6: offline quantize (16x16 blocks, row-major S) then re-pack both orientations
         self.q_rowmajor = QTensor(N, K, 16, FT_SF_ROWMAJOR, dev)
         ft_quantize_blockwise(R_bf16, self.q_rowmajor, stream=stream)
-        self.r_kmajor = QTensor(N, K, 16, FT_SF_TILE128x4, dev)
+        self.r_kmajor = QTensor(N, K, 16, FT_SF_TILE128x4, dev).with_ntile(224)
         self.r_kmajor.codes = self.q_rowmajor.codes
         self.r_kmajor.tensor_dec_scale = self.q_rowmajor.tensor_dec_scale
-        self.r_nmajor = QTensor(K, N, 16, FT_SF_TILE128x4, dev)
+        self.r_nmajor = QTensor(K, N, 16, FT_SF_TILE128x4, dev).with_ntile(224)
         qk, qkt, qn = self.q_rowmajor.c(), self.r_kmajor.c(), self.r_nmajor.c()
         _check(lib().ft_pack_weight(C.byref(qk), C.byref(qkt), C.byref(qn), _stream(stream)))
 

@@ -11,13 +11,13 @@ namespace ft {
 thread_local int g_last_cuda_error = 0;
 
 // kernels' host launchers (quantize.cu, quantize_fused.cu, gemm.cu, wgrad.cu)
-int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first);
+int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first, bool pdl);
 void set_quantize_mode(int mode);
 bool quantize_single_pass_fits(int64_t rows, int64_t cols, int r_t);
 int launch_quantize_generic(const void* x, int64_t rows, int64_t cols, const float* amax_t,
                             ft_qtensor* out, cudaStream_t st);
 int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t,
-                          const ft_proj* proj, ft_qtensor* out, void* workspace, bool zero_region_cleared,
+                          const ft_proj* proj, ft_qtensor* out, void* workspace, bool after_kernel,
                           bool* finalize_last, cudaStream_t st);
 int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, cudaStream_t st);
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
@@ -25,8 +25,7 @@ int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N,
                  cudaStream_t st);
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, bool beside_prev,
-                 cudaStream_t st);
+                 unsigned int* amax_g, bool after_kernel, bool beside_prev, cudaStream_t st);
 int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t st);
 int launch_wgrad_q4(const uint8_t* codes, const uint8_t* sf, const float* g_dec, int64_t M, int64_t K,
                     const void* p_saved, int r_t, int r_s, int r, float* dA, int accumulate, bool beside_prev,
@@ -159,12 +158,12 @@ static bool valid_rt(int r_t) { return r_t >= 0 && r_t <= 128 && r_t % 16 == 0; 
 
 // one direction of the layer: quantize `act` [M x Kd] (+ projection by lr_down
 // [Kd x r_t]) and multiply with the weight operand `w` ([Nd x Kd]); lr_up [Nd x r_t].
-// act_amax: device float with max |act| if the caller already has it (the fused backward, which has
-// also cleared the workspace's zero region), else NULL.
+// act_amax: device float with max |act| if the caller already has it (the fused backward), else NULL.
+// after_kernel: a kernel of the same call directly precedes the first launch.
 static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_up, int r_t,
                        const void* act, int64_t M, int64_t Kd, int64_t Nd, void* out,
                        void* saved, ft_qtensor* q, void* workspace, size_t ws_bytes,
-                       const float* act_amax, cudaStream_t st) {
+                       const float* act_amax, bool after_kernel, cudaStream_t st) {
   if (!act || !out || !q || !q->codes || !q->sf || !q->tensor_dec_scale || !workspace)
     return FT_ERR_INVALID_ARG;
   if (r_t > 0 && (!saved || !lr_down || !lr_up)) return FT_ERR_INVALID_ARG;
@@ -180,6 +179,8 @@ static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_
   q->cols = Kd;
   q->block_rows = 1;
   q->sf_layout = FT_SF_TILE128x4;
+  q->sf_ntile = nullptr;
+  q->ntile = 0;
   ft_proj pr;
   pr.down = lr_down;
   pr.out = saved;
@@ -188,10 +189,12 @@ static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_
   pr.r_t = r_t;
   // a0 + a1/a3: the tensor amax is found inside the quantize pass when the tensor fits the SMs'
   // shared memory (single pass), by a preceding k_amax launch otherwise
-  bool finalize_last = false;   // streaming route: k_finalize_h (which writes only H and Hs) is the last launch
-  rc = launch_quantize_fused(act, M, Kd, act_amax, r_t > 0 ? &pr : nullptr, q, workspace, act_amax != nullptr,
+  bool finalize_last = false;   // k_finalize_h (which writes only H and Hs) is the last launch of the quantize step
+  rc = launch_quantize_fused(act, M, Kd, act_amax, r_t > 0 ? &pr : nullptr, q, workspace, after_kernel,
                              &finalize_last, st);
   if (rc != FT_OK) return rc;
+  // lr_late invariant (gemm_pair.cu): the GEMM launch directly follows k_finalize_h of THIS call -- nothing may be
+  // enqueued between the two lines above and below
   return launch_gemm4(q, w, M, Nd, Kd, r_t > 0 ? hs : nullptr, lr_up, r_t, out, finalize_last, st);
 }
 
@@ -246,11 +249,23 @@ size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layou
   return (size_t)(ceil_div(rows, block_rows) * nblk);
 }
 
+size_t ft_sf_ntile_bytes(int64_t rows, int64_t cols, int32_t ntile) {
+  if (rows <= 0 || cols <= 0 || ntile <= 0) return 0;
+  return (size_t)(ceil_div(rows, ntile) * ceil_div(cols, 64) * 1024);
+}
+
 size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t) {
   (void)K;
   (void)N;
   if (M < 0 || r_t < 0) return 0;
   return ws_layout(M, r_t).total;
+}
+
+int ft_workspace_init(void* workspace, size_t workspace_bytes, void* stream) {
+  if (!workspace || !aligned16(workspace)) return FT_ERR_INVALID_ARG;
+  if (workspace_bytes < WS_CTL_BYTES) return FT_ERR_WORKSPACE_TOO_SMALL;
+  FT_CUDA_TRY(cudaMemsetAsync(workspace, 0, WS_CTL_BYTES, (cudaStream_t)stream));
+  return FT_OK;
 }
 
 size_t ft_workspace_hs_offset(int64_t M, int32_t r_t) {
@@ -260,7 +275,7 @@ size_t ft_workspace_hs_offset(int64_t M, int32_t r_t) {
 
 int ft_tensor_amax(const void* x_bf16, int64_t n, float* amax_out, void* stream) {
   if (!x_bf16 || !amax_out || n < 0 || !aligned16(x_bf16)) return FT_ERR_INVALID_ARG;
-  return launch_amax(x_bf16, n, amax_out, (cudaStream_t)stream, true);
+  return launch_amax(x_bf16, n, amax_out, (cudaStream_t)stream, true, false);
 }
 
 int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols, const float* tensor_amax,
@@ -293,16 +308,18 @@ int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols, const 
     if (workspace_bytes < ft_workspace_bytes(rows, cols, 0, r_t)) return FT_ERR_WORKSPACE_TOO_SMALL;
   }
   if (out->block_rows == 16) {
+    // offline path (a6): the amax goes to a scratch word of the workspace behind the control words (memset
+    // + k_amax: launch count does not matter here)
     const float* amax = tensor_amax;
     if (!amax) {
-      float* a = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + ws_layout(rows, r_t).amax_off);
-      rc = launch_amax(x_bf16, rows * cols, a, st, true);
+      float* a = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + ws_layout(rows, r_t).hs_off);
+      rc = launch_amax(x_bf16, rows * cols, a, st, true, false);
       if (rc != FT_OK) return rc;
       amax = a;
     }
     return launch_quantize_generic(x_bf16, rows, cols, amax, out, st);
   }
-  return launch_quantize_fused(x_bf16, rows, cols, tensor_amax, proj, out, workspace, false, nullptr, st);
+  return launch_quantize_fused(x_bf16, rows, cols, tensor_amax, proj, out, workspace, pdl_enabled(), nullptr, st);
 }
 
 int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, void* stream) {
@@ -311,6 +328,10 @@ int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, v
     return FT_ERR_INVALID_ARG;
   if (rk->block_rows != 16 || rk->sf_layout != FT_SF_ROWMAJOR) return FT_ERR_INVALID_ARG;
   if (rk_tiled && !rk_tiled->sf) return FT_ERR_INVALID_ARG;
+  const ft_qtensor* outs[2] = {rk_tiled, rn};
+  for (int i = 0; i < 2; ++i)
+    if (outs[i] && outs[i]->sf_ntile != nullptr && (outs[i]->ntile != 224 || !aligned16(outs[i]->sf_ntile)))
+      return FT_ERR_INVALID_ARG;
   if (rk->rows % 64 != 0 || rk->cols % 64 != 0 || rk->rows < 64 || rk->cols < 64)
     return FT_ERR_UNSUPPORTED_SHAPE;
   int rc = device_check();
@@ -353,7 +374,7 @@ int ft_linear_fwd(const ft_layer* L, const void* x_bf16, int64_t M, void* y_bf16
   int rc = check_layer(L);
   if (rc != FT_OK) return rc;
   return linear_pass(&L->r_kmajor, L->D_f, L->U_t, L->r_s + L->r, x_bf16, M, L->K, L->N, y_bf16,
-                     h_saved_bf16, qx_scratch, workspace, workspace_bytes, nullptr, (cudaStream_t)stream);
+                     h_saved_bf16, qx_scratch, workspace, workspace_bytes, nullptr, pdl_enabled(), (cudaStream_t)stream);
 }
 
 int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* dx_bf16,
@@ -362,7 +383,7 @@ int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* 
   int rc = check_layer(L);
   if (rc != FT_OK) return rc;
   return linear_pass(&L->r_nmajor, L->U_t, L->D_f, L->r_s + L->r, g_bf16, M, L->N, L->K, dx_bf16,
-                     p_saved_bf16, qg_scratch, workspace, workspace_bytes, nullptr, (cudaStream_t)stream);
+                     p_saved_bf16, qg_scratch, workspace, workspace_bytes, nullptr, pdl_enabled(), (cudaStream_t)stream);
 }
 
 static int check_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M, const void* h_saved_bf16,
@@ -384,7 +405,7 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   int rc = check_wgrad(L, x_bf16, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt);
   if (rc != FT_OK) return rc;
   return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, L->r_s + L->r, L->r_s, L->r, dA,
-                      dBt, accumulate, nullptr, nullptr, 0, false, false, (cudaStream_t)stream);
+                      dBt, accumulate, nullptr, pdl_enabled(), false, (cudaStream_t)stream);
 }
 
 int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16, int64_t M,
@@ -398,20 +419,19 @@ int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
     return FT_ERR_INVALID_ARG;
   cudaStream_t st = (cudaStream_t)stream;
   const int r_t = L->r_s + L->r;
-  // one clear for both gradients, then dB^T (it never reads X: the bf16 kernel, problem 2 only) and dA
-  // from the codes, both accumulating, both behind programmatic edges; the dA kernel does not wait for the
-  // dB^T kernel (they share nothing) and takes over the SMs as its CTAs retire
-  bool chained = false;
+  // dB^T (it never reads X: the bf16 kernel, problem 2 only, M slices combined inside the kernel), then dA from
+  // the codes, whose M slices combine with fp32 reductions into a cleared (or accumulating) buffer
+  bool chained = pdl_enabled();
   if (!accumulate) {
-    rc = launch_clear2(dA, (size_t)L->K * L->r * sizeof(float), dBt, (size_t)L->N * L->r * sizeof(float), st);
+    rc = launch_clear2(dA, (size_t)L->K * L->r * sizeof(float), nullptr, 0, st);
     if (rc != FT_OK) return rc;
     chained = true;
   }
   rc = launch_wgrad(2, nullptr, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                    1, nullptr, nullptr, 0, chained, false, st);
+                    accumulate, nullptr, chained, false, st);
   if (rc != FT_OK) return rc;
   return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA,
-                         1, chained, st);
+                         1, false, st);
 }
 
 // the whole backward; qx != NULL: dA from the saved 4-bit activations (x_bf16 unused)
@@ -434,41 +454,47 @@ static int linear_bwd(const ft_layer* L, const void* x_bf16, const ft_qtensor* q
   if (!workspace || !aligned16(workspace)) return FT_ERR_INVALID_ARG;
   if (workspace_bytes < ft_workspace_bytes(M, L->N, L->K, L->r_s + L->r)) return FT_ERR_WORKSPACE_TOO_SMALL;
   const int r_t = L->r_s + L->r;
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  bool chained = pdl_enabled();   // the first kernel of the call may carry a programmatic edge (it waits at its top)
+  // dA from the saved codes goes through fp32 reductions (k_wgrad_q4 has no slot path): clear it up front
+  if (qx != nullptr && !accumulate) {
+    rc = launch_clear2(dA, (size_t)L->K * L->r * sizeof(float), nullptr, 0, st);
+    if (rc != FT_OK) return rc;
+    chained = true;
+  }
   // G small enough for the single-pass quantizer (<= ~29 MB: it finds the amax itself and reads G once):
-  // quantize, GEMM, one wgrad launch for both gradients -- G is read twice either way, with two
-  // launches fewer than the schedule below
+  // quantize, GEMM, one wgrad launch for both gradients -- G is read twice either way, with one
+  // launch fewer than the schedule below
   if (quantize_single_pass_fits(M, L->N, r_t)) {
     rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
-                     workspace, workspace_bytes, nullptr, st);
+                     workspace, workspace_bytes, nullptr, chained, st);
     if (rc != FT_OK) return rc;
     if (qx == nullptr)
       return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                          accumulate, nullptr, nullptr, 0, false, false, st);
-    return ft_lora_wgrad_q4(L, qx, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt, accumulate, stream);
+                          accumulate, nullptr, true, false, st);
+    rc = launch_wgrad(2, nullptr, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
+                      accumulate, nullptr, true, false, st);
+    if (rc != FT_OK) return rc;
+    return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA, 1,
+                           false, st);
   }
-  // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0).  The
-  //    workspace's control words (the amax word among them) and dB^T are cleared by ONE small kernel with
-  //    programmatic edges on both sides instead of two memset nodes; the dB^T kernel also zero-fills dA
-  //    for step 3.  (accumulate: dB^T keeps its contents, only the control words are cleared.)
-  const WsLayout w = ws_layout(M, r_t);
-  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
-  rc = launch_clear2(ws + w.zero_off, w.zero_bytes, dBt, accumulate ? 0 : (size_t)L->N * L->r * sizeof(float), st);
-  if (rc != FT_OK) return rc;
-  unsigned int* amax_g = reinterpret_cast<unsigned int*>(ws + w.amax_ext_off);
+  // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0), into a control
+  //    word of the workspace (zero by the workspace invariant; the quantize kernel puts it back).  The M slices
+  //    combine over distributed shared memory inside the kernel: no clear kernel, no memset node.
+  unsigned int* amax_g = reinterpret_cast<unsigned int*>(ws + WS_CTL_AMAX_EXT);
   rc = launch_wgrad(2, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                    1, amax_g, accumulate ? nullptr : dA, accumulate ? 0 : L->K * (int64_t)L->r, true, false, st);
+                    accumulate, amax_g, chained, false, st);
   if (rc != FT_OK) return rc;
   // 2. a3 + a4 with that amax: Q(G), P = G U_t, dX
   rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
-                   workspace, workspace_bytes, reinterpret_cast<const float*>(amax_g), st);
+                   workspace, workspace_bytes, reinterpret_cast<const float*>(amax_g), true, st);
   if (rc != FT_OK) return rc;
-  // 3. dA = X^T (G B^T) needs P; its buffer was cleared by step 1 (accumulate == 1: nothing to clear).
-  //    Nothing it touches depends on the GEMM in front of it (X, P in; dA out), and every CTA of the GEMM
-  //    passes its own wait -- P complete -- before triggering: dA starts in the GEMM's tail and waits for
-  //    the GEMM only before it exits.
+  // 3. dA = X^T (G B^T) needs P.  Nothing it touches depends on the GEMM in front of it (X, P in; dA and its
+  //    out), and every CTA of the GEMM passes its own wait -- P complete -- before triggering: dA
+  //    starts in the GEMM's tail and waits for the GEMM only before it exits.
   if (qx == nullptr)
     return launch_wgrad(1, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                        1, nullptr, nullptr, 0, true, true, st);
+                        accumulate, nullptr, true, true, st);
   return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA, 1,
                          true, st);
 }

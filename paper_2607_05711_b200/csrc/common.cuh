@@ -39,27 +39,30 @@ int current_device();                // ordinal of the calling thread's current 
 int sm_count();                      // of the current device
 bool pdl_enabled();  // programmatic dependent launch of the GEMM and dA kernels (FT_PDL=0 turns it off)
 
-// Caller-provided workspace of one quantize (+ GEMM) pass over an [M x *] activation with a rank-r_t
-// projection.  [hs_off, +M*r_t*2): the pre-scaled bf16 intermediate Hs.  The "zero region" (256 bytes)
-// is cleared by one memset per call: the tensor-amax word, two grid-barrier counters and the word for
-// an amax found outside the quantize kernel.  Behind it:
-// one 128 x r_t fp32 slot per (CTA, row tile) segment of the quantize kernel -- at most
-// WS_MAX_QUANT_CTAS + row tiles of them -- holding partial H tiles.
-constexpr int WS_MAX_QUANT_CTAS = 320;   // 2 CTAs per SM, <= 160 SMs
+// Caller-provided workspace of one layer call.
+//   [0, WS_CTL_BYTES)      control words.  INVARIANT: all zero between calls.  ft_workspace_init (or the caller
+//                          zero-filling the buffer once) establishes it; the quantize kernel -- the only kernel
+//                          that uses them besides the writers of the two amax words -- puts every word back to
+//                          zero before its grid completes (the last CTA to leave), so no clear kernel or memset
+//                          node runs per call.  Fixed offset and size: one buffer may serve calls of any shapes.
+//       +0   amax word of the single-pass quantizer / of k_amax        +4  grid barrier (amax published)
+//       +8   exit counter of the quantize kernel
+//       +16  amax found by another kernel (the dB^T pass of ft_linear_bwd)
+//   [hs_off, +M*r_t*2)     the pre-scaled bf16 intermediate Hs (ft_workspace_hs_offset)
+//   [slots_off, ...)       one 128 x r_t fp32 slot per (CTA, row tile) segment of the quantize kernel -- at most
+//                          WS_MAX_QUANT_CTAS + row tiles of them -- holding partial H tiles
+constexpr int WS_MAX_QUANT_CTAS = 192;   // one CTA per SM
+constexpr size_t WS_CTL_BYTES = 4096;
+constexpr size_t WS_CTL_AMAX = 0, WS_CTL_BAR = 4, WS_CTL_EXIT = 8, WS_CTL_AMAX_EXT = 16;
 struct WsLayout {
-  size_t hs_off, zero_off, zero_bytes, amax_off, bar_off, amax_ext_off, slots_off, total;
+  size_t hs_off, slots_off, total;
 };
 inline WsLayout ws_layout(int64_t M, int r_t) {
   auto up = [](size_t v) { return (v + 255) / 256 * 256; };
   WsLayout w;
   const size_t tiles = (size_t)((M + 127) / 128);
-  w.hs_off = 256;
-  w.zero_off = w.hs_off + up((size_t)M * (size_t)r_t * 2);
-  w.amax_off = w.zero_off;
-  w.bar_off = w.zero_off + 4;
-  w.amax_ext_off = w.zero_off + 16;   // amax found by another kernel (the dB^T pass of ft_linear_bwd)
-  w.zero_bytes = 256;
-  w.slots_off = w.zero_off + w.zero_bytes;
+  w.hs_off = WS_CTL_BYTES;
+  w.slots_off = w.hs_off + up((size_t)M * (size_t)r_t * 2);
   w.total = w.slots_off + (WS_MAX_QUANT_CTAS + tiles) * 128 * (size_t)r_t * 4 + 256;
   return w;
 }

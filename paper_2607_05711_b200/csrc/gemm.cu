@@ -250,6 +250,7 @@ static int launch_gemm4_bn(const CUtensorMap& ma, const CUtensorMap& mb, const C
 int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
                       const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, bool lr_late, cudaStream_t st);
 int g_force_bn = 0;  // test/bench hook: 0 = CTA-pair kernel (default), else 1-CTA kernel with this N tile
+extern int g_pair_bn;   // gemm_pair.cu: 0 = tile width chosen per shape, else forced
 
 template <int BN>
 static int setup_and_launch(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
@@ -297,7 +298,13 @@ int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N,
 }  // namespace ft
 
 extern "C" int ft_debug_set_gemm_tile_n(int bn) {
+  if (bn == 1224 || bn == 1256) {   // the CTA-pair kernel with a forced tile width
+    ft::g_force_bn = 0;
+    ft::g_pair_bn = bn - 1000;
+    return FT_OK;
+  }
   if (bn != 0 && bn != 128 && bn != 192 && bn != 256) return FT_ERR_INVALID_ARG;
   ft::g_force_bn = bn;
+  ft::g_pair_bn = 0;
   return FT_OK;
 }

@@ -46,7 +46,10 @@ __global__ void __launch_bounds__(256) k_amax(const uint4* __restrict__ x, int64
   }
 }
 
-int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first) {
+// zero_first: the target word is not known to be zero (ft_tensor_amax): a memset node precedes the kernel.
+// pdl: a kernel of the same call directly precedes the launch (never together with zero_first: a memset
+// predecessor gets no programmatic edge).
+int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first, bool pdl) {
   if (zero_first) FT_CUDA_TRY(cudaMemsetAsync(amax_out, 0, sizeof(float), st));
   if (n == 0) return FT_OK;
   const int64_t n_vec = n / 8;
@@ -63,7 +66,7 @@ int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st,
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = (!zero_first && pdl_enabled()) ? 1 : 0;   // directly behind the caller's clear kernel
+  cfg.numAttrs = (!zero_first && pdl && pdl_enabled()) ? 1 : 0;
   FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_amax, reinterpret_cast<const uint4*>(x_bf16), n_vec,
                                  reinterpret_cast<const uint16_t*>(x_bf16) + n_vec * 8, n_tail,
                                  reinterpret_cast<unsigned int*>(amax_out)));
@@ -204,6 +207,31 @@ __global__ void __launch_bounds__(256) k_expand_sf(const uint8_t* __restrict__ S
   }
 }
 
+// The scales of a weight operand [rows x cols] (16x16 blocks) cut to output tiles of `ntile` rows
+// (ft_qtensor::sf_ntile): one thread per output byte.  transposed == 0: scale(row, kb) = S[row/16][kb] with S
+// [rows/16][cols/16]; transposed == 1 (the dgrad operand, rows = K, cols = N): scale(row, nb) = S[nb][row/16]
+// with S [cols/16][rows/16].
+__global__ void __launch_bounds__(256) k_expand_sf_ntile(const uint8_t* __restrict__ S, int64_t rows, int64_t cols,
+                                                         int ntile, int transposed, uint8_t* __restrict__ out) {
+  const int64_t k64 = cols / 64, tiles = (rows + ntile - 1) / ntile;
+  const int64_t total = tiles * k64 * 1024;
+  const int64_t o = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (o >= total) return;
+  const int64_t grp = o / 512;                 // (nt * k64 + ks) * 2 + half
+  const int within = (int)(o % 512);
+  const int half = (int)(grp & 1);
+  const int64_t ks = (grp >> 1) % k64, nt = (grp >> 1) / k64;
+  const int l = within / 16, gi = (within % 16) / 4, c = within % 4;
+  const int rt = half * 128 + gi * 32 + l;     // row inside the tile
+  const int64_t row = nt * ntile + rt;
+  uint8_t v = 0;
+  if (rt < ntile && row < rows) {
+    const int64_t kb = ks * 4 + c;
+    v = transposed ? S[kb * (rows / 16) + row / 16] : S[(row / 16) * (cols / 16) + kb];
+  }
+  out[o] = v;
+}
+
 int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn,
                        cudaStream_t st) {
   const int64_t N = rk->rows, K = rk->cols;
@@ -217,6 +245,16 @@ int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* r
   k_expand_sf<<<(unsigned)ceil_div(tmax, 256), 256, 0, st>>>(
       rk->sf, N, K, rk_tiled ? rk_tiled->sf : nullptr, rn->sf);
   FT_CUDA_TRY(cudaGetLastError());
+  if (rk_tiled != nullptr && rk_tiled->sf_ntile != nullptr && rk_tiled->ntile > 0) {
+    const int64_t total = ceil_div(N, rk_tiled->ntile) * (K / 64) * 1024;
+    k_expand_sf_ntile<<<(unsigned)ceil_div(total, 256), 256, 0, st>>>(rk->sf, N, K, rk_tiled->ntile, 0, rk_tiled->sf_ntile);
+    FT_CUDA_TRY(cudaGetLastError());
+  }
+  if (rn->sf_ntile != nullptr && rn->ntile > 0) {
+    const int64_t total = ceil_div(K, rn->ntile) * (N / 64) * 1024;
+    k_expand_sf_ntile<<<(unsigned)ceil_div(total, 256), 256, 0, st>>>(rk->sf, K, N, rn->ntile, 1, rn->sf_ntile);
+    FT_CUDA_TRY(cudaGetLastError());
+  }
   FT_CUDA_TRY(cudaMemcpyAsync(rn->tensor_dec_scale, rk->tensor_dec_scale, sizeof(float),
                               cudaMemcpyDeviceToDevice, st));
   if (rk_tiled != nullptr && rk_tiled->tensor_dec_scale != rk->tensor_dec_scale &&

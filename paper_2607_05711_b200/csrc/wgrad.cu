@@ -5,13 +5,19 @@
 // 64-row chunks that TMA stages (SWIZZLE_128B) through an mbarrier ring.  One thread issues
 // tcgen05.mma kind::f16 (M = 128 features, N = r, K = 16 rows, four per chunk) with BOTH
 // operands MN-major -- the staged chunks are used as they lie in memory, nothing is transposed
-// by the SM -- into a TMEM accumulator; four warps drain it and combine the M slices with
-// fp32 vector red.global.add.
+// by the SM -- into a TMEM accumulator; four warps drain it.  The M slices of one feature tile (at most 8) are
+// the CTAs of one thread-block cluster (1, slices, 1): each parks its fp32 partial tile in its own shared
+// memory, and after a cluster barrier every CTA sums an equal share of the tile over distributed shared memory,
+// in slice order, and writes (or adds to) the output.  No clear kernel, no atomics on the data, no workspace,
+// the same bits on every run.  (Round 1 combined the slices with red.global.add into a pre-cleared output: a
+// clear launch per call and an unordered sum.  Slots in global memory with an arrival counter per tile -- the
+// scheme of the quantize kernel -- cost 20 us per step here: the last arriver's sum is a chain of L2 round trips.)
+#include <cstdio>
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace ft {
-
-int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t st);
 
 constexpr int WG_F = 128;
 constexpr int WG_MC = 64;
@@ -25,19 +31,20 @@ struct WgParams {      // two problems in one launch: [0] dA = X^T P_lora, [1] d
   int64_t F[2];
   int r_s, r;
   int chunks_per_cta[2];
-  int direct[2];       // 1: a single M slice owns the output, plain stores (no zero-fill needed)
   float* out[2];
   unsigned int* amax_bits[2];   // non-null: atomicMax target for max |In| (bf16 bits << 16), pre-zeroed
   int late_wait;                // 1: nothing this launch touches depends on its predecessor, which passes
                                 //    griddepcontrol.wait in every CTA before triggering: start beside it and
                                 //    wait for it at the END (completion stays transitive for the next launch)
-  float4* zero_fill;            // non-null: buffer this launch clears for a LATER launch (zero_fill_n4 float4s)
-  int64_t zero_fill_n4;
+  int n_slices;                 // M slices = CTAs per cluster (gridDim.y); every slice has work
+  int accumulate;               // add to the output instead of overwriting it
 };
 
-__device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
-  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d)
-               : "memory");
+__device__ __forceinline__ float4 ld_cluster_f4(uint32_t cluster_addr) {
+  float4 v;
+  asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(cluster_addr) : "memory");
+  return v;
 }
 
 template <int R>
@@ -46,18 +53,13 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
         const __grid_constant__ CUtensorMap map_in1, const __grid_constant__ CUtensorMap map_l1,
         const WgParams p) {
   const int z = blockIdx.z;
-  if (p.zero_fill != nullptr) {   // grid-stride clear, every CTA of the launch (before any early return)
-    pdl_wait();                   // launched with a programmatic edge: nothing is written before the predecessor ends
-    const int64_t nthr = (int64_t)gridDim.x * gridDim.y * gridDim.z * WG_THREADS;
-    const int64_t me = ((int64_t)(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) * WG_THREADS + threadIdx.x;
-    for (int64_t i = me; i < p.zero_fill_n4; i += nthr) p.zero_fill[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-  }
   const CUtensorMap& map_in = z == 0 ? map_in0 : map_in1;
   const CUtensorMap& map_l = z == 0 ? map_l0 : map_l1;
   const int64_t F = p.F[z];
   const int cpc = p.chunks_per_cta[z];
-  // CTAs beyond this problem's feature tiles or M slices have nothing to do (uniform per CTA)
-  if ((int64_t)blockIdx.x * WG_F >= F || (int64_t)blockIdx.y * cpc >= (p.M + WG_MC - 1) / WG_MC) return;
+  // CTAs beyond this problem's feature tiles have nothing to do (uniform per cluster: a cluster spans blockIdx.y
+  // only).  Every M slice has work: the host sizes gridDim.y = ceil(chunks / chunks_per_cta).
+  if ((int64_t)blockIdx.x * WG_F >= F) return;
   constexpr int NG = (R + 63) / 64;
   constexpr int STAGE_BYTES = WG_IN_BYTES + NG * WG_LG_BYTES;
   constexpr uint32_t TMEM_COLS = R <= 32 ? 32 : (R <= 64 ? 64 : 128);
@@ -157,36 +159,80 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
   }
   __syncwarp();
 
-  if (n_chunks > 0) {   // ---- drain: thread = feature (TMEM lane), R fp32 columns
-    mbar_wait(&acc_bar, 0);
+  {   // ---- drain: thread = feature (TMEM lane), R fp32 columns
+    mbar_wait(&acc_bar, 0);   // every MMA has completed: the ring's shared memory is free
     tc_fence_after();
-    const int64_t f = (int64_t)f0 + warp * 32 + lane;
+    const int fl = warp * 32 + lane;
+    const int64_t f = (int64_t)f0 + fl;
+    const int ns = p.n_slices;
+    // several slices: park the partial tile in this CTA's shared memory (the ring's: every warp must be done with
+    // the staged chunks first -- the amax warps read them too), layout [column quad][feature][4 floats]
+    if (ns > 1) __syncthreads();
+    float* park = reinterpret_cast<float*>(smem);
 #pragma unroll
     for (int c0 = 0; c0 < R; c0 += 16) {
       uint32_t v[16];
-      asm volatile(
-          "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-          "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-          : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-            "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-          : "r"(tmem_base + ((uint32_t)(warp * 32) << 16) + c0)
-          : "memory");
+      tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + c0, v);
       tmem_ld_wait();
-      if (f < F) {
-        float* o = p.out[z] + f * R + c0;
-        if (p.direct[z]) {
+      if (ns > 1) {
 #pragma unroll
-          for (int j = 0; j < 16; j += 4)
-            *reinterpret_cast<uint4*>(o + j) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
-        } else {
+        for (int j = 0; j < 16; j += 4)
+          *reinterpret_cast<uint4*>(park + ((c0 + j) / 4 * WG_F + fl) * 4) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+      } else if (f < F) {
+        float4* o = reinterpret_cast<float4*>(p.out[z] + f * R + c0);
 #pragma unroll
-          for (int j = 0; j < 16; j += 4)
-            red_add_v4(o + j, __uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]),
-                       __uint_as_float(v[j + 3]));
+        for (int j = 0; j < 16; j += 4) {
+          float4 a = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]),
+                                 __uint_as_float(v[j + 3]));
+          if (p.accumulate) {
+            const float4 old = o[j / 4];
+            a.x += old.x;
+            a.y += old.y;
+            a.z += old.z;
+            a.w += old.w;
+          }
+          o[j / 4] = a;
         }
       }
     }
     tc_fence_before();
+    if (ns > 1) {
+      // the cluster = the M slices of this feature tile.  After the barrier slice s sums column quads
+      // s, s + ns, ... of the tile over all slices' shared memory, in slice order, and owns those outputs.
+      cluster_sync();
+      const uint32_t rank = cluster_ctarank();
+      const uint32_t park_u = smem_u32(park);
+#pragma unroll 1
+      for (int q = (int)rank; q < R / 4; q += ns) {
+        const uint32_t off = park_u + (uint32_t)((q * WG_F + fl) * 16);
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int s0 = 0; s0 < ns; s0 += 4) {
+          float4 v[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            v[j] = (s0 + j < ns) ? ld_cluster_f4(map_to_cta(off, (uint32_t)(s0 + j))) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            acc.x += v[j].x;
+            acc.y += v[j].y;
+            acc.z += v[j].z;
+            acc.w += v[j].w;
+          }
+        }
+        if (f < F) {
+          float4* o = reinterpret_cast<float4*>(p.out[z] + f * R + q * 4);
+          if (p.accumulate) {
+            const float4 old = *o;
+            acc.x += old.x;
+            acc.y += old.y;
+            acc.z += old.z;
+            acc.w += old.w;
+          }
+          *o = acc;
+        }
+      }
+      cluster_sync();   // no slice leaves (and frees its shared memory) while a peer still reads it
+    }
   }
   __syncthreads();
   if (warp == 2) {
@@ -199,30 +245,49 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
 template <int R>
 static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, bool pdl, cudaStream_t st) {
   constexpr int NG = (R + 63) / 64;
-  const int smem = WG_STAGES * (WG_IN_BYTES + NG * WG_LG_BYTES) + 1024;
+  const int smem = WG_STAGES * (WG_IN_BYTES + NG * WG_LG_BYTES) + 1024;   // >= the 128 x R fp32 parked tile
   FT_CUDA_TRY(cudaFuncSetAttribute(k_wgrad<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = grid;
   cfg.blockDim = dim3(WG_THREADS, 1, 1);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
-  cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cudaLaunchAttribute attr[2];
+  int na = 0;
+  if (grid.y > 1) {   // the M slices of a feature tile form one cluster
+    attr[na].id = cudaLaunchAttributeClusterDimension;
+    attr[na].val.clusterDim.x = 1;
+    attr[na].val.clusterDim.y = grid.y;
+    attr[na].val.clusterDim.z = 1;
+    ++na;
+  }
+  if (pdl && pdl_enabled()) {
+    attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+  }
   cfg.attrs = attr;
-  cfg.numAttrs = (pdl && pdl_enabled()) ? 1 : 0;
+  cfg.numAttrs = na;
+  if (getenv("FT_DEBUG_OCC") != nullptr) {
+    int ncl = -1, nb = -1;
+    cudaOccupancyMaxActiveClusters(&ncl, k_wgrad<R>, &cfg);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_wgrad<R>, WG_THREADS, smem);
+    fprintf(stderr, "k_wgrad<%d> grid (%u,%u,%u) smem %d: max active clusters %d, blocks/SM %d\n", R, grid.x, grid.y, grid.z,
+            smem, ncl, nb);
+  }
   FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_wgrad<R>, maps[0], maps[1], maps[2], maps[3], p));
   return FT_OK;
 }
 
 // which = 1: dA [K x r] = X^T P[:, r_s:];  which = 2: dBt [N x r] = G^T H[:, r_s:];  which = 3: both in
-// ONE launch (blockIdx.z picks the problem).  accumulate == 0 and a single M slice: plain stores;
-// otherwise the buffers are zeroed first (accumulate == 0) and the slices combine with fp32 reductions.
-// amax_g (which & 2 only): pre-zeroed word that receives the bit pattern of max |G|.
+// ONE launch (blockIdx.z picks the problem).  The M slices (at most 8, the portable cluster size) of a feature
+// tile are one cluster and combine over distributed shared memory in slice order.
+// amax_g (which & 2 only): zero word that receives the bit pattern of max |G|.
+// after_kernel: the launch directly follows a kernel of the same call (programmatic edge allowed).
+// beside_prev: see WgParams::late_wait (the caller's promise).
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, float* zero_fill, int64_t zero_fill_n, bool after_kernel, bool beside_prev,
-                 cudaStream_t st) {
+                 unsigned int* amax_g, bool after_kernel, bool beside_prev, cudaStream_t st) {
   CUtensorMap maps[4];
   const void* in_all[2] = {x, g};
   const void* lr_all[2] = {p_saved, h_saved};
@@ -232,8 +297,7 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
   p.M = M;
   p.r_s = r_s;
   p.r = r;
-  p.zero_fill = reinterpret_cast<float4*>(zero_fill);
-  p.zero_fill_n4 = zero_fill_n / 4;   // K * r, r % 16 == 0
+  p.accumulate = accumulate;
   const int64_t chunks = ceil_div(M, WG_MC);
   // the enabled problems, compacted into z = 0 .. nz-1
   int sel[2], nz = 0;
@@ -242,14 +306,15 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
   int64_t f_tiles_total = 0;
   for (int i = 0; i < nz; ++i) f_tiles_total += ceil_div(F_all[sel[i]], WG_F);
   // M slices: one wave of two resident CTAs per SM over all feature tiles (rounded DOWN: a second,
-  // mostly empty wave costs more than slightly longer slices), at least 8 chunks (512 rows) each
+  // mostly empty wave costs more than slightly longer slices), at least 8 chunks (512 rows) each, at most 8
   int64_t slices = (int64_t)2 * sm_count() / f_tiles_total;
   if (slices > chunks / 8) slices = chunks / 8;
+  if (slices > 8) slices = 8;
   if (slices < 1) slices = 1;
-  unsigned gx = 0, gy = 0;
-  void* clr[2] = {nullptr, nullptr};
-  size_t clr_bytes[2] = {0, 0};
-  int nclr = 0;
+  const int cpc = (int)ceil_div(chunks, slices);
+  const unsigned sl = (unsigned)ceil_div(chunks, cpc);   // every slice has at least one chunk
+  p.n_slices = (int)sl;
+  unsigned gx = 0;
   for (int i = 0; i < 2; ++i) {
     const int z = i < nz ? sel[i] : sel[0];
     int rc = make_tensor_map_2d(&maps[2 * i], in_all[z], 2, (uint64_t)F_all[z], (uint64_t)M, (uint64_t)F_all[z] * 2, 64,
@@ -259,32 +324,16 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
                             Swizzle::B128);
     if (rc != FT_OK) return rc;
     p.F[i] = F_all[z];
-    p.chunks_per_cta[i] = (int)ceil_div(chunks, slices);
-    const unsigned sl = (unsigned)ceil_div(chunks, p.chunks_per_cta[i]);
-    p.direct[i] = (sl == 1 && !accumulate) ? 1 : 0;
+    p.chunks_per_cta[i] = cpc;
     p.out[i] = out_all[z];
     p.amax_bits[i] = z == 1 ? amax_g : nullptr;
     if (i >= nz) continue;
-    if (!accumulate && !p.direct[i]) {   // cleared below by one kernel with programmatic edges
-      clr[nclr] = out_all[z];
-      clr_bytes[nclr++] = (size_t)F_all[z] * r * sizeof(float);
-    }
     const unsigned ft = (unsigned)ceil_div(F_all[z], WG_F);
     if (ft > gx) gx = ft;
-    if (sl > gy) gy = sl;
   }
-  const dim3 grid(gx, gy, (unsigned)nz);
-  if (nclr > 0) {
-    int rc = launch_clear2(clr[0], clr_bytes[0], clr[1], clr_bytes[1], st);
-    if (rc != FT_OK) return rc;
-    after_kernel = true;
-  }
-  // after_kernel: the launch directly follows a kernel of the same call (the clear above, or the caller's
-  // previous launch with accumulate set): it may set itself up while that kernel drains
-  const bool pdl = after_kernel && (accumulate != 0 || nclr > 0 || (p.direct[0] && (nz == 1 || p.direct[1])));
-  // beside_prev (caller's promise, see WgParams::late_wait): only without a clear kernel in between and
-  // without a zero-fill job, whose wait comes first
-  p.late_wait = (beside_prev && pdl && nclr == 0 && zero_fill == nullptr) ? 1 : 0;
+  const dim3 grid(gx, sl, (unsigned)nz);
+  const bool pdl = after_kernel;
+  p.late_wait = (beside_prev && pdl) ? 1 : 0;
   switch (r) {
     case 16: return launch_wg<16>(maps, p, grid, pdl, st);
     case 32: return launch_wg<32>(maps, p, grid, pdl, st);

@@ -38,6 +38,20 @@ def rel(a, b):
     return np.linalg.norm(np.asarray(a, np.float64) - np.asarray(b, np.float64)) / (d if d > 0 else 1.0)
 
 
+def sf_ntile_layout(sf_rows, ntile):
+    """The scales of a weight operand cut to output tiles of `ntile` rows (include/fourtune.h, ft_qtensor::sf_ntile),
+    from per-row scales [rows x nblk]: an index function of its own, written from the header's description."""
+    rows, nblk = sf_rows.shape
+    k64, tiles = nblk // 4, (rows + ntile - 1) // ntile
+    out = np.zeros(tiles * k64 * 1024, dtype=np.uint8)
+    r, c = np.meshgrid(np.arange(rows), np.arange(nblk), indexing="ij")
+    nt, rt = r // ntile, r % ntile
+    half, r128 = rt // 128, rt % 128
+    off = ((nt * k64 + c // 4) * 2 + half) * 512 + (r128 % 32) * 16 + (r128 // 32) * 4 + c % 4
+    out[off] = sf_rows
+    return out
+
+
 def assert_q_equal(qt, q, layout, B):
     rows, cols = q["codes"].shape
     assert np.array_equal(qt.codes.cpu().numpy(), q["packed"])
@@ -133,6 +147,11 @@ def test_weight_quantize_16x16_and_pack(B, N, K):
     assert_q_equal(L.r_nmajor, qT, B.FT_SF_TILE128x4, B)
     q2 = nvfp4.quantize_blockwise(np.ascontiguousarray(W.T), 16)
     assert np.array_equal(q2["packed"], qT["packed"]) and np.array_equal(q2["sf"], qT["sf"])
+    # the same scales once more, cut to the 224-wide tiles of the GEMM (both orientations)
+    for qt, qo in ((L.r_kmajor, q), (L.r_nmajor, qT)):
+        assert qt.ntile == 224
+        want = sf_ntile_layout(nvfp4.sf_expand_rows(qo["sf"], 16), 224)
+        assert np.array_equal(qt.sf_ntile.cpu().numpy(), want)
 
 
 @pytest.mark.parametrize("rows,cols,r_t,kind", [(128, 512, 16, "x"), (200, 1024, 64, "x"), (256, 3072, 48, "x"),
@@ -259,10 +278,15 @@ def run_layer(B, L, X, G, M, K, N, r_t, r, fused_bwd=False):
                 xt=xt, gt=gt, ht=h, pt=p)
 
 
-LAYER_CASES = [  # seed, M, K, N, r_s, r, tile_n
+LAYER_CASES = [  # seed, M, K, N, r_s, r, tile_n (fourtune_debug.h: 0 auto, 128/192/256 1-CTA, 1224/1256 pair kernel)
     (11, 1, 64, 64, 0, 0, 0), (12, 128, 256, 128, 0, 0, 256), (13, 130, 320, 192, 16, 16, 0),
     (14, 256, 512, 384, 16, 16, 192), (15, 200, 1024, 768, 32, 64, 256), (16, 300, 576, 448, 32, 32, 128),
-    (17, 129, 2048, 640, 0, 16, 192)]
+    (17, 129, 2048, 640, 0, 16, 192),
+    # the CTA-pair kernel with 224-wide tiles: N = 64 (one ragged tile of 64), 192, 448 (two full tiles), 640 (224 + 224
+    # + 192), 768 (3 x 224 + 96: a 32-column unit in a ragged tile), K with a partial stage; and the 256-wide one forced
+    (18, 1, 64, 64, 0, 0, 1224), (19, 130, 320, 192, 16, 16, 1224), (20, 300, 576, 448, 32, 32, 1224),
+    (21, 129, 2048, 640, 0, 16, 1224), (22, 200, 1024, 768, 32, 64, 1224), (23, 260, 448, 1024, 16, 96, 1224),
+    (24, 300, 576, 448, 32, 32, 1256), (25, 200, 1024, 768, 32, 64, 1256)]
 
 
 @pytest.mark.parametrize("seed,M,K,N,r_s,r,bn", LAYER_CASES)
@@ -354,10 +378,17 @@ MULTI_TILE_CASES = [   # seed, M, K, N, r_s, r
 ]
 
 
+@pytest.mark.parametrize("bn", [1224, 1256], ids=["pair224", "pair256"])
 @pytest.mark.parametrize("seed,M,K,N,r_s,r", MULTI_TILE_CASES)
-def test_layer_multi_tile_per_cta_pair(B, seed, M, K, N, r_s, r):
-    d, R, D_f, U_f, L = make_layer_fast(B, seed, M, K, N, r_s, r)
-    out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=r > 0)
+def test_layer_multi_tile_per_cta_pair(B, seed, M, K, N, r_s, r, bn):
+    """Both tile widths of the CTA-pair GEMM: 256 (scale columns overlaid on the draining accumulator, hand-over
+    per tile) and 224 (scale columns of their own, ragged last tile of every row of tiles)."""
+    B.debug_set_gemm_tile_n(bn)
+    try:
+        d, R, D_f, U_f, L = make_layer_fast(B, seed, M, K, N, r_s, r)
+        out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=r > 0)
+    finally:
+        B.debug_set_gemm_tile_n(0)
     check_layer(B, d, R, D_f, U_f, out, r_s, r)
 
 
