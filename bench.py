@@ -28,9 +28,45 @@ WORKLOAD = dict(name="C2 FLUX.1-dev fused QKV projection", M=4608, K=3072, N=921
 METRIC = "W4A4G4 linear fwd+bwd TFLOPS (4*M*N*K per step / step time)"
 UNIT = "TFLOP/s"
 FP4_OVER_BF16 = 4.0   # nominal dense ratio 9 / 2.25 PFLOP/s (B200_PROFILING.md)
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_gemm4 launch (C2 forward), from the
-# ncu --set full capture summarised in profiles/r01h_launches.md (ncu flushes caches per launch).
-GEMM_DRAM_TRAFFIC_BYTES = 57846272   # 25.69 MB read + 32.15 MB written, profiles/r01h_launches.md
+FP4_NOMINAL_TFLOPS = 9000.0   # dense NVFP4, B200 (B200_PROFILING.md): the peak north_star's 60 % bar refers to
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the C2 step
+# summarised in profiles/r02_full_summary.md (ncu flushes the caches before every launch: cold-cache figures)
+NCU_DRAM_TRAFFIC = {"gemm_fwd": None, "gemm_dgrad": None, "quantize_X": None, "quantize_G": None,
+                    "wgrad_dBt": None, "wgrad_dA": None}
+PROBE_SRC = os.path.join(ROOT, "bench_fp4_probe.cu")
+PROBE_BIN = os.path.join(ROOT, "build", "bench_fp4_probe")
+
+
+def build_fp4_probe():
+    """nvcc the FP4 tensor-core probe (bench_fp4_probe.cu) into build/ if it is missing or stale."""
+    if os.path.exists(PROBE_BIN) and os.path.getmtime(PROBE_BIN) >= os.path.getmtime(PROBE_SRC):
+        return PROBE_BIN
+    os.makedirs(os.path.dirname(PROBE_BIN), exist_ok=True)
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "--expt-relaxed-constexpr",
+                    "-I", ROOT, "-o", PROBE_BIN, PROBE_SRC, "-lcuda"], check=True, capture_output=True)
+    return PROBE_BIN
+
+
+def run_fp4_probe(seconds, gpu_index):
+    """MMA-only FP4 rate (operands resident in shared memory, no TMA, no epilogue) sustained for `seconds`,
+    with the SM clock sampled meanwhile: the measured ceiling next to the nominal 9 PFLOP/s."""
+    try:
+        exe = build_fp4_probe()
+        sampler = ClockSampler(gpu_index)
+        sampler.start()
+        env = dict(os.environ, CUDA_VISIBLE_DEVICES=os.environ.get("CUDA_VISIBLE_DEVICES", str(gpu_index)))
+        r = subprocess.run([exe, "--sustained", str(seconds)], capture_output=True, text=True, timeout=120, env=env)
+        clocks = sampler.stop()
+        line = [l for l in r.stdout.splitlines() if l.startswith("sustained")]
+        if r.returncode != 0 or not line:
+            return {"error": (r.stdout + r.stderr)[-300:]}
+        tf = float(line[0].split()[-2])
+        cyc = float(line[0].split("launches:")[1].split()[0])
+        return {"tflops": tf, "cycles_per_mma_m256_n256_k64": cyc, "seconds": seconds, "sm_mhz_median": clocks["sm_mhz"],
+                "reasons": clocks["reasons"], "raw": line[0]}
+    except Exception as e:   # noqa: BLE001
+        return {"error": str(e)[-300:]}
 
 
 def load_peaks():
@@ -186,10 +222,10 @@ def run_ours(args):
         B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws)
         if world > 1:
             parallel.allreduce_lora_grads(dA, dBt)
-    # fwd: k_quantize_fused (single pass, amax inside) + k_gemm4_pair; bwd (ft_linear_bwd): k_wgrad (dB^T + amax
-    # of G) + k_quantize_fused (streaming, row sums inside) + k_gemm4_pair + k_wgrad (dA): 6 kernels, no clear
+    # fwd: k_quantize_fused (single pass, amax inside) + k_finalize_h + k_gemm4_pair; bwd (ft_linear_bwd): k_wgrad
+    # (dB^T + amax of G) + k_quantize_fused (streaming) + k_finalize_h + k_gemm4_pair + k_wgrad (dA): 8 kernels, no clear
     # kernel and no memset node (the workspace's control words are put back by the kernels that use them)
-    KERNELS_PER_STEP = 6
+    KERNELS_PER_STEP = 8
 
     def barrier():
         if world > 1:
@@ -300,56 +336,21 @@ def run_ours(args):
     h2d = (Xh.numel() + Gh.numel()) * 2
     d2h = (yh.numel() + dxh.numel()) * 2 + (dAh.numel() + dBh.numel()) * 4
 
-    # ---- per-kernel breakdown: each launch alone, CUDA events on its stream, L2 flushed between
-    flush = torch.zeros(256 << 20, dtype=torch.uint8, device=dev)
-    flush_sink = torch.zeros((), dtype=torch.uint8, device=dev)
+    # ---- per-kernel breakdown.  Each call is captured N times back to back in ONE CUDA graph, cycling over
+    # enough copies of its input that the copies together exceed twice the L2 (so every launch reads its tensor from
+    # HBM, as in a training step), and the graph is replayed: kernel-to-kernel time, no launch gap, no L2 flush in
+    # the timed region.  The GEMMs replay on the same operands (42 MB: L2-resident in the real step as well).
     hs = B.workspace_hs(ws, M, r_t)
     amax = torch.empty(1, dtype=torch.float32, device=dev)
 
-    def timed(fn, n=20):
-        fn()
-        tot = 0.0
-        for _ in range(n):
-            flush_sink.copy_(flush.max())   # evict L2 with clean lines (a write flush would leave
-            #                                 126 MB of dirty lines to be written back under fn)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            fn()
-            b.record(stream)
-            torch.cuda.synchronize()
-            tot += a.elapsed_time(b)
-        return tot / n * 1e3   # us
-
-    kern = {}
-    kern["amax_X_us"] = timed(lambda: B.ft_tensor_amax(X, amax))
-    kern["quant_X_us"] = timed(lambda: B.ft_quantize_blockwise(
-        X, qx, tensor_amax=amax, down=D_f, h_out=h, hs_out=hs, other_dec_scale=layer.r_kmajor.tensor_dec_scale,
-        workspace=ws))
-    kern["amax_quant_X_single_pass_us"] = timed(lambda: B.ft_quantize_blockwise(
-        X, qx, down=D_f, h_out=h, hs_out=hs, other_dec_scale=layer.r_kmajor.tensor_dec_scale, workspace=ws))
-    kern["gemm_fwd_us"] = timed(lambda: B.ft_gemm4(qx, layer.r_kmajor, hs, U_t, y))
-    amax_g = B.ft_tensor_amax(G)
-    kern["amax_G_us"] = timed(lambda: B.ft_tensor_amax(G, amax_g))
-    kern["quant_G_us"] = timed(lambda: B.ft_quantize_blockwise(
-        G, qg, tensor_amax=amax_g, down=U_t, h_out=p, hs_out=hs, other_dec_scale=layer.r_nmajor.tensor_dec_scale,
-        workspace=ws))
-    kern["gemm_dgrad_us"] = timed(lambda: B.ft_gemm4(qg, layer.r_nmajor, hs, D_f, dx))
-    kern["wgrad_us"] = timed(lambda: B.ft_lora_wgrad(layer, X, G, h, p, dA, dBt))
-    kern["wgrad_saved4_us"] = timed(lambda: B.ft_lora_wgrad_q4(layer, qx, G, h, p, dA, dBt))
-    kern["bwd_fused_us"] = timed(lambda: B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws))
-    kern["fwd_us"] = timed(lambda: B.ft_linear_fwd(layer, X, y, h, qx, ws))
-
-    # the same step with 4-bit saved activations (NEXT-2): fwd + ft_linear_bwd_q4, as a CUDA graph
-    def step_saved4():
-        B.ft_linear_fwd(layer, X, y, h, qx, ws)
-        B.ft_linear_bwd_q4(layer, qx, G, h, dx, p, dA, dBt, qg, ws)
-
-    def graph_us(fn, n=100):
-        fn()
+    def graph_us(fns, n=20):
+        for f in fns:
+            f()
         torch.cuda.synchronize()
         gg = torch.cuda.CUDAGraph()
         with torch.cuda.graph(gg):
-            fn()
+            for f in fns:
+                f()
         for _ in range(3):
             gg.replay()
         torch.cuda.synchronize()
@@ -359,15 +360,63 @@ def run_ours(args):
             gg.replay()
         b.record(stream)
         torch.cuda.synchronize()
-        return a.elapsed_time(b) / n * 1e3
+        return a.elapsed_time(b) / (n * len(fns)) * 1e3
+
+    def copies(t, total_bytes=300e6):
+        k = max(2, int(total_bytes // (t.numel() * t.element_size())) + 1)
+        return [t] + [t.clone() for _ in range(k - 1)]
+
+    Xs, Gs = copies(X), copies(G)
+    kern = {}
+    kern["amax_X_us"] = graph_us([lambda x=x: B.ft_tensor_amax(x, amax) for x in Xs])
+    kern["quantize_X_a0a1_us"] = graph_us([lambda x=x: B.ft_quantize_blockwise(
+        x, qx, down=D_f, h_out=h, hs_out=hs, other_dec_scale=layer.r_kmajor.tensor_dec_scale, workspace=ws) for x in Xs])
+    amax_g = B.ft_tensor_amax(G)
+    kern["amax_G_us"] = graph_us([lambda g_=g_: B.ft_tensor_amax(g_, amax) for g_ in Gs])
+    kern["quantize_G_a3_us"] = graph_us([lambda g_=g_: B.ft_quantize_blockwise(
+        g_, qg, tensor_amax=amax_g, down=U_t, h_out=p, hs_out=hs, other_dec_scale=layer.r_nmajor.tensor_dec_scale,
+        workspace=ws) for g_ in Gs])
+    B.ft_quantize_blockwise(X, qx, down=D_f, h_out=h, hs_out=hs, other_dec_scale=layer.r_kmajor.tensor_dec_scale,
+                            workspace=ws)
+    kern["gemm_fwd_us"] = graph_us([lambda: B.ft_gemm4(qx, layer.r_kmajor, hs, U_t, y)] * 4)
+    B.ft_quantize_blockwise(G, qg, tensor_amax=amax_g, down=U_t, h_out=p, hs_out=hs,
+                            other_dec_scale=layer.r_nmajor.tensor_dec_scale, workspace=ws)
+    kern["gemm_dgrad_us"] = graph_us([lambda: B.ft_gemm4(qg, layer.r_nmajor, hs, D_f, dx)] * 4)
+    kern["wgrad_dA_dBt_us"] = graph_us([lambda g_=g_, x=Xs[i % len(Xs)]: B.ft_lora_wgrad(layer, x, g_, h, p, dA, dBt)
+                                        for i, g_ in enumerate(Gs)])
+    kern["wgrad_saved4_us"] = graph_us([lambda g_=g_: B.ft_lora_wgrad_q4(layer, qx, g_, h, p, dA, dBt) for g_ in Gs])
+    kern["fwd_us"] = graph_us([lambda x=x: B.ft_linear_fwd(layer, x, y, h, qx, ws) for x in Xs])
+    kern["bwd_us"] = graph_us([lambda g_=g_, x=Xs[i % len(Xs)]: B.ft_linear_bwd(layer, x, g_, h, dx, p, dA, dBt, qg, ws)
+                               for i, g_ in enumerate(Gs)])
+
+    # the same step with 4-bit saved activations (NEXT-2): fwd + ft_linear_bwd_q4, as a CUDA graph
+    def step_saved4():
+        B.ft_linear_fwd(layer, X, y, h, qx, ws)
+        B.ft_linear_bwd_q4(layer, qx, G, h, dx, p, dA, dBt, qg, ws)
 
     def step_bf16x():
         B.ft_linear_fwd(layer, X, y, h, qx, ws)
         B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws)
-    kern["step_saved4_us"] = graph_us(step_saved4)
-    kern["step_bf16x_us"] = graph_us(step_bf16x)
+    kern["step_saved4_us"] = graph_us([step_saved4], 100)
+    kern["step_bf16x_us"] = graph_us([step_bf16x], 100)
 
-    # bf16 cuBLAS LoRA layer on the same GPU, same shapes (context: speedup vs BF16 LoRA)
+    # the step WITHOUT a graph: 8 launches enqueued by the host each step (tensor maps come from the library's memo)
+    def eager_us(fn, n=50):
+        for _ in range(5):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(n):
+            fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / n * 1e3
+    kern["step_eager_us"] = eager_us(step_bf16x)
+    del Xs, Gs
+    torch.cuda.empty_cache()
+
+    # bf16 cuBLAS LoRA layer on the same GPU, same shapes, same protocol (CUDA graph, back-to-back replays)
     Am, Bm = A, Bt.t().contiguous()
 
     def bf16_lora():
@@ -377,18 +426,45 @@ def run_ours(args):
         dxx = G @ Wt + gb @ Am.t()                    # noqa: F841
         da = X.t() @ gb                               # noqa: F841
         db = xa.t() @ G                               # noqa: F841
-    bf16_us = timed(bf16_lora, n=10)
+    bf16_us = graph_us([bf16_lora], 20)
 
     extra = {}
     if rank == 0 and world == 1 and not args.no_sweep:
         del yh, dxh
-        extra = sweep(B, prepare, dev, timed, peaks, full=not args.c4_only)
+        extra = sweep(B, prepare, dev, graph_us, peaks, full=not args.c4_only)
+    probe = run_fp4_probe(args.probe_seconds, local) if (rank == 0 and args.probe_seconds > 0) else None
     out = None
     if rank == 0:
+        fp4_derived = peaks["bf16"] * FP4_OVER_BF16
+        fp4_probe = probe["tflops"] if probe and "tflops" in probe else None
+        gemm_flop = 2.0 * M * N * K
+
+        def gemm_entry(name, us, step):
+            tf = gemm_flop / (us * 1e-6) / 1e12
+            return {"kernel": "k_gemm4_pair (%s)" % name, "step": step, "bound": "tensor", "work": gemm_flop, "work_unit": "flop",
+                    "us": round(us, 2), "achieved": tf, "unit": "TFLOP/s", "peak": FP4_NOMINAL_TFLOPS, "frac": tf / FP4_NOMINAL_TFLOPS,
+                    "frac_of_probe": (tf / fp4_probe) if fp4_probe else None, "frac_of_derived": tf / fp4_derived,
+                    "traffic": NCU_DRAM_TRAFFIC["gemm_" + name]}
+
+        def hbm_entry(kernel, step, nbytes, us, key):
+            gbs = nbytes / us / 1e3
+            return {"kernel": kernel, "step": step, "bound": "hbm", "work": nbytes, "work_unit": "bytes", "us": round(us, 2),
+                    "achieved": gbs, "unit": "GB/s", "peak": peaks["hbm"], "frac": gbs / peaks["hbm"],
+                    "frac_of_nominal_8TBps": gbs / 8000.0, "traffic": NCU_DRAM_TRAFFIC[key]}
+        qb = 2.5625 + 4.0 * r_t / K                       # codes + scales + H, Hs and the D slice per element of X
+        qbg = 2.5625 + 4.0 * r_t / N
+        roofs = [
+            gemm_entry("fwd", kern["gemm_fwd_us"], "a2"),
+            gemm_entry("dgrad", kern["gemm_dgrad_us"], "a4"),
+            hbm_entry("k_quantize_fused<64,single> + k_finalize_h (X: amax + quantize + projection, one call)", "a0+a1",
+                      qb * M * K, kern["quantize_X_a0a1_us"], "quantize_X"),
+            hbm_entry("k_quantize_fused<64,streaming> + k_finalize_h (G, amax given)", "a3", qbg * M * N,
+                      kern["quantize_G_a3_us"], "quantize_G"),
+            hbm_entry("k_wgrad<32> (dA and dB^T in one launch: reads X and G once)", "a5", 2.0 * M * (K + N),
+                      kern["wgrad_dA_dBt_us"], "wgrad_dBt"),
+        ]
         gemm_us = 0.5 * (kern["gemm_fwd_us"] + kern["gemm_dgrad_us"])
-        gemm_tflops = 2.0 * M * N * K / (gemm_us * 1e-6) / 1e12
-        fp4_peak = peaks["bf16"] * FP4_OVER_BF16
-        q_bytes_x, q_bytes_g = 2.5625 * M * K, 2.5625 * M * N
+        gemm_tflops = gemm_flop / (gemm_us * 1e-6) / 1e12
         cpu_flops, cpu_times = oracle_sample(M, 2)
         cpu_val = cpu_flops / (sum(cpu_times) / 2) / 1e12
         out = {
@@ -396,7 +472,8 @@ def run_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "nvfp4 (e2m1 x ue4m3, fp32 accumulate) + bf16 low-rank", "data": "synthetic",
             "config": {"workload": w["name"], "M": M, "K": K, "N": N, "r_s": r_s, "r": r, "tokens_per_gpu": M,
-                       "launch": launch, "l2": "step working set ~330 MB > 126 MB L2; per-kernel timings evict L2 by reading 256 MB",
+                       "launch": launch, "l2": "step working set ~330 MB > 126 MB L2; per-kernel timings cycle over input "
+                                                "copies that together exceed 2 x L2",
                        "parallelism": "dp%d (tokens), all-reduce of dA,dB only" % world,
                        "peaks": peaks["source"]},
             "clocks": clocks,
@@ -406,24 +483,27 @@ def run_ours(args):
                            "dB^T copied back every step; copies on two side streams with double-buffered device tensors "
                            "(H2D of step i+1 and D2H of step i-1 overlap the kernels of step i); PCIe-bound"},
             "gpu_launches": KERNELS_PER_STEP * args.steps,
-            "roofline": {"kernel": "k_gemm4 (mean of fwd and dgrad launches)", "bound": "tensor",
-                         "achieved": gemm_tflops, "peak": fp4_peak, "unit": "TFLOP/s", "frac": gemm_tflops / fp4_peak,
-                         "peak_note": "measured bf16 burst %.1f x nominal fp4/bf16 ratio 4 (of %s); nominal 9000"
-                                      % (peaks["bf16"], peaks["source"]),
-                         "traffic": GEMM_DRAM_TRAFFIC_BYTES},
+            "roofline": {"kernel": "k_gemm4_pair (mean of the forward and the dgrad launch: the dominant kernel, %.0f %% of "
+                                   "the step)" % (100.0 * (kern["gemm_fwd_us"] + kern["gemm_dgrad_us"]) / (ms_per_step * 1e3)),
+                         "bound": "tensor", "achieved": gemm_tflops, "peak": FP4_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                         "frac": gemm_tflops / FP4_NOMINAL_TFLOPS,
+                         "peak_note": "nominal dense NVFP4 peak of B200 (B200_PROFILING.md); MEASURED_PEAKS.json holds no FP4 "
+                                      "figure, so two measured ceilings are reported beside it",
+                         "frac_of_probe": (gemm_tflops / fp4_probe) if fp4_probe else None,
+                         "frac_of_derived": gemm_tflops / fp4_derived,
+                         "derived_peak": fp4_derived,
+                         "derived_note": "measured bf16 burst %.1f x nominal fp4/bf16 ratio 4 (of %s)" % (peaks["bf16"], peaks["source"]),
+                         "traffic": NCU_DRAM_TRAFFIC["gemm_fwd"]},
+            "roofline_kernels": roofs,
+            "fp4_probe": probe,
             "kernels_us": {k: round(v, 2) for k, v in kern.items()},
-            "quantize": {"X_GBps": q_bytes_x / kern["amax_quant_X_single_pass_us"] / 1e3,
-                         "G_GBps": q_bytes_g / kern["quant_G_us"] / 1e3,
-                         "frac_of_hbm_X": q_bytes_x / kern["amax_quant_X_single_pass_us"] / 1e3 / peaks["hbm"],
-                         "frac_of_hbm_G": q_bytes_g / kern["quant_G_us"] / 1e3 / peaks["hbm"],
-                         "bytes_per_element": 2.5625, "hbm_peak_GBps": peaks["hbm"],
-                         "note": "X: a0 + a1 in ONE kernel (tensor read once, amax found inside); G: a3 with the amax "
-                                 "from the dB^T pass, k_quantize_fused + k_finalize_h; isolated launches, ~6 us of "
-                                 "each figure is launch overhead"},
+            "kernels_us_note": "CUDA graph of back-to-back launches cycling over input copies (> 2 x L2 in total), replayed 20 "
+                               "times: kernel-to-kernel time; step_eager_us = the same step without a graph",
             "bf16_lora_baseline": {"us_per_step": bf16_us, "speedup": bf16_us / (ms_per_step * 1e3),
-                                   "how": "torch.matmul (cuBLAS) bf16, frozen W, same shapes, same GPU"},
+                                   "how": "torch.matmul (cuBLAS) bf16, frozen W, same shapes, same GPU, same protocol "
+                                          "(CUDA graph, back-to-back replays)"},
             "saved4_activations": {
-                "wgrad_bf16_x_us": round(kern["wgrad_us"], 2), "wgrad_saved4_us": round(kern["wgrad_saved4_us"], 2),
+                "wgrad_bf16_x_us": round(kern["wgrad_dA_dBt_us"], 2), "wgrad_saved4_us": round(kern["wgrad_saved4_us"], 2),
                 "step_us": round(kern["step_saved4_us"], 2), "step_bf16_x_us": round(kern["step_bf16x_us"], 2),
                 "saved_bytes_per_layer_bf16": 2 * M * K, "saved_bytes_per_layer_4bit": int(0.5625 * M * K),
                 "note": "NEXT-2: ft_lora_wgrad_q4 takes dA = dequant(Q(X))^T (G B^T) from the codes and scales the "
@@ -443,7 +523,7 @@ def run_ours(args):
 
 
 # ------------------------------------------------------------------ the other BASELINE.json configs
-def sweep(B, prepare, dev, timed, peaks, full=False):
+def sweep(B, prepare, dev, graph_us, peaks, full=False):
     """C4 (quantizer-only sweep; always) and, with --sweep, C1 / C3 / C5 layer timings.  Inputs are
     torch-generated on the device with the configs' shapes (N(0,1) with 1 % channels x50; gradients
     1e-3 N(0,1)): throughput does not depend on the values; parity on these shapes is in tests/."""
@@ -462,27 +542,34 @@ def sweep(B, prepare, dev, timed, peaks, full=False):
     out = {}
     c4 = []
     for rows, cols in ((4608, 3072), (4608, 12288), (4608, 15360), (9216, 3072)):
-        x = acts(rows, cols)
+        ncopy = max(2, int(300e6 // (rows * cols * 2)) + 1)          # together > 2 x L2: every launch reads HBM
+        xs = [acts(rows, cols) for _ in range(ncopy)]
         q = B.QTensor(rows, cols, device=dev)
         ws = B.new_workspace(rows, cols, 0, 32, dev)
-        amax = B.ft_tensor_amax(x)
+        amax = B.ft_tensor_amax(xs[0])
         d = (torch.randn(cols, 32, device=dev, generator=g) * 0.01).to(torch.bfloat16)
         h = torch.empty(rows, 32, dtype=torch.bfloat16, device=dev)
-        t_a = timed(lambda: B.ft_tensor_amax(x, amax))
-        t_q = timed(lambda: B.ft_quantize_blockwise(x, q, tensor_amax=amax, workspace=ws))
-        t_p = timed(lambda: B.ft_quantize_blockwise(x, q, tensor_amax=amax, down=d, h_out=h, workspace=ws))
-        t_f = timed(lambda: B.ft_quantize_blockwise(x, q, down=d, h_out=h, workspace=ws))   # a0 + a1 in one call
+        t_a = graph_us([lambda x=x: B.ft_tensor_amax(x, amax) for x in xs])
+        amax = B.ft_tensor_amax(xs[0])
+        t_q = graph_us([lambda x=x: B.ft_quantize_blockwise(x, q, tensor_amax=amax, workspace=ws) for x in xs])
+        t_p = graph_us([lambda x=x: B.ft_quantize_blockwise(x, q, tensor_amax=amax, down=d, h_out=h, workspace=ws) for x in xs])
+        t_f = graph_us([lambda x=x: B.ft_quantize_blockwise(x, q, down=d, h_out=h, workspace=ws) for x in xs])   # a0 + a1, one call
         by = 2.5625 * rows * cols
+        byp = by + 4.0 * 32 * rows            # + H (bf16) and the D slices, once per row tile pass: 4 r_t / cols per element
         c4.append({"shape": [rows, cols], "amax_us": round(t_a, 2), "amax_GBps": round(2.0 * rows * cols / t_a / 1e3),
                    "quant_us": round(t_q, 2), "quant_GBps": round(by / t_q / 1e3),
-                   "quant_proj32_us": round(t_p, 2), "quant_proj32_GBps": round(by / t_p / 1e3),
+                   "quant_proj32_us": round(t_p, 2), "quant_proj32_GBps": round(byp / t_p / 1e3),
                    "amax_quant_proj32_one_call_us": round(t_f, 2),
                    "frac_of_hbm": round(by / t_q / 1e3 / peaks["hbm"], 3),
-                   "frac_of_hbm_proj32": round(by / t_p / 1e3 / peaks["hbm"], 3)})
-        del x, q, ws, d, h
+                   "frac_of_hbm_proj32": round(byp / t_p / 1e3 / peaks["hbm"], 3),
+                   "frac_of_nominal_8TBps_proj32": round(byp / t_p / 1e3 / 8000.0, 3)})
+        del xs, q, ws, d, h
+        torch.cuda.empty_cache()
     out["C4_quantizer_sweep"] = {"bytes_per_element": 2.5625, "hbm_peak_GBps": peaks["hbm"],
-                                 "note": "each launch timed alone (CUDA events, L2 evicted); ~6 us of every figure is "
-                                         "launch overhead of the isolated measurement", "cases": c4}
+                                 "note": "amax given (except the one-call column); each call captured back to back in one "
+                                         "CUDA graph over input copies that together exceed 2 x L2, replayed 20 times: "
+                                         "kernel-to-kernel time of k_quantize_fused (+ k_finalize_h with the projection)",
+                                 "cases": c4}
     if not full:
         return out
 
@@ -505,23 +592,7 @@ def sweep(B, prepare, dev, timed, peaks, full=False):
         def step():
             B.ft_linear_fwd(layer, X, y, h, qx, ws)
             B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws)
-        for _ in range(3):
-            step()
-        torch.cuda.synchronize()
-        gr = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(gr):
-            step()
-        for _ in range(3):
-            gr.replay()
-        torch.cuda.synchronize()
-        n = 20
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        for _ in range(n):
-            gr.replay()
-        b.record()
-        torch.cuda.synchronize()
-        ours = a.elapsed_time(b) / n * 1e3
+        ours = graph_us([step], 20)
         A_, B_ = D_f[:, r_s:].contiguous(), U_t[:, r_s:].t().contiguous()
 
         def bf16():
@@ -531,14 +602,7 @@ def sweep(B, prepare, dev, timed, peaks, full=False):
             G @ W + gb @ A_.t()
             X.t() @ gb
             xa.t() @ G
-        for _ in range(2):
-            bf16()
-        a.record()
-        for _ in range(5):
-            bf16()
-        b.record()
-        torch.cuda.synchronize()
-        base = a.elapsed_time(b) / 5 * 1e3
+        base = graph_us([bf16], 5)            # the same protocol for the baseline: CUDA graph, back-to-back replays
         return ours, base
 
     out["fusion_ablation_C2"] = fusion_ablation(B, dev, acts, g)
@@ -562,7 +626,8 @@ def sweep(B, prepare, dev, timed, peaks, full=False):
                      "bf16_lora_us": round(base, 1)})
         torch.cuda.empty_cache()
     out["C5_dit_linear_layers"] = {"layers": 228, "distinct_shapes": rows, "how": "each distinct (M,K,N) timed once "
-                                   "(CUDA graph, 20 replays back to back) and multiplied by its count",
+                                   "(CUDA graph, 20 replays back to back; the bf16 baseline the same way) and multiplied by "
+                                   "its count",
                                    "fwd_bwd_ms": round(tot_ours / 1e3, 2), "TFLOPs": round(tot_flop / tot_ours / 1e6, 1),
                                    "bf16_lora_ms": round(tot_base / 1e3, 2),
                                    "speedup_vs_bf16_lora": round(tot_base / tot_ours, 2)}
@@ -630,8 +695,9 @@ def fusion_ablation(B, dev, acts, g):
         res[name] = round(a.elapsed_time(b) / 20 * 1e3, 1)
     res["fusion_speedup"] = round(res["unfused_4bit_us"] / res["fused_us"], 2)
     res["note"] = ("both arms as CUDA graphs; unfused = k_amax, quantize without projection, cuBLAS bf16 down-/up-"
-                   "projections, elementwise adds, the same 4-bit GEMM kernel; paper (other GPUs, whole DiT): LoRA "
-                   "fusion 1.82x (PAPER.md:245)")
+                   "projections, elementwise adds, the same 4-bit GEMM kernel: a TIMING shape only, its outputs are "
+                   "UNCHECKED (it does not pre-scale H, so its numbers are not the library's); paper (other GPUs, whole "
+                   "DiT): LoRA fusion 1.82x (PAPER.md:245)")
     return res
 
 
@@ -646,6 +712,8 @@ def main():
                                                          "C5 layer list: adds ~25 s")
     ap.add_argument("--c4-only", dest="c4_only", action="store_true", help="of the other configs, time only the C4 sweep")
     ap.add_argument("--no-sweep", dest="no_sweep", action="store_true", help="time the C2 step only")
+    ap.add_argument("--probe-seconds", dest="probe_seconds", type=float, default=1.5,
+                    help="duration of the sustained FP4 tensor-core probe (0 = skip)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

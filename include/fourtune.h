@@ -25,7 +25,7 @@
  *    the structs themselves are host memory, read during the call only.
  *  - the caller owns every buffer; the library never allocates, frees or keeps
  *    a pointer after the call returns.  Scratch comes from `workspace`, a device buffer of at least
- *    ft_workspace_bytes() bytes whose first 4 KB hold control words that must be ZERO when a call starts:
+ *    ft_workspace_bytes() bytes whose first 36 KB hold control words that must be ZERO when a call starts:
  *    zero-fill the buffer once (or call ft_workspace_init); every call leaves them zero again (the kernels
  *    put each word back when they are done with it), so no clearing runs per call.  One workspace serves any
  *    number of stream-ordered calls of any shapes, but not two calls that run concurrently.
@@ -66,7 +66,9 @@ typedef enum {
                              rows padded to 128, blocks to 4 (padding bytes are 0).  With
                              block_rows = 16 row r carries the scale of block r/16.      */
 
-#define FT_ROUND_NEAREST_EVEN 0 /* the only mode of the paper's reading O-6 */
+#define FT_ROUND_NEAREST_EVEN 0 /* reading O-6: what every layer call uses                                  */
+#define FT_ROUND_STOCHASTIC 1   /* reading O-6': the E2M1 codes by stochastic rounding, the
+                                   scales unchanged; ft_quantize_blockwise only (see there)              */
 
 /* A quantized tensor Q(T) of a logical [rows x cols] matrix, blocked along cols. */
 typedef struct {
@@ -125,11 +127,18 @@ int ft_tensor_amax(const void* x_bf16, int64_t n, float* amax_out, void* stream)
  *   workspace may be NULL only if tensor_amax != NULL and proj == NULL.
  * proj: NULL => quantize only.  Requires out->block_rows == 1 if non-NULL.
  * Requirements: cols % 64 == 0; rows % 16 == 0 if block_rows == 16; any rows >= 1
- *   otherwise.  out->rows/cols must equal rows/cols.  round_mode must be
- *   FT_ROUND_NEAREST_EVEN.  workspace >= ft_workspace_bytes(rows, cols, 0, r_t). */
+ *   otherwise.  out->rows/cols must equal rows/cols.  workspace >= ft_workspace_bytes(rows, cols, 0, r_t).
+ * round_mode FT_ROUND_NEAREST_EVEN: seed and offset are ignored.
+ * round_mode FT_ROUND_STOCHASTIC (PAPER.md:59 writes Round(W / s) without naming the mode; O-6'):
+ *   x_i * enc_b goes to the E2M1 neighbour above with probability (|v| - lo) / (hi - lo), else to the one below:
+ *   hi iff u_i * (hi - lo) < |v| - lo, u_i = (word >> 8) * 2^-24 with word = output[idx % 4] of
+ *   Philox4x32-10(counter = (lo, hi, 0, 0) of offset + idx / 4, key = (lo, hi) of seed), idx = row * cols + col.
+ *   Counter-based: a caller that quantizes a tensor in row slices passes offset + first_row * cols / 4 and gets
+ *   the bits of the whole-tensor call.  Requires out->block_rows == 1 and proj == NULL (a plain kernel, not the
+ *   fused one: the mode is a variant for gradients, not the hot path). */
 int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols,
                           const float* tensor_amax, const ft_proj* proj,
-                          ft_qtensor* out, int32_t round_mode,
+                          ft_qtensor* out, int32_t round_mode, uint64_t seed, uint64_t offset,
                           void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---- a6 helper: build Q(R)^T ([K x N], N contiguous) from Q(R) ([N x K]) by
@@ -172,9 +181,9 @@ int ft_gemm4(const ft_qtensor* a, const ft_qtensor* b, const void* lr_a_scaled, 
 /* ---- a5: LoRA weight gradients (Eq. 4), fp32.
  * dA  [K x r]  = X^T  * P[:, r_s:]      dBt [N x r] = G^T * H[:, r_s:]  (= dB^T)
  * h_saved / p_saved are the [M x r_t] outputs of the two calls above.
- * accumulate: 0 overwrite, 1 add to the existing contents.  This call has no workspace: partial sums over
- * slices of M are combined with fp32 atomics, so the order of additions is not fixed (ft_linear_bwd combines
- * them through its workspace in a fixed order instead). */
+ * accumulate: 0 overwrite, 1 add to the existing contents.  Partial sums over slices of M are added in a fixed
+ * order (the same bits on every run): this call, which has no workspace, combines them over distributed shared
+ * memory inside a thread-block cluster; ft_linear_bwd combines them through its workspace. */
 int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
                   const void* h_saved_bf16, const void* p_saved_bf16, float* dA,
                   float* dBt, int32_t accumulate, void* stream);
@@ -214,7 +223,7 @@ int ft_linear_bwd_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
 size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout);
 size_t ft_sf_ntile_bytes(int64_t rows, int64_t cols, int32_t ntile);   /* ft_qtensor::sf_ntile */
 size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t);
-/* Zero the control words at the head of a workspace (one 4 KB memset on `stream`).  Needed once per buffer,
+/* Zero the control words at the head of a workspace (one 36 KB memset on `stream`).  Needed once per buffer,
  * before its first use, unless the caller zero-filled it; never per call.  Also the way to recover a workspace
  * after a call was aborted by a CUDA error. */
 int ft_workspace_init(void* workspace, size_t workspace_bytes, void* stream);

@@ -137,3 +137,51 @@ def wgrad_saved4(qX, G, H, P, r_s):
         dA[k,j] = sum_m (E2M1(code[m,k]) * sf[m,k/16] * g_dec) * P[m, r_s+j]
     dB is unchanged (it never touches X).  float64 sums, float32 results."""
     return wgrad(nvfp4.dequantize(qX), G, H, P, r_s)
+
+
+# ---------------------------------------------------------------- NEXT-1: MLP fusion (PAPER.md:112-114, sec. 3.3)
+# "we fuse the first fully connected (FC1) GEMM with the subsequent FC2 quantization kernel.  This approach allows
+#  intermediate results to be consumed immediately without materializing large tensors in global memory".
+# The paper names GeLU and says nothing else; reading O-16 of DESIGN.md pins the rest:
+#   * GeLU is the tanh form (FLUX's MLP), evaluated on the bf16-rounded FC1 output Y1, and rounded to bf16: Z;
+#   * Q(Z) (1x16 blocks along FC2's reduction dim) takes its tensor amax from the CALLER (delayed scaling: the
+#     value of the previous step; the epilogue of a GEMM cannot know max|Z| before its last tile), and so does the
+#     second quantized tensor the block keeps, Q(Y1), the pre-activation that GeLU's backward consumes;
+#   * FC2's low-rank branches consume the bf16 Z (O-10 unchanged): H2 = bf16(Z D_f2);
+#   * backward: dY1 = bf16( dZ * gelu'(dequant(Q(Y1))) ), dZ the bf16 dgrad of FC2; FC2's dA uses dequant(Q(Z))
+#     (reading O-12', since the bf16 Z is never materialized).
+# The fused forward is BY DEFINITION the composition of the two layer forwards with that quantizer in between:
+# mlp_forward below is written as that composition, so "fused == unfused" holds by construction and the CUDA
+# kernel is what has to match it.
+
+def gelu_tanh(y):
+    """GeLU, tanh form: 0.5 y (1 + tanh( sqrt(2/pi) (y + 0.044715 y^3) )), float64."""
+    y = np.asarray(y, dtype=np.float64)
+    return 0.5 * y * (1.0 + np.tanh(np.sqrt(2.0 / np.pi) * (y + 0.044715 * y * y * y)))
+
+
+def gelu_tanh_grad(y):
+    """d/dy of gelu_tanh, float64:  0.5 (1 + t) + 0.5 y (1 - t^2) sqrt(2/pi) (1 + 3 * 0.044715 y^2),  t = tanh(.)."""
+    y = np.asarray(y, dtype=np.float64)
+    c = np.sqrt(2.0 / np.pi)
+    t = np.tanh(c * (y + 0.044715 * y * y * y))
+    return 0.5 * (1.0 + t) + 0.5 * y * (1.0 - t * t) * c * (1.0 + 3.0 * 0.044715 * y * y)
+
+
+def mlp_forward(X, qR1, D1, U1, qR2, D2, U2, z_amax, y1_amax, Y1_given=None, Z_given=None, H1s_given=None,
+                H2s_given=None):
+    """FC1 -> GeLU -> FC2 under reading O-16 (pre-scaled low-rank intermediates, O-10').
+    *_given: bf16 values produced by the CUDA path that replace the oracle's own at that point (the staged
+    comparison of DESIGN.md O-11: each stage is checked on its own, then fed forward bit for bit).
+    Returns Y1, Z (bf16), qZ, qY1, Y2, and the two layer dicts."""
+    f1 = forward(X, qR1, D1, U1, prescale=True, H_given=H1s_given)
+    Y1 = f1["Y"] if Y1_given is None else np.asarray(Y1_given, np.float32)
+    Z = bf16_round_from_f64(gelu_tanh(Y1)) if Z_given is None else np.asarray(Z_given, np.float32)
+    qY1 = nvfp4.quantize_blockwise(Y1, block_rows=1, block_cols=16, amax_t=y1_amax)
+    f2 = forward(Z, qR2, D2, U2, prescale=True, x_amax=z_amax, H_given=H2s_given)
+    return {"Y1": Y1, "Z": Z, "qZ": f2["qX"], "qY1": qY1, "Y2": f2["Y"], "fc1": f1, "fc2": f2}
+
+
+def gelu_backward_saved4(dZ, qY1):
+    """dY1 = bf16( dZ * gelu'(dequant(Q(Y1))) ): GeLU's backward on the 4-bit saved pre-activation (O-16)."""
+    return bf16_round_from_f64(np.asarray(dZ, np.float64) * gelu_tanh_grad(nvfp4.dequantize(qY1)))

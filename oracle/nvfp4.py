@@ -160,11 +160,74 @@ def tensor_amax(x):
     return F32(np.max(np.abs(x))) if x.size else F32(0.0)
 
 
+# ------------------------------ O-6': stochastic rounding of the element codes (NEXT-4 variant)
+
+PHILOX_M0, PHILOX_M1 = np.uint64(0xD2511F53), np.uint64(0xCD9E8D57)
+PHILOX_W0, PHILOX_W1 = np.uint32(0x9E3779B9), np.uint32(0xBB67AE85)
+
+
+def philox4x32_10(counter, key):
+    """Philox4x32-10 (Salmon, Moraes, Dror, Shaw: "Parallel random numbers: as easy as 1, 2, 3", SC'11), the
+    counter-based generator both the oracle and the CUDA kernel implement, each on its own.
+    counter: uint32 [..., 4], key: uint32 [2] -> uint32 [..., 4].  Ten rounds of
+        hi0:lo0 = M0 * c0,  hi1:lo1 = M1 * c2,   c = (hi1 ^ c1 ^ k0, lo1, hi0 ^ c3 ^ k1, lo0),   k += (W0, W1)."""
+    c = np.array(counter, dtype=np.uint32, copy=True)
+    k0, k1 = np.uint32(key[0]), np.uint32(key[1])
+    m32 = np.uint64(0xFFFFFFFF)
+    with np.errstate(over="ignore"):
+        for _ in range(10):
+            p0 = PHILOX_M0 * c[..., 0].astype(np.uint64)
+            p1 = PHILOX_M1 * c[..., 2].astype(np.uint64)
+            hi0, lo0 = (p0 >> np.uint64(32)).astype(np.uint32), (p0 & m32).astype(np.uint32)
+            hi1, lo1 = (p1 >> np.uint64(32)).astype(np.uint32), (p1 & m32).astype(np.uint32)
+            c = np.stack([hi1 ^ c[..., 1] ^ k0, lo1, hi0 ^ c[..., 3] ^ k1, lo0], axis=-1)
+            k0, k1 = np.uint32(k0 + PHILOX_W0), np.uint32(k1 + PHILOX_W1)
+    return c
+
+
+def sr_uniforms(n_elements, seed, offset):
+    """One uniform u in [0, 1) per element of a tensor, in linear (row-major) element order: element idx takes
+    word idx % 4 of philox4x32_10(counter = (lo, hi, 0, 0) of the 64-bit value offset + idx // 4, key = (lo, hi) of
+    the 64-bit seed), and u = (word >> 8) * 2**-24 (24 bits: exact in float32).  n_elements % 4 == 0."""
+    assert n_elements % 4 == 0
+    ctr = np.uint64(offset) + np.arange(n_elements // 4, dtype=np.uint64)
+    counter = np.zeros((n_elements // 4, 4), dtype=np.uint32)
+    counter[:, 0] = (ctr & np.uint64(0xFFFFFFFF)).astype(np.uint32)
+    counter[:, 1] = (ctr >> np.uint64(32)).astype(np.uint32)
+    key = (np.uint32(np.uint64(seed) & np.uint64(0xFFFFFFFF)), np.uint32(np.uint64(seed) >> np.uint64(32)))
+    words = philox4x32_10(counter, key).reshape(-1)
+    return ((words >> np.uint32(8)).astype(np.float32) * np.float32(2.0 ** -24)).astype(np.float32)
+
+
+def e2m1_encode_stochastic(v, u):
+    """Stochastic rounding onto the E2M1 grid (reading O-6' of DESIGN.md): with lo <= |v| < hi the neighbouring
+    magnitudes, the result is hi with probability (|v| - lo) / (hi - lo) and lo otherwise -- decided by
+    `u * (hi - lo) < |v| - lo` on the element's uniform u -- so that E[dequant] = v (unbiased) inside the grid.
+    |v| >= 6 saturates to 6; a value already on the grid is kept (|v| - lo = 0); the sign bit is the input's.
+    Every quantity is exact in float32 (|v| - lo by Sterbenz, hi - lo a power of two, u a 24-bit fraction)."""
+    v = np.asarray(v, dtype=np.float32)
+    u = np.asarray(u, dtype=np.float32)
+    mag = np.abs(v).astype(np.float64)
+    grid = E2M1_VALUES
+    lo_idx = np.clip(np.searchsorted(grid, mag, side="right") - 1, 0, 7)      # largest grid value <= |v|
+    lo = grid[lo_idx]
+    hi = grid[np.minimum(lo_idx + 1, 7)]
+    step = hi - lo                                                            # 0 at the top of the grid
+    up = (u.astype(np.float64) * step < mag - lo) & (lo_idx < 7)
+    code = (lo_idx + up).astype(np.uint8)
+    sign = np.signbit(v).astype(np.uint8)
+    return (code | (sign << 3)).astype(np.uint8)
+
+
 # ------------------------------------------------------ Q4: per-block quantize
 
 
-def quantize_blockwise(x, block_rows=1, block_cols=16, amax_t=None):
+def quantize_blockwise(x, block_rows=1, block_cols=16, amax_t=None, round_mode="nearest", seed=0, offset=0):
     """Q(.) of DESIGN.md Q3-Q5 on a [rows, cols] float32 array of bf16 values.
+
+    round_mode "nearest" (reading O-6, the default) or "stochastic" (O-6', the NEXT-4 variant for gradients):
+    the scales are computed the same way; only the last line changes to
+        code_i = E2M1_stochastic(float(x_i) * enc_b, u_i),  u_i = sr_uniforms(...)[row * cols + col].
 
     Blocks are block_rows x block_cols (1x16 for X and G along the reduction
     dim, 16x16 for the residual weights R; O-2).  Every float32
@@ -202,7 +265,13 @@ def quantize_blockwise(x, block_rows=1, block_cols=16, amax_t=None):
         enc_b = np.where(sf8 == 0, F32(0.0), F32(1.0) / prod).astype(np.float32)
     with np.errstate(over="ignore", invalid="ignore"):
         scaled = (xb * enc_b[:, None, :, None]).astype(np.float32)
-    codes = e2m1_encode(scaled).reshape(rows, cols)
+    if round_mode == "nearest":
+        codes = e2m1_encode(scaled).reshape(rows, cols)
+    elif round_mode == "stochastic":
+        u = sr_uniforms(rows * cols, seed, offset).reshape(nbr, block_rows, nbc, block_cols)
+        codes = e2m1_encode_stochastic(scaled, u).reshape(rows, cols)
+    else:
+        raise ValueError(round_mode)
     return {
         "codes": codes,
         "packed": pack_codes(codes),

@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libfourtune.so")
 
 FT_SF_ROWMAJOR, FT_SF_TILE128x4 = 0, 1
-FT_ROUND_NEAREST_EVEN = 0
+FT_ROUND_NEAREST_EVEN, FT_ROUND_STOCHASTIC = 0, 1
 
 
 class FtError(RuntimeError):
@@ -50,7 +50,8 @@ def lib():
         L = C.CDLL(LIB_PATH)
         vp, i64, i32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_size_t
         L.ft_tensor_amax.argtypes = [vp, i64, vp, vp]
-        L.ft_quantize_blockwise.argtypes = [vp, i64, i64, vp, C.POINTER(_Proj), C.POINTER(_QT), i32, vp, sz, vp]
+        L.ft_quantize_blockwise.argtypes = [vp, i64, i64, vp, C.POINTER(_Proj), C.POINTER(_QT), i32, C.c_uint64, C.c_uint64,
+                                            vp, sz, vp]
         L.ft_pack_weight.argtypes = [C.POINTER(_QT), C.POINTER(_QT), C.POINTER(_QT), vp]
         L.ft_linear_fwd.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
         L.ft_linear_bwd_dgrad.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
@@ -157,8 +158,10 @@ def ft_tensor_amax(x, out=None, stream=None):
 
 
 def ft_quantize_blockwise(x, out, tensor_amax=None, down=None, h_out=None, hs_out=None,
-                          other_dec_scale=None, workspace=None, stream=None):
-    """x [rows x cols] bf16 -> out (QTensor).  down [cols x r_t] enables the fused projection."""
+                          other_dec_scale=None, workspace=None, stream=None, round_mode=FT_ROUND_NEAREST_EVEN,
+                          seed=0, offset=0):
+    """x [rows x cols] bf16 -> out (QTensor).  down [cols x r_t] enables the fused projection.
+    round_mode=FT_ROUND_STOCHASTIC: stochastic rounding of the codes from the Philox stream (seed, offset)."""
     _bf16(x)
     rows, cols = x.shape
     if workspace is None:
@@ -172,7 +175,7 @@ def ft_quantize_blockwise(x, out, tensor_amax=None, down=None, h_out=None, hs_ou
     q = out.c()
     _check(lib().ft_quantize_blockwise(_ptr(x), rows, cols, _ptr(tensor_amax),
                                        None if proj is None else C.byref(proj), C.byref(q),
-                                       FT_ROUND_NEAREST_EVEN, _ptr(workspace), workspace.numel(),
+                                       round_mode, seed, offset, _ptr(workspace), workspace.numel(),
                                        _stream(stream)))
     return out
 

@@ -151,6 +151,98 @@ __global__ void __launch_bounds__(256) k_quantize_generic(
   }
 }
 
+// ------------------------------- stochastic rounding of the element codes (NEXT-4 variant, O-6')
+// Philox4x32-10 (Salmon et al., SC'11): counter (c0..c3), key (k0, k1), ten rounds.  Written from the paper's
+// round function; the oracle has its own copy (no shared code), both pinned by the published known answers.
+__device__ __forceinline__ uint4 philox4x32_10(uint4 c, uint2 k) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+    c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+    k.x += 0x9E3779B9u;
+    k.y += 0xBB67AE85u;
+  }
+  return c;
+}
+// v -> the E2M1 neighbour below |v| or the one above, the latter iff u * (hi - lo) < |v| - lo with u = (word >> 8) *
+// 2^-24; returned as a float on the grid carrying v's sign (the hardware convert then packs it exactly).  Every
+// operation is exact in fp32: lo is |v| with all but the top mantissa bit cleared (the grid above 1 has one mantissa
+// bit), hi - lo a power of two, |v| - lo within a factor of two of |v|.
+__device__ __forceinline__ float e2m1_sr(float v, uint32_t word) {
+  const float mag = fabsf(v);
+  const uint32_t b = __float_as_uint(mag);
+  const float u = __uint2float_rn(word >> 8) * 5.9604644775390625e-8f;   // 24 bits: exact
+  float lo, step;
+  if (mag >= 1.0f) {
+    lo = __uint_as_float(b & 0xFFC00000u);
+    step = __uint_as_float((b & 0x7F800000u) - 0x00800000u);
+  } else {
+    lo = mag >= 0.5f ? 0.5f : 0.0f;
+    step = 0.5f;
+  }
+  const float r = (__fmul_rn(u, step) < __fsub_rn(mag, lo)) ? __fadd_rn(lo, step) : lo;   // >= 6 saturates in the convert
+  return copysignf(r, v);
+}
+
+// One thread per 1x16 block: the scales exactly as in the nearest-rounding quantizer (Q3, Q4), the codes by
+// e2m1_sr on x_i * enc_b with the uniform of element idx = row * cols + col: word idx % 4 of
+// philox4x32_10(counter = offset + idx / 4, key = seed).
+__global__ void __launch_bounds__(256) k_quantize_sr(
+    const uint4* __restrict__ x, int64_t rows, int64_t cols, const float* __restrict__ amax_t,
+    uint8_t* __restrict__ codes, uint8_t* __restrict__ sf, float* __restrict__ g_dec_out, int sf_layout,
+    uint64_t seed, uint64_t offset) {
+  const int64_t nblk = cols / 16;
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const TensorScale ts = tensor_scale(__ldg(amax_t));
+  const int64_t bc = t % nblk, row = t / nblk;
+  if (row >= rows) return;
+  if (t == 0) *g_dec_out = ts.g_dec;
+  const uint4* src = x + (row * cols + bc * 16) / 8;
+  const uint4 v0 = __ldg(src), v1 = __ldg(src + 1);
+  const float amax_b = fmaxf(amax_bf16x8(v0), amax_bf16x8(v1));
+  uint32_t sf8;
+  float enc_b;
+  block_scale(amax_b, ts, sf8, enc_b);
+  const uint32_t w[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+  const uint64_t ctr0 = offset + (uint64_t)(row * cols + bc * 16) / 4;
+  const uint2 key = make_uint2((uint32_t)seed, (uint32_t)(seed >> 32));
+  uint32_t packed[2];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {       // four elements (two words of the block) per Philox call
+    const uint64_t ctr = ctr0 + q;
+    const uint4 rnd = philox4x32_10(make_uint4((uint32_t)ctr, (uint32_t)(ctr >> 32), 0u, 0u), key);
+    const uint32_t wa = w[2 * q], wb = w[2 * q + 1];
+    const float f0 = e2m1_sr(__fmul_rn(__uint_as_float(wa << 16), enc_b), rnd.x);
+    const float f1 = e2m1_sr(__fmul_rn(__uint_as_float(wa & 0xFFFF0000u), enc_b), rnd.y);
+    const float f2 = e2m1_sr(__fmul_rn(__uint_as_float(wb << 16), enc_b), rnd.z);
+    const float f3 = e2m1_sr(__fmul_rn(__uint_as_float(wb & 0xFFFF0000u), enc_b), rnd.w);
+    uint32_t two;
+    asm("{\n\t.reg .b8 b0, b1;\n\t"
+        "cvt.rn.satfinite.e2m1x2.f32 b0, %2, %1;\n\t"
+        "cvt.rn.satfinite.e2m1x2.f32 b1, %4, %3;\n\t"
+        "mov.b32 %0, {b0, b1, 0, 0};\n\t}"
+        : "=r"(two) : "f"(f0), "f"(f1), "f"(f2), "f"(f3));
+    if (q & 1) packed[q >> 1] |= two << 16;
+    else packed[q >> 1] = two;
+  }
+  *reinterpret_cast<uint2*>(codes + row * (cols / 2) + bc * 8) = make_uint2(packed[0], packed[1]);
+  if (sf_layout == FT_SF_TILE128x4) sf[sf_tile_offset(row, bc, nblk)] = (uint8_t)sf8;
+  else sf[row * nblk + bc] = (uint8_t)sf8;
+}
+
+int launch_quantize_sr(const void* x, int64_t rows, int64_t cols, const float* amax_t, ft_qtensor* out,
+                       uint64_t seed, uint64_t offset, cudaStream_t st) {
+  const int64_t threads = rows * (cols / 16);
+  if (out->sf_layout == FT_SF_TILE128x4)
+    FT_CUDA_TRY(cudaMemsetAsync(out->sf, 0, ft_sf_bytes(rows, cols, 1, FT_SF_TILE128x4), st));
+  k_quantize_sr<<<(unsigned)ceil_div(threads, 256), 256, 0, st>>>(reinterpret_cast<const uint4*>(x), rows, cols, amax_t,
+                                                                  out->codes, out->sf, out->tensor_dec_scale,
+                                                                  out->sf_layout, seed, offset);
+  FT_CUDA_TRY(cudaGetLastError());
+  return FT_OK;
+}
+
 int launch_quantize_generic(const void* x, int64_t rows, int64_t cols, const float* amax_t,
                             ft_qtensor* out, cudaStream_t st) {
   const int64_t threads = rows * (cols / 16);

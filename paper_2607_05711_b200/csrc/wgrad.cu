@@ -19,25 +19,47 @@
 
 namespace ft {
 
-constexpr int WG_F = 128;
-constexpr int WG_MC = 64;
-constexpr int WG_STAGES = 4;
+constexpr int WG_MC = 64;         // rows of M per ring stage
 constexpr int WG_THREADS = 128;
-constexpr int WG_IN_BYTES = 2 * WG_MC * 128;  // two 64-feature boxes
 constexpr int WG_LG_BYTES = WG_MC * 128;      // one 64-column group of L
+// Two shapes of the same kernel.
+//   SLOTS (FW = 128 features per CTA, 3 stages of 20 KB, three CTAs per SM): a CTA's TMA stream runs at ~15 bytes per
+//     clock whatever its tile width or ring depth (measured: the same rate with no MMA and no amax work), so the
+//     pass needs ~400 CTAs in flight to reach the HBM rate; the M slices of a feature tile combine through slots of
+//     the caller's workspace (below).  Used by ft_linear_bwd.
+//   CLUSTER (FW = 256, ring as deep as shared memory allows, one CTA per SM -- the runtime co-schedules one CTA per
+//     SM of a cluster kernel that allocates tensor memory): the M slices of a feature tile are one cluster and
+//     combine over distributed shared memory.  Needs no workspace: used by ft_lora_wgrad.
+template <int R, int FW>
+struct WgCfg {
+  static constexpr int NG = (R + 63) / 64;
+  static constexpr int HALVES = FW / 128;                    // MMA halves of 128 features
+  static constexpr int IN_BYTES = (FW / 64) * WG_MC * 128;   // FW / 64 boxes of 64 features x 64 rows
+  static constexpr int STAGE_BYTES = IN_BYTES + NG * WG_LG_BYTES;
+  static constexpr int DEEP = (226 * 1024) / STAGE_BYTES > 6 ? 6 : (226 * 1024) / STAGE_BYTES;
+  static constexpr int STAGES = FW == 128 ? 3 : DEEP;
+  static constexpr int SMEM = STAGES * STAGE_BYTES + 1024;
+  static constexpr uint32_t HALF_COLS = R <= 32 ? 32 : (R <= 64 ? 64 : 128);   // TMEM columns of one 128-feature half
+  static_assert(FW == 128 || FW == 256, "feature tile");
+};
 
 struct WgParams {      // two problems in one launch: [0] dA = X^T P_lora, [1] dB^T = G^T H_lora
   int64_t M;
   int64_t F[2];
   int r_s, r;
-  int chunks_per_cta[2];
+  int chunks_per_cta;
   float* out[2];
   unsigned int* amax_bits[2];   // non-null: atomicMax target for max |In| (bf16 bits << 16), pre-zeroed
   int late_wait;                // 1: nothing this launch touches depends on its predecessor, which passes
                                 //    griddepcontrol.wait in every CTA before triggering: start beside it and
                                 //    wait for it at the END (completion stays transitive for the next launch)
-  int n_slices;                 // M slices = CTAs per cluster (gridDim.y); every slice has work
+  int n_slices;                 // M slices (gridDim.y); every slice has work
   int accumulate;               // add to the output instead of overwriting it
+  float* slots[2];              // SLOTS: partial tiles go to slot (feature tile * n_slices + slice), 128 x r fp32 each
+  uint32_t* counters[2];        //        one arrival counter per feature tile (zero between calls)
+#ifdef FT_TRACE
+  int dbg;                      // development builds: 1 = no MMAs, 2 = no amax fold
+#endif
 };
 
 __device__ __forceinline__ float4 ld_cluster_f4(uint32_t cluster_addr) {
@@ -47,32 +69,34 @@ __device__ __forceinline__ float4 ld_cluster_f4(uint32_t cluster_addr) {
   return v;
 }
 
-template <int R>
-__global__ void __launch_bounds__(WG_THREADS, 2)
+template <int R, int FW>
+__global__ void __launch_bounds__(WG_THREADS, FW == 128 ? 3 : 1)
 k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUtensorMap map_l0,
         const __grid_constant__ CUtensorMap map_in1, const __grid_constant__ CUtensorMap map_l1,
         const WgParams p) {
+  using Cfg = WgCfg<R, FW>;
+  constexpr int NG = Cfg::NG, HALVES = Cfg::HALVES, STAGE_BYTES = Cfg::STAGE_BYTES, WG_STAGES = Cfg::STAGES;
+  constexpr int IN_BYTES = Cfg::IN_BYTES;
+  constexpr uint32_t HALF_COLS = Cfg::HALF_COLS;
+  constexpr uint32_t TMEM_COLS = HALVES * HALF_COLS < 32 ? 32 : HALVES * HALF_COLS;
   const int z = blockIdx.z;
   const CUtensorMap& map_in = z == 0 ? map_in0 : map_in1;
   const CUtensorMap& map_l = z == 0 ? map_l0 : map_l1;
   const int64_t F = p.F[z];
-  const int cpc = p.chunks_per_cta[z];
+  const int cpc = p.chunks_per_cta;
   // CTAs beyond this problem's feature tiles have nothing to do (uniform per cluster: a cluster spans blockIdx.y
   // only).  Every M slice has work: the host sizes gridDim.y = ceil(chunks / chunks_per_cta).
-  if ((int64_t)blockIdx.x * WG_F >= F) return;
-  constexpr int NG = (R + 63) / 64;
-  constexpr int STAGE_BYTES = WG_IN_BYTES + NG * WG_LG_BYTES;
-  constexpr uint32_t TMEM_COLS = R <= 32 ? 32 : (R <= 64 ? 64 : 128);
+  if ((int64_t)blockIdx.x * FW >= F) return;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   __shared__ uint64_t full_bar[WG_STAGES], empty_bar[WG_STAGES], acc_bar;
   __shared__ uint32_t tmem_base_s;
+  __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int32_t f0 = (int32_t)blockIdx.x * WG_F;
+  const int32_t f0 = (int32_t)blockIdx.x * FW;
   const int64_t chunks_total = (p.M + WG_MC - 1) / WG_MC;
   const int64_t c_begin = (int64_t)blockIdx.y * cpc;
-  int n_chunks = (int)min((int64_t)cpc, chunks_total - c_begin);
-  if (n_chunks < 0) n_chunks = 0;
+  const int n_chunks = (int)min((int64_t)cpc, chunks_total - c_begin);   // >= 1
 
   if (tid == 0) {
     prefetch_tmap(&map_in);
@@ -106,31 +130,37 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
         uint8_t* base = smem + s * STAGE_BYTES;
         const int32_t m0 = (int32_t)((c_begin + it) * WG_MC);
         mbar_expect_tx(&full_bar[s], STAGE_BYTES);
-        if (keep) {
-          tma_load_2d_hint(base, &map_in, &full_bar[s], f0, m0, pol);
-          tma_load_2d_hint(base + WG_MC * 128, &map_in, &full_bar[s], f0 + 64, m0, pol);
-        } else {
-          tma_load_2d(base, &map_in, &full_bar[s], f0, m0);
-          tma_load_2d(base + WG_MC * 128, &map_in, &full_bar[s], f0 + 64, m0);
+#pragma unroll
+        for (int b = 0; b < FW / 64; ++b) {
+          if (keep) tma_load_2d_hint(base + b * (WG_MC * 128), &map_in, &full_bar[s], f0 + b * 64, m0, pol);
+          else tma_load_2d(base + b * (WG_MC * 128), &map_in, &full_bar[s], f0 + b * 64, m0);
         }
 #pragma unroll
         for (int g = 0; g < NG; ++g)
-          tma_load_2d(base + WG_IN_BYTES + g * WG_LG_BYTES, &map_l, &full_bar[s], p.r_s + g * 64, m0);
+          tma_load_2d(base + IN_BYTES + g * WG_LG_BYTES, &map_l, &full_bar[s], p.r_s + g * 64, m0);
       }
     }
   } else if (warp == 1) {
-    if (elect_one()) {   // ---- MMA issuer: acc[128 f x R] += In[64 m, 128 f]^T * L[64 m, R]
-      constexpr uint32_t idesc = idesc_bf16(WG_F, R) | (1u << 15) | (1u << 16);  // A and B MN-major
+    if (elect_one()) {   // ---- MMA issuer: acc_h[128 f x R] += In[64 m, 128 f of half h]^T * L[64 m, R]
+      constexpr uint32_t idesc = idesc_bf16(128, R) | (1u << 15) | (1u << 16);  // A and B MN-major
       for (int it = 0; it < n_chunks; ++it) {
         const int s = it % WG_STAGES;
         mbar_wait(&full_bar[s], (it / WG_STAGES) & 1);
         tc_fence_after();
         const uint32_t in_u = smem_u32(smem + s * STAGE_BYTES);
-        const uint32_t l_u = in_u + WG_IN_BYTES;
+        const uint32_t l_u = in_u + IN_BYTES;
+#ifdef FT_TRACE
+        if (p.dbg & 1) {
+          tc_commit(&empty_bar[s]);
+          continue;
+        }
+#endif
 #pragma unroll
-        for (int k = 0; k < 4; ++k)   // 16 rows of m per MMA = two 8-row swizzle groups = 2048 bytes
-          mma_bf16(tmem_base, make_smem_desc(in_u + k * 2048, 1024, WG_MC * 128, 2),
-                   make_smem_desc(l_u + k * 2048, 1024, WG_LG_BYTES, 2), idesc, (it | k) != 0);
+        for (int hf = 0; hf < HALVES; ++hf)
+#pragma unroll
+          for (int k = 0; k < 4; ++k)   // 16 rows of m per MMA = two 8-row swizzle groups = 2048 bytes
+            mma_bf16(tmem_base + hf * HALF_COLS, make_smem_desc(in_u + hf * (2 * WG_MC * 128) + k * 2048, 1024, WG_MC * 128, 2),
+                     make_smem_desc(l_u + k * 2048, 1024, WG_LG_BYTES, 2), idesc, (it | k) != 0);
         tc_commit(&empty_bar[s]);
       }
       tc_commit(&acc_bar);
@@ -145,7 +175,7 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
       mbar_wait(&full_bar[s], (it / WG_STAGES) & 1);
       const uint4* src = reinterpret_cast<const uint4*>(smem + s * STAGE_BYTES);
 #pragma unroll 4
-      for (int j = 0; j < WG_IN_BYTES / 16 / 64; ++j) {
+      for (int j = 0; j < IN_BYTES / 16 / 64; ++j) {
         const uint4 v = src[t64 + j * 64];
         acc = __vmaxu2(acc, __vmaxu2(__vmaxu2(v.x & m, v.y & m), __vmaxu2(v.z & m, v.w & m)));
       }
@@ -159,52 +189,65 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
   }
   __syncwarp();
 
-  {   // ---- drain: thread = feature (TMEM lane), R fp32 columns
+  {   // ---- drain: thread = feature (TMEM lane) of each 128-feature half, R fp32 columns
     mbar_wait(&acc_bar, 0);   // every MMA has completed: the ring's shared memory is free
     tc_fence_after();
     const int fl = warp * 32 + lane;
-    const int64_t f = (int64_t)f0 + fl;
     const int ns = p.n_slices;
-    // several slices: park the partial tile in this CTA's shared memory (the ring's: every warp must be done with
-    // the staged chunks first -- the amax warps read them too), layout [column quad][feature][4 floats]
-    if (ns > 1) __syncthreads();
+    constexpr int QH = R / 4;   // column quads per half
+    const bool via_slots = FW == 128 && ns > 1;        // SLOTS shape
+    const bool via_cluster = FW == 256 && ns > 1;      // CLUSTER shape
+    // CLUSTER: park the partial tile in this CTA's shared memory (the ring's: every warp must be done with the staged
+    // chunks first -- the amax warps read them too), layout [half][column quad][feature][4 floats]
+    if (via_cluster) __syncthreads();
     float* park = reinterpret_cast<float*>(smem);
+    // SLOTS: the same layout in this slice's slot of the workspace: a warp's store covers 512 contiguous bytes
+    float* slot = via_slots ? p.slots[z] + ((int64_t)blockIdx.x * ns + blockIdx.y) * (128 * R) : nullptr;
 #pragma unroll
-    for (int c0 = 0; c0 < R; c0 += 16) {
-      uint32_t v[16];
-      tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + c0, v);
-      tmem_ld_wait();
-      if (ns > 1) {
+    for (int hf = 0; hf < HALVES; ++hf) {
+      const int64_t f = (int64_t)f0 + hf * 128 + fl;
 #pragma unroll
-        for (int j = 0; j < 16; j += 4)
-          *reinterpret_cast<uint4*>(park + ((c0 + j) / 4 * WG_F + fl) * 4) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
-      } else if (f < F) {
-        float4* o = reinterpret_cast<float4*>(p.out[z] + f * R + c0);
+      for (int c0 = 0; c0 < R; c0 += 16) {
+        uint32_t v[16];
+        tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + hf * HALF_COLS + c0, v);
+        tmem_ld_wait();
+        if (via_cluster || via_slots) {
+          float* dst = via_cluster ? park : slot;
 #pragma unroll
-        for (int j = 0; j < 16; j += 4) {
-          float4 a = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]),
-                                 __uint_as_float(v[j + 3]));
-          if (p.accumulate) {
-            const float4 old = o[j / 4];
-            a.x += old.x;
-            a.y += old.y;
-            a.z += old.z;
-            a.w += old.w;
+          for (int j = 0; j < 16; j += 4)
+            *reinterpret_cast<uint4*>(dst + ((hf * QH + (c0 + j) / 4) * 128 + fl) * 4) =
+                make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+        } else if (f < F) {
+          float4* o = reinterpret_cast<float4*>(p.out[z] + f * R + c0);
+#pragma unroll
+          for (int j = 0; j < 16; j += 4) {
+            float4 a = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]), __uint_as_float(v[j + 2]),
+                                   __uint_as_float(v[j + 3]));
+            if (p.accumulate) {
+              const float4 old = o[j / 4];
+              a.x += old.x;
+              a.y += old.y;
+              a.z += old.z;
+              a.w += old.w;
+            }
+            o[j / 4] = a;
           }
-          o[j / 4] = a;
         }
       }
     }
     tc_fence_before();
-    if (ns > 1) {
+    if (via_cluster) {
       // the cluster = the M slices of this feature tile.  After the barrier slice s sums column quads
-      // s, s + ns, ... of the tile over all slices' shared memory, in slice order, and owns those outputs.
+      // s, s + ns, ... (of the HALVES x R / 4 of the tile) over all slices' shared memory, in slice order, and owns
+      // those outputs.
       cluster_sync();
       const uint32_t rank = cluster_ctarank();
       const uint32_t park_u = smem_u32(park);
 #pragma unroll 1
-      for (int q = (int)rank; q < R / 4; q += ns) {
-        const uint32_t off = park_u + (uint32_t)((q * WG_F + fl) * 16);
+      for (int qi = (int)rank; qi < HALVES * QH; qi += ns) {
+        const int hf = qi / QH, q = qi % QH;
+        const int64_t f = (int64_t)f0 + hf * 128 + fl;
+        const uint32_t off = park_u + (uint32_t)((qi * 128 + fl) * 16);
         float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
         for (int s0 = 0; s0 < ns; s0 += 4) {
           float4 v[4];
@@ -232,6 +275,62 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
         }
       }
       cluster_sync();   // no slice leaves (and frees its shared memory) while a peer still reads it
+    } else if (via_slots) {
+      // count this slice on its feature tile; the slice whose arrival completes the tile sums the slots in slice
+      // order -- all of its loads in flight at once (one L2 round trip, not one per slice) -- and writes the output
+      __syncthreads();                              // the slot is written by all four warps
+      if (tid == 0) {
+        __threadfence();                            // ... and visible before the slice is counted
+        const uint32_t old = atomicAdd(p.counters[z] + blockIdx.x, 1u);
+        const int last = (int)old == ns - 1;
+        if (last) __threadfence();                  // the other slices' slots are visible to what follows
+        s_last = last;
+      }
+      __syncthreads();
+      if (s_last) {
+        const int64_t f = (int64_t)f0 + fl;
+        const float4* src = reinterpret_cast<const float4*>(p.slots[z]) + (int64_t)blockIdx.x * ns * (128 * R / 4) + fl;
+        constexpr int QB = 2;        // column quads per batch: QB * ns loads in flight per thread
+#pragma unroll 1
+        for (int q0 = 0; q0 < QH; q0 += QB) {
+          float4 acc[QB];
+#pragma unroll
+          for (int j = 0; j < QB; ++j) acc[j] = make_float4(0.f, 0.f, 0.f, 0.f);
+          for (int s0 = 0; s0 < ns; s0 += 8) {
+            float4 v[QB][8];
+#pragma unroll
+            for (int j = 0; j < QB; ++j)
+#pragma unroll
+              for (int k = 0; k < 8; ++k)
+                v[j][k] = (s0 + k < ns) ? __ldcg(src + (int64_t)(s0 + k) * (128 * R / 4) + (q0 + j) * 128)
+                                        : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+            for (int j = 0; j < QB; ++j)
+#pragma unroll
+              for (int k = 0; k < 8; ++k) {
+                acc[j].x += v[j][k].x;
+                acc[j].y += v[j][k].y;
+                acc[j].z += v[j][k].z;
+                acc[j].w += v[j][k].w;
+              }
+          }
+          if (f < F) {
+#pragma unroll
+            for (int j = 0; j < QB; ++j) {
+              float4* o = reinterpret_cast<float4*>(p.out[z] + f * R + (q0 + j) * 4);
+              if (p.accumulate) {
+                const float4 old = *o;
+                acc[j].x += old.x;
+                acc[j].y += old.y;
+                acc[j].z += old.z;
+                acc[j].w += old.w;
+              }
+              *o = acc[j];
+            }
+          }
+        }
+        if (tid == 0) p.counters[z][blockIdx.x] = 0u;   // back to zero for the next call
+      }
     }
   }
   __syncthreads();
@@ -242,19 +341,61 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
   if (p.late_wait) pdl_wait();
 }
 
+// one-time per-device setup: shared-memory opt-in and the largest carveout (three CTAs of 61 KB per SM)
+template <int R, int FW>
+static int wg_prepare() {
+  static bool done[FT_MAX_DEVICES] = {};
+  const int dev = current_device();
+  if (dev >= 0 && dev < FT_MAX_DEVICES && done[dev]) return FT_OK;
+  FT_CUDA_TRY(cudaFuncSetAttribute(k_wgrad<R, FW>, cudaFuncAttributeMaxDynamicSharedMemorySize, WgCfg<R, FW>::SMEM));
+  FT_CUDA_TRY(cudaFuncSetAttribute(k_wgrad<R, FW>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                   cudaSharedmemCarveoutMaxShared));
+  if (dev >= 0 && dev < FT_MAX_DEVICES) done[dev] = true;
+  return FT_OK;
+}
+
+// CLUSTER shape: how many clusters (1, s, 1) the device holds at once (cached per device and s): a grid that does
+// not fit in one wave runs its last clusters alone
 template <int R>
+static int wg_max_active_clusters(int s) {
+  static int cached[FT_MAX_DEVICES][9] = {};
+  const int dev = current_device();
+  const bool ok = dev >= 0 && dev < FT_MAX_DEVICES && s >= 1 && s <= 8;
+  if (ok && cached[dev][s] != 0) return cached[dev][s];
+  if (wg_prepare<R, 256>() != FT_OK) return 1;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(1, (unsigned)s, 1);
+  cfg.blockDim = dim3(WG_THREADS, 1, 1);
+  cfg.dynamicSmemBytes = WgCfg<R, 256>::SMEM;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = 1;
+  attr[0].val.clusterDim.y = (unsigned)s;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int n = 0;
+  if (cudaOccupancyMaxActiveClusters(&n, k_wgrad<R, 256>, &cfg) != cudaSuccess || n < 1) {
+    (void)cudaGetLastError();
+    n = sm_count() / s;   // one CTA per SM, perfect packing: a guess that only sizes the slices
+    if (n < 1) n = 1;
+  }
+  if (ok) cached[dev][s] = n;
+  return n;
+}
+
+template <int R, int FW>
 static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, bool pdl, cudaStream_t st) {
-  constexpr int NG = (R + 63) / 64;
-  const int smem = WG_STAGES * (WG_IN_BYTES + NG * WG_LG_BYTES) + 1024;   // >= the 128 x R fp32 parked tile
-  FT_CUDA_TRY(cudaFuncSetAttribute(k_wgrad<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  int rc = wg_prepare<R, FW>();
+  if (rc != FT_OK) return rc;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = grid;
   cfg.blockDim = dim3(WG_THREADS, 1, 1);
-  cfg.dynamicSmemBytes = smem;
+  cfg.dynamicSmemBytes = WgCfg<R, FW>::SMEM;
   cfg.stream = st;
   cudaLaunchAttribute attr[2];
   int na = 0;
-  if (grid.y > 1) {   // the M slices of a feature tile form one cluster
+  if (FW == 256 && grid.y > 1) {   // CLUSTER: the M slices of a feature tile form one cluster
     attr[na].id = cudaLaunchAttributeClusterDimension;
     attr[na].val.clusterDim.x = 1;
     attr[na].val.clusterDim.y = grid.y;
@@ -268,31 +409,59 @@ static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, bool
   }
   cfg.attrs = attr;
   cfg.numAttrs = na;
-  if (getenv("FT_DEBUG_OCC") != nullptr) {
-    int ncl = -1, nb = -1;
-    cudaOccupancyMaxActiveClusters(&ncl, k_wgrad<R>, &cfg);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k_wgrad<R>, WG_THREADS, smem);
-    fprintf(stderr, "k_wgrad<%d> grid (%u,%u,%u) smem %d: max active clusters %d, blocks/SM %d\n", R, grid.x, grid.y, grid.z,
-            smem, ncl, nb);
-  }
-  FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_wgrad<R>, maps[0], maps[1], maps[2], maps[3], p));
+  FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_wgrad<R, FW>, maps[0], maps[1], maps[2], maps[3], p));
   return FT_OK;
 }
 
+static int wg_clusters_for(int r, int s) {
+  switch (r) {
+    case 16: return wg_max_active_clusters<16>(s);
+    case 32: return wg_max_active_clusters<32>(s);
+    case 48: return wg_max_active_clusters<48>(s);
+    case 64: return wg_max_active_clusters<64>(s);
+    case 80: return wg_max_active_clusters<80>(s);
+    case 96: return wg_max_active_clusters<96>(s);
+    case 112: return wg_max_active_clusters<112>(s);
+    case 128: return wg_max_active_clusters<128>(s);
+    default: return 1;
+  }
+}
+
+template <int FW>
+static int launch_wg_r(int r, const CUtensorMap* maps, const WgParams& p, dim3 grid, bool pdl, cudaStream_t st) {
+  switch (r) {
+    case 16: return launch_wg<16, FW>(maps, p, grid, pdl, st);
+    case 32: return launch_wg<32, FW>(maps, p, grid, pdl, st);
+    case 48: return launch_wg<48, FW>(maps, p, grid, pdl, st);
+    case 64: return launch_wg<64, FW>(maps, p, grid, pdl, st);
+    case 80: return launch_wg<80, FW>(maps, p, grid, pdl, st);
+    case 96: return launch_wg<96, FW>(maps, p, grid, pdl, st);
+    case 112: return launch_wg<112, FW>(maps, p, grid, pdl, st);
+    case 128: return launch_wg<128, FW>(maps, p, grid, pdl, st);
+    default: return FT_ERR_UNSUPPORTED_SHAPE;
+  }
+}
+
 // which = 1: dA [K x r] = X^T P[:, r_s:];  which = 2: dBt [N x r] = G^T H[:, r_s:];  which = 3: both in
-// ONE launch (blockIdx.z picks the problem).  The M slices (at most 8, the portable cluster size) of a feature
-// tile are one cluster and combine over distributed shared memory in slice order.
+// ONE launch (blockIdx.z picks the problem).
+// workspace != NULL (the caller's layer workspace, control words zero): the SLOTS shape -- 128-feature tiles, three
+//   CTAs per SM, M slices sized for one wave, combined through slots and arrival counters of the workspace.
+// workspace == NULL: the CLUSTER shape -- 256-feature tiles, at most 8 M slices = one cluster, combined over
+//   distributed shared memory.
+// Either way: no clear kernel, no atomics on the data, a fixed order of additions.
 // amax_g (which & 2 only): zero word that receives the bit pattern of max |G|.
 // after_kernel: the launch directly follows a kernel of the same call (programmatic edge allowed).
 // beside_prev: see WgParams::late_wait (the caller's promise).
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, bool after_kernel, bool beside_prev, cudaStream_t st) {
+                 unsigned int* amax_g, void* workspace, bool after_kernel, bool beside_prev, cudaStream_t st) {
   CUtensorMap maps[4];
   const void* in_all[2] = {x, g};
   const void* lr_all[2] = {p_saved, h_saved};
   const int64_t F_all[2] = {K, N};
   float* out_all[2] = {dA, dBt};
+  const bool slots_shape = workspace != nullptr;
+  const int FW = slots_shape ? 128 : 256;
   WgParams p;
   p.M = M;
   p.r_s = r_s;
@@ -303,18 +472,46 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
   int sel[2], nz = 0;
   for (int z = 0; z < 2; ++z)
     if (which & (1 << z)) sel[nz++] = z;
-  int64_t f_tiles_total = 0;
-  for (int i = 0; i < nz; ++i) f_tiles_total += ceil_div(F_all[sel[i]], WG_F);
-  // M slices: one wave of two resident CTAs per SM over all feature tiles (rounded DOWN: a second,
-  // mostly empty wave costs more than slightly longer slices), at least 8 chunks (512 rows) each, at most 8
-  int64_t slices = (int64_t)2 * sm_count() / f_tiles_total;
-  if (slices > chunks / 8) slices = chunks / 8;
-  if (slices > 8) slices = 8;
-  if (slices < 1) slices = 1;
+  int64_t f_tiles_total = 0, f_tiles_max = 0;
+  for (int i = 0; i < nz; ++i) {
+    const int64_t ft = ceil_div(F_all[sel[i]], FW);
+    f_tiles_total += ft;
+    if (ft > f_tiles_max) f_tiles_max = ft;
+  }
+  int64_t slices = 1;
+  if (slots_shape) {
+    if (f_tiles_max > WS_MAX_FEATURE_TILES) return FT_ERR_UNSUPPORTED_SHAPE;
+    // one wave of three CTAs per SM over all feature tiles (rounded DOWN: a second, mostly empty wave costs more
+    // than slightly longer slices), at least 4 chunks (256 rows) each, and no more slices than the workspace
+    // has slots for
+    slices = (int64_t)3 * sm_count() / f_tiles_total;
+    if (slices > chunks / 4) slices = chunks / 4;
+    if (slices * f_tiles_total > WS_MAX_WGRAD_SLOTS) slices = WS_MAX_WGRAD_SLOTS / f_tiles_total;
+    if (slices < 1) slices = 1;
+  } else {
+    // M slices = cluster size, at most 8, at least 4 chunks each: the count s that minimises waves(s) x chunks
+    // per slice, where waves(s) = clusters of the launch / clusters of size s the device holds at once (one CTA
+    // per SM, and clusters of 3 or more strand a few SMs: 148, 74, 45, 33, 26, 22, 15, 15 on B200)
+    int64_t max_slices = chunks / 4;
+    if (max_slices > 8) max_slices = 8;
+    if (max_slices < 1) max_slices = 1;
+    int64_t best_cost = -1;
+    for (int64_t s = 1; s <= max_slices; ++s) {
+      const int64_t cap = wg_clusters_for(r, (int)s);
+      const int64_t cost = ceil_div(f_tiles_total, cap) * ceil_div(chunks, s);
+      if (best_cost < 0 || cost < best_cost) {
+        best_cost = cost;
+        slices = s;
+      }
+    }
+  }
   const int cpc = (int)ceil_div(chunks, slices);
   const unsigned sl = (unsigned)ceil_div(chunks, cpc);   // every slice has at least one chunk
   p.n_slices = (int)sl;
+  p.chunks_per_cta = cpc;
   unsigned gx = 0;
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  float* slot_cursor = ws ? reinterpret_cast<float*>(ws + ws_layout(M, r_t).wg_slots_off) : nullptr;
   for (int i = 0; i < 2; ++i) {
     const int z = i < nz ? sel[i] : sel[0];
     int rc = make_tensor_map_2d(&maps[2 * i], in_all[z], 2, (uint64_t)F_all[z], (uint64_t)M, (uint64_t)F_all[z] * 2, 64,
@@ -324,27 +521,27 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
                             Swizzle::B128);
     if (rc != FT_OK) return rc;
     p.F[i] = F_all[z];
-    p.chunks_per_cta[i] = cpc;
     p.out[i] = out_all[z];
     p.amax_bits[i] = z == 1 ? amax_g : nullptr;
+    p.slots[i] = nullptr;
+    p.counters[i] = nullptr;
     if (i >= nz) continue;
-    const unsigned ft = (unsigned)ceil_div(F_all[z], WG_F);
+    const unsigned ft = (unsigned)ceil_div(F_all[z], FW);
+    if (slots_shape && sl > 1) {
+      p.slots[i] = slot_cursor;
+      slot_cursor += (size_t)ft * sl * 128 * r;
+      p.counters[i] = reinterpret_cast<uint32_t*>(ws + WS_CTL_WGTILES) + (size_t)z * WS_MAX_FEATURE_TILES;
+    }
     if (ft > gx) gx = ft;
   }
   const dim3 grid(gx, sl, (unsigned)nz);
   const bool pdl = after_kernel;
   p.late_wait = (beside_prev && pdl) ? 1 : 0;
-  switch (r) {
-    case 16: return launch_wg<16>(maps, p, grid, pdl, st);
-    case 32: return launch_wg<32>(maps, p, grid, pdl, st);
-    case 48: return launch_wg<48>(maps, p, grid, pdl, st);
-    case 64: return launch_wg<64>(maps, p, grid, pdl, st);
-    case 80: return launch_wg<80>(maps, p, grid, pdl, st);
-    case 96: return launch_wg<96>(maps, p, grid, pdl, st);
-    case 112: return launch_wg<112>(maps, p, grid, pdl, st);
-    case 128: return launch_wg<128>(maps, p, grid, pdl, st);
-    default: return FT_ERR_UNSUPPORTED_SHAPE;
-  }
+#ifdef FT_TRACE
+  p.dbg = getenv("FT_WG_DBG") ? atoi(getenv("FT_WG_DBG")) : 0;
+  if (p.dbg & 2) p.amax_bits[0] = p.amax_bits[1] = nullptr;
+#endif
+  return slots_shape ? launch_wg_r<128>(r, maps, p, grid, pdl, st) : launch_wg_r<256>(r, maps, p, grid, pdl, st);
 }
 
 }  // namespace ft

@@ -243,6 +243,9 @@ static int launch_wq(const CUtensorMap* maps, const WqParams& p, dim3 grid, bool
   constexpr int NG = (R + 63) / 64;
   const int smem = WQ_STAGES * (WQ_IN_BYTES + NG * WQ_LG_BYTES + WQ_CODE_BYTES + WQ_SF_BYTES) + 1024;
   FT_CUDA_TRY(cudaFuncSetAttribute(k_wgrad_q4<R>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  // two CTAs per SM need the largest carveout (the default one fits a single CTA of this size)
+  FT_CUDA_TRY(cudaFuncSetAttribute(k_wgrad_q4<R>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                   cudaSharedmemCarveoutMaxShared));
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = grid;
   cfg.blockDim = dim3(WQ_THREADS, 1, 1);

@@ -61,8 +61,9 @@ def test_argument_validation_needs_no_gpu(lib):
     vp = C.c_void_p
     lib.ft_tensor_amax.argtypes = [vp, C.c_int64, vp, vp]
     assert lib.ft_tensor_amax(None, 16, None, None) == -1
-    lib.ft_quantize_blockwise.argtypes = [vp, C.c_int64, C.c_int64, vp, vp, vp, C.c_int32, vp, C.c_size_t, vp]
-    assert lib.ft_quantize_blockwise(None, 128, 64, None, None, None, 0, None, 0, None) == -1
+    lib.ft_quantize_blockwise.argtypes = [vp, C.c_int64, C.c_int64, vp, vp, vp, C.c_int32, C.c_uint64, C.c_uint64, vp,
+                                          C.c_size_t, vp]
+    assert lib.ft_quantize_blockwise(None, 128, 64, None, None, None, 0, 0, 0, None, 0, None) == -1
     lib.ft_linear_fwd.argtypes = [vp, vp, C.c_int64, vp, vp, vp, vp, C.c_size_t, vp]
     assert lib.ft_linear_fwd(None, None, 1, None, None, None, None, 0, None) == -1
     assert lib.ft_debug_set_gemm_tile_n(100) == -1 and lib.ft_debug_set_gemm_tile_n(0) == 0

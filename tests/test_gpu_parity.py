@@ -112,6 +112,82 @@ def test_quantize_with_caller_amax(B):
     assert_q_equal(out, nvfp4.quantize_blockwise(x, 1), B.FT_SF_TILE128x4, B)
 
 
+@pytest.mark.parametrize("rows,cols,layout", [(1, 64, 0), (130, 512, 1), (300, 1024, 0), (2304, 3072, 1)])
+def test_quantize_stochastic_rounding_bit_exact(B, rows, cols, layout):
+    """NEXT-4 / O-6': FT_ROUND_STOCHASTIC against the oracle's stochastic quantizer on the same Philox4x32-10 stream
+    (64-bit seed, an offset that crosses 2^32): codes, scales and tensor scale bit for bit.  Counter-based: the lower
+    part of the tensor quantized alone, with the whole tensor's amax and the offset advanced, gives the same bits."""
+    rng = synth.make_rng(rows * 7 + cols)
+    x = synth.student_t_grad(rng, rows, cols)
+    seed, offset = 0x1234567890ABCDEF, (1 << 32) - 100
+    out = B.QTensor(rows, cols, 1, layout)
+    B.ft_quantize_blockwise(t16(x), out, round_mode=B.FT_ROUND_STOCHASTIC, seed=seed, offset=offset)
+    q = nvfp4.quantize_blockwise(x, 1, round_mode="stochastic", seed=seed, offset=offset)
+    assert_q_equal(out, q, layout, B)
+    qn = nvfp4.quantize_blockwise(x, 1)
+    assert np.array_equal(q["sf"], qn["sf"]) and (q["codes"] != qn["codes"]).mean() > 0.05   # same scales, other codes
+    if rows >= 130:
+        a = 64
+        amax = torch.tensor([float(nvfp4.tensor_amax(x))], dtype=torch.float32, device="cuda")
+        part = B.QTensor(rows - a, cols, 1, layout)
+        B.ft_quantize_blockwise(t16(x[a:]), part, tensor_amax=amax, round_mode=B.FT_ROUND_STOCHASTIC, seed=seed,
+                                offset=offset + a * cols // 4)
+        assert np.array_equal(part.codes.cpu().numpy(), q["packed"][a:])
+    # the mode is a variant of the plain quantizer: no fused projection, no 16x16 blocks
+    with pytest.raises(B.FtError):
+        B.ft_quantize_blockwise(t16(x), out, down=t16(np.zeros((cols, 16), np.float32)), round_mode=B.FT_ROUND_STOCHASTIC)
+
+
+def test_dgrad_with_stochastically_rounded_gradient(B):
+    """The use the variant is meant for: Q(G) by stochastic rounding feeding the dgrad GEMM (ft_quantize_blockwise +
+    ft_gemm4 with Q(R)^T), against the oracle's float64 product of the same dequantized operands."""
+    M, K, N = 300, 512, 768
+    rng = synth.make_rng(91)
+    G = synth.student_t_grad(rng, M, N)
+    W = synth.normal(rng, (N, K), 0.02)
+    L = B.Layer(t16(W), None, None, 0, 0)
+    qg = B.QTensor(M, N)
+    B.ft_quantize_blockwise(t16(G), qg, round_mode=B.FT_ROUND_STOCHASTIC, seed=5, offset=17)
+    dx = torch.zeros(M, K, dtype=torch.bfloat16, device="cuda")
+    B.ft_gemm4(qg, L.r_nmajor, None, None, dx)
+    oG = nvfp4.quantize_blockwise(G, 1, round_mode="stochastic", seed=5, offset=17)
+    oR = nvfp4.quantize_blockwise(W, 16)
+    assert_q_equal(qg, oG, B.FT_SF_TILE128x4, B)
+    alpha = np.float64(np.float32(oG["g_dec"]) * np.float32(oR["g_dec"]))
+    uG, uR = nvfp4.dequantize_unscaled(oG), nvfp4.dequantize_unscaled(oR)
+    want = nvfp4.bf16_round_from_f64(alpha * (uG @ uR))
+    got = npf(dx)
+    assert rel(got, want) <= TOL and (got == want).mean() >= 0.95
+    elementwise_ok(got, want, alpha * (np.abs(uG) @ np.abs(uR)), "dX")
+
+
+def test_quantize_16x16_blocks_on_activations_through_the_gemm(B):
+    """NEXT-4's third arm (Table 5 at 240-243; reading O-2 keeps 1x16 for activations): an ACTIVATION
+    quantized in 16x16 blocks -- ft_quantize_blockwise(block_rows = 16), scales expanded per row by the TILE128x4
+    layout -- fed to ft_gemm4 against 16x16 weights, compared with the oracle; and it is the coarser quantizer."""
+    M, K, N = 256, 512, 384
+    rng = synth.make_rng(92)
+    X = synth.outlier_normal(rng, M, K)
+    W = synth.normal(rng, (N, K), 0.02)
+    qx = B.QTensor(M, K, 16, B.FT_SF_TILE128x4)
+    B.ft_quantize_blockwise(t16(X), qx)
+    oX = nvfp4.quantize_blockwise(X, 16)
+    assert_q_equal(qx, oX, B.FT_SF_TILE128x4, B)
+    L = B.Layer(t16(W), None, None, 0, 0)
+    y = torch.zeros(M, N, dtype=torch.bfloat16, device="cuda")
+    B.ft_gemm4(qx, L.r_kmajor, None, None, y)
+    oW = nvfp4.quantize_blockwise(W, 16)
+    alpha = np.float64(np.float32(oX["g_dec"]) * np.float32(oW["g_dec"]))
+    uX, uW = nvfp4.dequantize_unscaled(oX), nvfp4.dequantize_unscaled(oW)
+    want = nvfp4.bf16_round_from_f64(alpha * (uX @ uW.T))
+    got = npf(y)
+    assert rel(got, want) <= TOL and (got == want).mean() >= 0.95
+    elementwise_ok(got, want, alpha * (np.abs(uX) @ np.abs(uW).T), "Y")
+    # Table 5's direction on activations too: 16x16 blocks lose more than 1x16 (an outlier channel costs its 15
+    # neighbouring ROWS their resolution as well)
+    assert rel(nvfp4.dequantize(oX), X) > rel(nvfp4.dequantize(nvfp4.quantize_blockwise(X, 1)), X)
+
+
 def test_quantize_degenerate_inputs(B):
     # all zeros; -0.0; a block of tiny values next to the tensor maximum; saturating ties
     x = np.zeros((128, 128), np.float32)

@@ -282,3 +282,82 @@ def test_wgrad_saved4_bruteforce_and_special_cases():
     assert np.array_equal(nvfp4.dequantize(qXe), Xe.astype(np.float64))
     assert np.array_equal(layer.wgrad_saved4(qXe, G, fw["H"], P, r_s)["dA"],
                           layer.wgrad(Xe, G, fw["H"], P, r_s)["dA"])
+
+
+# ------------------------------------------------------------------ NEXT-1: MLP fusion oracle (reading O-16)
+def test_gelu_tanh_closed_forms_and_derivative():
+    """gelu_tanh against what the mathematics fixes: gelu(0) = 0; gelu(y) - gelu(-y) = y (the tanh form's 1 + tanh
+    and 1 - tanh halves add to 2); gelu(y) -> y and gelu(-y) -> 0 for large y; within 1e-3 of the erf form it
+    approximates (Hendrycks & Gimpel); hand value gelu(1) = 0.5 (1 + tanh(0.7978845608 * 1.044715)); and the
+    derivative against central differences."""
+    import math
+    assert layer.gelu_tanh(0.0) == 0.0
+    y = np.linspace(-6, 6, 2401)
+    g = layer.gelu_tanh(y)
+    assert np.allclose(g - layer.gelu_tanh(-y), y, rtol=0, atol=1e-15)
+    assert abs(layer.gelu_tanh(12.0) - 12.0) < 1e-12 and abs(layer.gelu_tanh(-12.0)) < 1e-12
+    erf_form = np.array([0.5 * v * (1.0 + math.erf(v / math.sqrt(2.0))) for v in y])
+    assert np.max(np.abs(g - erf_form)) < 1e-3 and np.max(np.abs(g - erf_form)) > 1e-5      # close, not the same function
+    assert abs(layer.gelu_tanh(1.0) - 0.5 * (1.0 + math.tanh(0.7978845608028654 * 1.044715))) < 1e-15
+    h = 1e-6
+    fd = (layer.gelu_tanh(y + h) - layer.gelu_tanh(y - h)) / (2 * h)
+    assert np.max(np.abs(fd - layer.gelu_tanh_grad(y))) < 1e-8
+    assert abs(layer.gelu_tanh_grad(0.0) - 0.5) < 1e-15
+
+
+def test_mlp_forward_is_the_two_layers_with_the_quantizer_in_between():
+    """mlp_forward against a brute-force restatement on a tiny MLP: FC1 by the layer oracle's own brute-force-pinned
+    forward, GeLU element by element in Python floats, Q(Z) with the CALLER's amax (delayed scaling: a stale, larger
+    amax must change the scales), FC2 by Python triple loops over the dequantized codes; and the staged inputs
+    (Z_given) are honoured."""
+    import math
+    rng = np.random.default_rng(3)
+    M, K, N1, N2, r_t = 8, 64, 32, 16, 16
+    bf = nvfp4.bf16_round
+    X = bf(rng.standard_normal((M, K)).astype(np.float32))
+    R1 = bf((rng.standard_normal((N1, K)) * 0.05).astype(np.float32)); R2 = bf((rng.standard_normal((N2, N1)) * 0.05).astype(np.float32))
+    D1 = bf((rng.standard_normal((K, r_t)) * 0.1).astype(np.float32)); U1 = bf((rng.standard_normal((r_t, N1)) * 0.1).astype(np.float32))
+    D2 = bf((rng.standard_normal((N1, r_t)) * 0.1).astype(np.float32)); U2 = bf((rng.standard_normal((r_t, N2)) * 0.1).astype(np.float32))
+    q1, q2 = layer.quantize_weight(R1), layer.quantize_weight(R2)
+    f1 = layer.forward(X, q1, D1, U1, prescale=True)
+    Zb = np.zeros((M, N1), np.float32)
+    for m in range(M):
+        for n in range(N1):
+            v = float(f1["Y"][m, n])
+            Zb[m, n] = 0.5 * v * (1.0 + math.tanh(math.sqrt(2.0 / math.pi) * (v + 0.044715 * v ** 3)))
+    Zb = nvfp4.bf16_round_from_f64(Zb.astype(np.float64))
+    z_amax = np.float32(2.0) * nvfp4.tensor_amax(Zb)          # a stale amax from "the previous step"
+    out = layer.mlp_forward(X, q1, D1, U1, q2, D2, U2, z_amax=z_amax, y1_amax=nvfp4.tensor_amax(f1["Y"]))
+    assert np.array_equal(out["Y1"], f1["Y"]) and np.array_equal(out["Z"], Zb)
+    qZ = nvfp4.quantize_blockwise(Zb, 1, amax_t=z_amax)
+    assert np.array_equal(out["qZ"]["codes"], qZ["codes"]) and np.array_equal(out["qZ"]["sf"], qZ["sf"])
+    assert not np.array_equal(qZ["sf"], nvfp4.quantize_blockwise(Zb, 1)["sf"])     # the caller's amax is what counts
+    assert np.array_equal(out["qY1"]["codes"], nvfp4.quantize_blockwise(f1["Y"], 1)["codes"])
+    dZ, dR2 = nvfp4.dequantize_unscaled(qZ), nvfp4.dequantize_unscaled(q2)
+    alpha2 = float(np.float32(qZ["g_dec"]) * np.float32(q2["g_dec"]))
+    H2 = Zb.astype(np.float64) @ D2.astype(np.float64)
+    H2s = nvfp4.bf16_round_from_f64(H2 / alpha2).astype(np.float64)
+    Y2 = np.zeros((M, N2))
+    for m in range(M):
+        for n in range(N2):
+            acc = 0.0
+            for k in range(N1):
+                acc += dZ[m, k] * dR2[n, k]
+            for j in range(r_t):
+                acc += H2s[m, j] * float(U2[j, n])
+            Y2[m, n] = alpha2 * acc
+    assert np.array_equal(out["Y2"], nvfp4.bf16_round_from_f64(Y2))
+    # staged comparison: a given Z replaces the oracle's own
+    Z2 = Zb.copy(); Z2[0, 0] += np.float32(0.5)
+    out2 = layer.mlp_forward(X, q1, D1, U1, q2, D2, U2, z_amax=z_amax, y1_amax=nvfp4.tensor_amax(f1["Y"]), Z_given=Z2)
+    assert np.array_equal(out2["Z"], Z2) and not np.array_equal(out2["Y2"][0], out["Y2"][0])
+    # GeLU backward on the saved 4-bit pre-activation, element by element
+    G = bf((rng.standard_normal((M, N1)) * 1e-2).astype(np.float32))
+    dY1 = layer.gelu_backward_saved4(G, out["qY1"])
+    y1q = nvfp4.dequantize(out["qY1"])
+    for m in (0, 3, 7):
+        for n in (0, 5, 31):
+            v = float(y1q[m, n]); c = math.sqrt(2.0 / math.pi)
+            t = math.tanh(c * (v + 0.044715 * v ** 3))
+            want = float(G[m, n]) * (0.5 * (1 + t) + 0.5 * v * (1 - t * t) * c * (1 + 3 * 0.044715 * v * v))
+            assert dY1[m, n] == nvfp4.bf16_round_from_f64(np.float64(want))

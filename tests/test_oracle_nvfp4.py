@@ -257,3 +257,100 @@ def test_error_magnitudes():
     q0 = nvfp4.quantize_blockwise(g, 1, amax_t=2688.0)
     assert q0["sf"].max() < 0x08 and np.mean((q0["codes"] & 7) == 0) > 0.85
     assert rel(q0, g) > 3 * eg
+
+
+# ------------------------------------------------------------------ O-6': stochastic rounding (NEXT-4 variant)
+def test_philox4x32_10_known_answers():
+    """The generator against its authors' published known-answer vectors (tests/golden/philox4x32_10_kat.txt)."""
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "philox4x32_10_kat.txt")
+    rows = [l.split() for l in open(path) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(t, 16) for t in r]
+        got = nvfp4.philox4x32_10(np.array(v[0:4], np.uint32), np.array(v[4:6], np.uint32))
+        assert [int(g) for g in got] == v[6:10]
+    # vectorised over counters = one call per counter
+    ctr = np.array([[0, 0, 0, 0], [1, 0, 0, 0], [0xFFFFFFFF, 7, 0, 0]], np.uint32)
+    both = nvfp4.philox4x32_10(ctr, (123, 456))
+    for i in range(3):
+        assert np.array_equal(both[i], nvfp4.philox4x32_10(ctr[i], (123, 456)))
+
+
+def test_sr_uniforms_counter_mapping():
+    """Element idx -> word idx % 4 of counter offset + idx // 4: a tensor quantized in two halves with the second
+    half's offset advanced by its first element's counter draws the same uniforms as the whole tensor; u is a
+    24-bit fraction in [0, 1); the 64-bit seed and offset split into (lo, hi) words."""
+    u = nvfp4.sr_uniforms(4096, seed=0x1234567890ABCDEF, offset=(1 << 32) - 100)
+    assert u.dtype == np.float32 and u.min() >= 0.0 and u.max() < 1.0
+    assert np.all(u * 2.0 ** 24 == np.round(u * 2.0 ** 24))
+    a = nvfp4.sr_uniforms(1024, seed=0x1234567890ABCDEF, offset=(1 << 32) - 100)
+    b = nvfp4.sr_uniforms(3072, seed=0x1234567890ABCDEF, offset=(1 << 32) - 100 + 256)
+    assert np.array_equal(u, np.concatenate([a, b]))
+    # first element by hand: counter (lo, hi, 0, 0), key (lo, hi) of the seed
+    w = nvfp4.philox4x32_10(np.array([0xFFFFFF9C, 0, 0, 0], np.uint32), (0x90ABCDEF, 0x12345678))
+    assert u[0] == np.float32(int(w[0]) >> 8) * np.float32(2.0 ** -24) and u[3] == np.float32(int(w[3]) >> 8) * np.float32(2.0 ** -24)
+    # plausibly uniform: mean 1/2, variance 1/12
+    big = nvfp4.sr_uniforms(1 << 18, seed=7, offset=0).astype(np.float64)
+    assert abs(big.mean() - 0.5) < 4 * np.sqrt(1 / 12 / big.size) and abs(big.var() - 1 / 12) < 2e-3
+
+
+def test_e2m1_stochastic_rounding_definition():
+    """Brute force over a fine grid of values and thresholds: the result is one of the two neighbours, hi exactly when
+    u * (hi - lo) < |v| - lo; values on the grid never move; |v| >= 6 saturates; the sign bit is the input's."""
+    grid = [0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0]
+    vs = np.concatenate([np.linspace(-7.5, 7.5, 481, dtype=np.float32), np.array(grid + [-g for g in grid], np.float32),
+                         np.array([-0.0, 1e-30, -1e-30, 5.9999995, 6.0000005], np.float32)])
+    for uu in (0.0, 2.0 ** -24, 0.25, 0.5, 0.75, 1.0 - 2.0 ** -24):
+        codes = nvfp4.e2m1_encode_stochastic(vs, np.full(vs.shape, uu, np.float32))
+        for v, c in zip(vs, codes):
+            mag = abs(float(v))
+            lo_i = max(i for i, g in enumerate(grid) if g <= mag)
+            if lo_i == 7:
+                want = 7
+            else:
+                lo, hi = grid[lo_i], grid[lo_i + 1]
+                want = lo_i + (1 if uu * (hi - lo) < mag - lo else 0)
+            assert (c & 7) == want and (c >> 3) == int(np.signbit(v)), (v, uu, c)
+    # a grid value is a fixed point for every u, i.e. stochastic == nearest there
+    g = np.array(grid + [-x for x in grid], np.float32)
+    for uu in (0.0, 0.3, 0.999):
+        assert np.array_equal(nvfp4.e2m1_encode_stochastic(g, np.full(g.shape, uu, np.float32)), nvfp4.e2m1_encode(g))
+
+
+def test_stochastic_quantizer_is_unbiased_and_next_to_nearest():
+    """quantize_blockwise(round_mode='stochastic'): the same scales as nearest rounding; every code is the nearest
+    code or its neighbour on the far side of the value; E[dequant] = x inside the grid (checked on a constant tensor
+    over 2^16 draws, 5 sigma); exactly representable data is reproduced bit for bit whatever the seed."""
+    rng = np.random.default_rng(5)
+    x = nvfp4.bf16_round(rng.standard_normal((64, 256)).astype(np.float32))
+    qn = nvfp4.quantize_blockwise(x, 1)
+    qs = nvfp4.quantize_blockwise(x, 1, round_mode="stochastic", seed=42, offset=1000)
+    assert np.array_equal(qn["sf"], qs["sf"]) and qn["g_dec"] == qs["g_dec"]
+    dn, ds = nvfp4.e2m1_decode(qn["codes"]), nvfp4.e2m1_decode(qs["codes"])
+    sc = qn["scaled"].astype(np.float64)
+    assert np.all(np.abs(ds - sc)[np.abs(sc) <= 6] < np.array([0.5, 0.5, 0.5, 0.5, 1.0, 1.0, 2.0, 2.0])[np.minimum(qs["codes"] & 7, qn["codes"] & 7)][np.abs(sc) <= 6] + 1e-12)
+    assert np.all(np.abs((qs["codes"] & 7).astype(int) - (qn["codes"] & 7).astype(int)) <= 1)
+    assert (qs["codes"] != qn["codes"]).mean() > 0.05            # it does round differently ...
+    q2 = nvfp4.quantize_blockwise(x, 1, round_mode="stochastic", seed=43, offset=1000)
+    assert (q2["codes"] != qs["codes"]).mean() > 0.05            # ... and differently per seed
+    assert np.array_equal(nvfp4.quantize_blockwise(x, 1, round_mode="stochastic", seed=42, offset=1000)["codes"], qs["codes"])
+    # unbiased: a constant 0.7 next to one 6.0 per block (so the block scale is exactly 1: amax_t = 2688 given)
+    n = 1 << 16
+    c = np.full((n // 16, 16), 0.7, np.float32)
+    c[:, 0] = 6.0
+    c = nvfp4.bf16_round(c)
+    q = nvfp4.quantize_blockwise(c, 1, amax_t=np.float32(2688.0), round_mode="stochastic", seed=9, offset=0)
+    assert np.all(q["sf"] == 0x38)
+    deq = nvfp4.dequantize(q)[:, 1:]
+    v = float(c[0, 1])
+    assert set(np.unique(deq)) == {0.5, 1.0}
+    p_up = (v - 0.5) / 0.5
+    sigma = 0.5 * np.sqrt(p_up * (1 - p_up) / deq.size)
+    assert abs(deq.mean() - v) < 5 * sigma
+    # nearest rounding of the same tensor is biased by 0.2 (0.7 -> 0.5 always): the test can fail
+    assert abs(nvfp4.dequantize(nvfp4.quantize_blockwise(c, 1, amax_t=np.float32(2688.0)))[:, 1:].mean() - v) > 0.19
+    # representable data: a fixed point for every seed
+    e = rng.choice(np.array([0, 0.5, 1, 1.5, 2, 3, 4, 6, -0.5, -1, -1.5, -2, -3, -4, -6], np.float32), size=(32, 64))
+    e[:, ::16] = 6.0
+    qe = nvfp4.quantize_blockwise(e, 1, amax_t=np.float32(2688.0), round_mode="stochastic", seed=77, offset=5)
+    assert np.array_equal(nvfp4.dequantize(qe).astype(np.float32), e)
