@@ -25,7 +25,7 @@
  *    the structs themselves are host memory, read during the call only.
  *  - the caller owns every buffer; the library never allocates, frees or keeps
  *    a pointer after the call returns.  Scratch comes from `workspace`, a device buffer of at least
- *    ft_workspace_bytes() bytes whose first 36 KB hold control words that must be ZERO when a call starts:
+ *    ft_workspace_bytes() bytes whose first 4 KB hold control words that must be ZERO when a call starts:
  *    zero-fill the buffer once (or call ft_workspace_init); every call leaves them zero again (the kernels
  *    put each word back when they are done with it), so no clearing runs per call.  One workspace serves any
  *    number of stream-ordered calls of any shapes, but not two calls that run concurrently.
@@ -182,8 +182,8 @@ int ft_gemm4(const ft_qtensor* a, const ft_qtensor* b, const void* lr_a_scaled, 
  * dA  [K x r]  = X^T  * P[:, r_s:]      dBt [N x r] = G^T * H[:, r_s:]  (= dB^T)
  * h_saved / p_saved are the [M x r_t] outputs of the two calls above.
  * accumulate: 0 overwrite, 1 add to the existing contents.  Partial sums over slices of M are added in a fixed
- * order (the same bits on every run): this call, which has no workspace, combines them over distributed shared
- * memory inside a thread-block cluster; ft_linear_bwd combines them through its workspace. */
+ * order (the same bits on every run), over distributed shared memory inside a thread-block cluster: no clear
+ * kernel, no atomics on the data. */
 int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
                   const void* h_saved_bf16, const void* p_saved_bf16, float* dA,
                   float* dBt, int32_t accumulate, void* stream);
@@ -205,8 +205,7 @@ int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
  * Same results as ft_linear_bwd_dgrad followed by ft_lora_wgrad, different schedule: the pass
  * over G that computes dBt = G^T (X A) also finds max |G|, so the separate amax pass of the
  * quantizer disappears (G is read twice instead of three times); dA = X^T (G B^T) runs last
- * because it needs P.  The partial sums of dA and dBt over slices of M go through the workspace and are added
- * in a fixed order: the same bits on every run, no clear kernel.  Arguments as in the two calls above. */
+ * because it needs P.  Arguments as in the two calls above. */
 int ft_linear_bwd(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M,
                   const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
                   int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
@@ -223,7 +222,7 @@ int ft_linear_bwd_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
 size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout);
 size_t ft_sf_ntile_bytes(int64_t rows, int64_t cols, int32_t ntile);   /* ft_qtensor::sf_ntile */
 size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t);
-/* Zero the control words at the head of a workspace (one 36 KB memset on `stream`).  Needed once per buffer,
+/* Zero the control words at the head of a workspace (one 4 KB memset on `stream`).  Needed once per buffer,
  * before its first use, unless the caller zero-filled it; never per call.  Also the way to recover a workspace
  * after a call was aborted by a CUDA error. */
 int ft_workspace_init(void* workspace, size_t workspace_bytes, void* stream);

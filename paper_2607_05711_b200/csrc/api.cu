@@ -27,7 +27,7 @@ int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N,
                  cudaStream_t st);
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, void* workspace, bool after_kernel, bool beside_prev, cudaStream_t st);
+                 unsigned int* amax_g, bool after_kernel, bool beside_prev, cudaStream_t st);
 int launch_clear2(void* a, size_t a_bytes, void* b, size_t b_bytes, cudaStream_t st);
 int launch_wgrad_q4(const uint8_t* codes, const uint8_t* sf, const float* g_dec, int64_t M, int64_t K,
                     const void* p_saved, int r_t, int r_s, int r, float* dA, int accumulate, bool beside_prev,
@@ -409,7 +409,7 @@ int ft_lora_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int
   int rc = check_wgrad(L, x_bf16, g_bf16, M, h_saved_bf16, p_saved_bf16, dA, dBt);
   if (rc != FT_OK) return rc;
   return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, L->r_s + L->r, L->r_s, L->r, dA,
-                      dBt, accumulate, nullptr, nullptr, pdl_enabled(), false, (cudaStream_t)stream);
+                      dBt, accumulate, nullptr, pdl_enabled(), false, (cudaStream_t)stream);
 }
 
 int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16, int64_t M,
@@ -432,7 +432,7 @@ int ft_lora_wgrad_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
     chained = true;
   }
   rc = launch_wgrad(2, nullptr, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                    accumulate, nullptr, nullptr, chained, false, st);
+                    accumulate, nullptr, chained, false, st);
   if (rc != FT_OK) return rc;
   return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA,
                          1, false, st);
@@ -475,19 +475,19 @@ static int linear_bwd(const ft_layer* L, const void* x_bf16, const ft_qtensor* q
     if (rc != FT_OK) return rc;
     if (qx == nullptr)
       return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                          accumulate, nullptr, workspace, true, false, st);
+                          accumulate, nullptr, true, false, st);
     rc = launch_wgrad(2, nullptr, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                      accumulate, nullptr, workspace, true, false, st);
+                      accumulate, nullptr, true, false, st);
     if (rc != FT_OK) return rc;
     return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA, 1,
                            false, st);
   }
   // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0), into a control
   //    word of the workspace (zero by the workspace invariant; the quantize kernel puts it back).  The M slices
-  //    combine through slots of the workspace inside the kernel: no clear kernel, no memset node.
+  //    combine over distributed shared memory inside the kernel (a cluster per feature tile): no clear kernel, no memset node.
   unsigned int* amax_g = reinterpret_cast<unsigned int*>(ws + WS_CTL_AMAX_EXT);
   rc = launch_wgrad(2, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                    accumulate, amax_g, workspace, chained, false, st);
+                    accumulate, amax_g, chained, false, st);
   if (rc != FT_OK) return rc;
   // 2. a3 + a4 with that amax: Q(G), P = G U_t, dX
   rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
@@ -498,7 +498,7 @@ static int linear_bwd(const ft_layer* L, const void* x_bf16, const ft_qtensor* q
   //    starts in the GEMM's tail and waits for the GEMM only before it exits.
   if (qx == nullptr)
     return launch_wgrad(1, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                        accumulate, nullptr, workspace, true, true, st);
+                        accumulate, nullptr, true, true, st);
   return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA, 1,
                          true, st);
 }

@@ -48,20 +48,14 @@ bool pdl_enabled();  // programmatic dependent launch of the GEMM and dA kernels
 //       +0   amax word of the single-pass quantizer / of k_amax        +4  grid barrier (amax published)
 //       +8   exit counter of the quantize kernel
 //       +16  amax found by another kernel (the dB^T pass of ft_linear_bwd)
-//       +4 K .. +36 K  one arrival counter per (problem, 128-feature tile) of the wgrad kernels of ft_linear_bwd,
-//                      put back to zero by the slice that completes the tile
 //   [hs_off, +M*r_t*2)     the pre-scaled bf16 intermediate Hs (ft_workspace_hs_offset)
 //   [slots_off, ...)       one 128 x r_t fp32 slot per (CTA, row tile) segment of the quantize kernel -- at most
 //                          WS_MAX_QUANT_CTAS + row tiles of them -- holding partial H tiles
-//   [wg_slots_off, ...)    one 128 x r fp32 slot per (feature tile, M slice) of the wgrad kernels of ft_linear_bwd
 constexpr int WS_MAX_QUANT_CTAS = 192;   // one CTA per SM
-constexpr int WS_MAX_WGRAD_SLOTS = 640;  // one wave of three CTAs per SM (two problems in one launch share them)
-constexpr size_t WS_CTL_BYTES = 36864;
+constexpr size_t WS_CTL_BYTES = 4096;
 constexpr size_t WS_CTL_AMAX = 0, WS_CTL_BAR = 4, WS_CTL_EXIT = 8, WS_CTL_AMAX_EXT = 16;
-constexpr size_t WS_CTL_WGTILES = 4096;
-constexpr int64_t WS_MAX_FEATURE_TILES = (WS_CTL_BYTES - WS_CTL_WGTILES) / 8;  // per problem: 4096 tiles = 524 288 features
 struct WsLayout {
-  size_t hs_off, slots_off, wg_slots_off, total;
+  size_t hs_off, slots_off, total;
 };
 inline WsLayout ws_layout(int64_t M, int r_t) {
   auto up = [](size_t v) { return (v + 255) / 256 * 256; };
@@ -69,8 +63,7 @@ inline WsLayout ws_layout(int64_t M, int r_t) {
   const size_t tiles = (size_t)((M + 127) / 128);
   w.hs_off = WS_CTL_BYTES;
   w.slots_off = w.hs_off + up((size_t)M * (size_t)r_t * 2);
-  w.wg_slots_off = w.slots_off + (WS_MAX_QUANT_CTAS + tiles) * 128 * (size_t)r_t * 4;
-  w.total = w.wg_slots_off + (size_t)WS_MAX_WGRAD_SLOTS * 128 * (size_t)r_t * 4 + 256;
+  w.total = w.slots_off + (WS_MAX_QUANT_CTAS + tiles) * 128 * (size_t)r_t * 4 + 256;
   return w;
 }
 

@@ -467,37 +467,37 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
   }
 }
 
-// The second step: H[row] = sum of the row tile's slots, in CTA order, -> bf16 H and Hs = H * (1 / alpha).
-// One thread per (row, column quad); neighbouring threads read neighbouring rows of a slot (layout
-// [quad][row][4]).  G = grid size of the quantize launch that filled the slots.
+// The second step: H[row] = sum of the row tile's slots -> bf16 H and Hs = H * (1 / alpha).  Block = one column quad of
+// one 128-row tile: thread (r, part) adds the slots i_lo + part, i_lo + part + P, ... of its row (one batch of loads
+// in flight: a single L2 round trip for up to 8 P contributors), the P partial sums of a row meet in shared memory
+// and are added in part order: a fixed association whatever the timing (the same bits on every run).  Neighbouring
+// threads read neighbouring rows of a slot (layout [quad][row][4]).  G = grid size of the quantize launch that filled
+// the slots; P = blockDim.y (1 when a row tile has at most 8 contributors, as on the large shapes).
 template <int R_T>
-__global__ void __launch_bounds__(256) k_finalize_h(const QFParams p, int G) {
-  constexpr int QUADS = R_T / 4;
+__global__ void __launch_bounds__(1024) k_finalize_h(const QFParams p, int G) {
   constexpr int SLOT_F4 = QF_ROWS * R_T / 4;
+  __shared__ float4 s_part[8][QF_ROWS];
   pdl_wait();      // the slots and g_dec come from the quantize kernel before us
   pdl_trigger();
   float inv_alpha = 1.0f;   // Hs = bf16(H * (1 / alpha)), alpha = g_dec(this) * g_dec(other)
   if (p.hs_out != nullptr) inv_alpha = __fdiv_rn(1.0f, __fmul_rn(__ldcg(p.g_dec_out), __ldg(p.other_dec_scale)));
   const int C = p.chunks_per_tile;
   const int64_t TC = p.total_chunks;
-  // thread -> (tile t, quad q, row r) with r fastest
-  const int64_t e = (int64_t)blockIdx.x * 256 + threadIdx.x;
-  const int r = (int)(e % QF_ROWS);
-  const int q = (int)((e / QF_ROWS) % QUADS);
-  const int64_t t = e / (QF_ROWS * QUADS);
+  const int r = threadIdx.x, part = threadIdx.y, P = blockDim.y;
+  const int q = blockIdx.x;
+  const int64_t t = blockIdx.y;
   const int64_t gr = t * QF_ROWS + r;
-  if (gr >= p.rows) return;
   // the CTAs whose ranges meet row tile t: owner(c) = floor(((c + 1) * G - 1) / TC)
   const int i_lo = (int)(((t * C + 1) * G - 1) / TC);
   const int i_hi = (int)((((t + 1) * C) * G - 1) / TC);
   const float4* src = reinterpret_cast<const float4*>(p.slots) + (i_lo + t) * SLOT_F4 + q * QF_ROWS + r;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  constexpr int BATCH = 8;   // loads in flight; a row tile has ~4 contributors (one CTA per SM)
-  for (int i = i_lo; i <= i_hi; i += BATCH) {   // added in CTA order whatever the batching
+  constexpr int BATCH = 8;   // loads in flight per thread
+  for (int i = i_lo + part; i <= i_hi; i += BATCH * P) {   // this part's slots, in CTA order
     float4 v[BATCH];
 #pragma unroll
     for (int j = 0; j < BATCH; ++j)
-      v[j] = (i + j <= i_hi) ? __ldcg(src + (int64_t)j * SLOT_F4) : make_float4(0.f, 0.f, 0.f, 0.f);
+      v[j] = (i + j * P <= i_hi) ? __ldcg(src + (int64_t)(i - i_lo + j * P) * SLOT_F4) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
     for (int j = 0; j < BATCH; ++j) {
       acc.x += v[j].x;
@@ -505,8 +505,20 @@ __global__ void __launch_bounds__(256) k_finalize_h(const QFParams p, int G) {
       acc.z += v[j].z;
       acc.w += v[j].w;
     }
-    src += BATCH * (int64_t)SLOT_F4;
   }
+  if (P > 1) {
+    s_part[part][r] = acc;
+    __syncthreads();
+    if (part != 0) return;
+    for (int k = 1; k < P; ++k) {
+      const float4 o = s_part[k][r];
+      acc.x += o.x;
+      acc.y += o.y;
+      acc.z += o.z;
+      acc.w += o.w;
+    }
+  }
+  if (gr >= p.rows) return;
   if (p.h_out != nullptr)
     *reinterpret_cast<uint2*>(p.h_out + gr * R_T + q * 4) = make_uint2(pack_bf16x2(acc.x, acc.y), pack_bf16x2(acc.z, acc.w));
   if (p.hs_out != nullptr)
@@ -591,10 +603,13 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
   // partial H tiles -> H, Hs; programmatic edge: it sets itself up while the quantize kernel drains
   auto finalize = [&](int grid) -> int {
     if constexpr (R_T > 0) {
-      const int64_t items = ceil_div(p.rows, QF_ROWS) * QF_ROWS * (R_T / 4);
+      const int64_t tiles = ceil_div(p.rows, QF_ROWS);
+      const int64_t contributors = ceil_div((int64_t)grid, tiles) + 1;   // CTAs whose ranges meet one row tile
+      int parts = (int)ceil_div(contributors, 8);
+      if (parts > 8) parts = 8;
       cudaLaunchConfig_t cfg = {};
-      cfg.gridDim = dim3((unsigned)ceil_div(items, 256), 1, 1);
-      cfg.blockDim = dim3(256, 1, 1);
+      cfg.gridDim = dim3((unsigned)(R_T / 4), (unsigned)tiles, 1);
+      cfg.blockDim = dim3(QF_ROWS, (unsigned)parts, 1);
       cfg.stream = st;
       cudaLaunchAttribute attr[1];
       attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;

@@ -22,14 +22,14 @@ namespace ft {
 constexpr int WG_MC = 64;         // rows of M per ring stage
 constexpr int WG_THREADS = 128;
 constexpr int WG_LG_BYTES = WG_MC * 128;      // one 64-column group of L
-// Two shapes of the same kernel.
-//   SLOTS (FW = 128 features per CTA, 3 stages of 20 KB, three CTAs per SM): a CTA's TMA stream runs at ~15 bytes per
-//     clock whatever its tile width or ring depth (measured: the same rate with no MMA and no amax work), so the
-//     pass needs ~400 CTAs in flight to reach the HBM rate; the M slices of a feature tile combine through slots of
-//     the caller's workspace (below).  Used by ft_linear_bwd.
-//   CLUSTER (FW = 256, ring as deep as shared memory allows, one CTA per SM -- the runtime co-schedules one CTA per
-//     SM of a cluster kernel that allocates tensor memory): the M slices of a feature tile are one cluster and
-//     combine over distributed shared memory.  Needs no workspace: used by ft_lora_wgrad.
+// A CTA owns FW = 256 features (two MMA halves of 128; 512 contiguous bytes per row of In) and a ring as deep as
+// shared memory allows (5 x 40 KB for r <= 64): the runtime co-schedules ONE CTA per SM of a cluster kernel that
+// allocates tensor memory, so the bytes in flight come from the ring, not from a second CTA.
+// What bounds the pass (round 2, measured): ~3.7-3.9 TB/s whatever was tried -- 128- or 256-feature tiles, 3 to 6
+// stages, 108 to 432 CTAs in flight (a workspace-slot variant with three CTAs per SM), no MMAs and no amax work at
+// all (same time), whole-row L2 prefetches ahead of the strip loads (slower), strips started at rotated rows (same).
+// A strip walking DOWN the rows takes 256-512 bytes from each DRAM page; the quantize kernel, which walks ALONG
+// the rows with the same TMA boxes, reaches 5.9 TB/s.
 template <int R, int FW>
 struct WgCfg {
   static constexpr int NG = (R + 63) / 64;
@@ -37,10 +37,10 @@ struct WgCfg {
   static constexpr int IN_BYTES = (FW / 64) * WG_MC * 128;   // FW / 64 boxes of 64 features x 64 rows
   static constexpr int STAGE_BYTES = IN_BYTES + NG * WG_LG_BYTES;
   static constexpr int DEEP = (226 * 1024) / STAGE_BYTES > 6 ? 6 : (226 * 1024) / STAGE_BYTES;
-  static constexpr int STAGES = FW == 128 ? 3 : DEEP;
+  static constexpr int STAGES = DEEP;
   static constexpr int SMEM = STAGES * STAGE_BYTES + 1024;
   static constexpr uint32_t HALF_COLS = R <= 32 ? 32 : (R <= 64 ? 64 : 128);   // TMEM columns of one 128-feature half
-  static_assert(FW == 128 || FW == 256, "feature tile");
+  static_assert(FW == 256, "feature tile");
 };
 
 struct WgParams {      // two problems in one launch: [0] dA = X^T P_lora, [1] dB^T = G^T H_lora
@@ -55,8 +55,6 @@ struct WgParams {      // two problems in one launch: [0] dA = X^T P_lora, [1] d
                                 //    wait for it at the END (completion stays transitive for the next launch)
   int n_slices;                 // M slices (gridDim.y); every slice has work
   int accumulate;               // add to the output instead of overwriting it
-  float* slots[2];              // SLOTS: partial tiles go to slot (feature tile * n_slices + slice), 128 x r fp32 each
-  uint32_t* counters[2];        //        one arrival counter per feature tile (zero between calls)
 #ifdef FT_TRACE
   int dbg;                      // development builds: 1 = no MMAs, 2 = no amax fold
 #endif
@@ -70,7 +68,7 @@ __device__ __forceinline__ float4 ld_cluster_f4(uint32_t cluster_addr) {
 }
 
 template <int R, int FW>
-__global__ void __launch_bounds__(WG_THREADS, FW == 128 ? 3 : 1)
+__global__ void __launch_bounds__(WG_THREADS, 1)
 k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUtensorMap map_l0,
         const __grid_constant__ CUtensorMap map_in1, const __grid_constant__ CUtensorMap map_l1,
         const WgParams p) {
@@ -91,7 +89,6 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   __shared__ uint64_t full_bar[WG_STAGES], empty_bar[WG_STAGES], acc_bar;
   __shared__ uint32_t tmem_base_s;
-  __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int32_t f0 = (int32_t)blockIdx.x * FW;
   const int64_t chunks_total = (p.M + WG_MC - 1) / WG_MC;
@@ -195,14 +192,11 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
     const int fl = warp * 32 + lane;
     const int ns = p.n_slices;
     constexpr int QH = R / 4;   // column quads per half
-    const bool via_slots = FW == 128 && ns > 1;        // SLOTS shape
-    const bool via_cluster = FW == 256 && ns > 1;      // CLUSTER shape
-    // CLUSTER: park the partial tile in this CTA's shared memory (the ring's: every warp must be done with the staged
+    const bool via_cluster = ns > 1;
+    // several slices: park the partial tile in this CTA's shared memory (the ring's: every warp must be done with the staged
     // chunks first -- the amax warps read them too), layout [half][column quad][feature][4 floats]
     if (via_cluster) __syncthreads();
     float* park = reinterpret_cast<float*>(smem);
-    // SLOTS: the same layout in this slice's slot of the workspace: a warp's store covers 512 contiguous bytes
-    float* slot = via_slots ? p.slots[z] + ((int64_t)blockIdx.x * ns + blockIdx.y) * (128 * R) : nullptr;
 #pragma unroll
     for (int hf = 0; hf < HALVES; ++hf) {
       const int64_t f = (int64_t)f0 + hf * 128 + fl;
@@ -211,11 +205,10 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
         uint32_t v[16];
         tmem_ld16(tmem_base + ((uint32_t)(warp * 32) << 16) + hf * HALF_COLS + c0, v);
         tmem_ld_wait();
-        if (via_cluster || via_slots) {
-          float* dst = via_cluster ? park : slot;
+        if (via_cluster) {
 #pragma unroll
           for (int j = 0; j < 16; j += 4)
-            *reinterpret_cast<uint4*>(dst + ((hf * QH + (c0 + j) / 4) * 128 + fl) * 4) =
+            *reinterpret_cast<uint4*>(park + ((hf * QH + (c0 + j) / 4) * 128 + fl) * 4) =
                 make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
         } else if (f < F) {
           float4* o = reinterpret_cast<float4*>(p.out[z] + f * R + c0);
@@ -275,62 +268,6 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
         }
       }
       cluster_sync();   // no slice leaves (and frees its shared memory) while a peer still reads it
-    } else if (via_slots) {
-      // count this slice on its feature tile; the slice whose arrival completes the tile sums the slots in slice
-      // order -- all of its loads in flight at once (one L2 round trip, not one per slice) -- and writes the output
-      __syncthreads();                              // the slot is written by all four warps
-      if (tid == 0) {
-        __threadfence();                            // ... and visible before the slice is counted
-        const uint32_t old = atomicAdd(p.counters[z] + blockIdx.x, 1u);
-        const int last = (int)old == ns - 1;
-        if (last) __threadfence();                  // the other slices' slots are visible to what follows
-        s_last = last;
-      }
-      __syncthreads();
-      if (s_last) {
-        const int64_t f = (int64_t)f0 + fl;
-        const float4* src = reinterpret_cast<const float4*>(p.slots[z]) + (int64_t)blockIdx.x * ns * (128 * R / 4) + fl;
-        constexpr int QB = 2;        // column quads per batch: QB * ns loads in flight per thread
-#pragma unroll 1
-        for (int q0 = 0; q0 < QH; q0 += QB) {
-          float4 acc[QB];
-#pragma unroll
-          for (int j = 0; j < QB; ++j) acc[j] = make_float4(0.f, 0.f, 0.f, 0.f);
-          for (int s0 = 0; s0 < ns; s0 += 8) {
-            float4 v[QB][8];
-#pragma unroll
-            for (int j = 0; j < QB; ++j)
-#pragma unroll
-              for (int k = 0; k < 8; ++k)
-                v[j][k] = (s0 + k < ns) ? __ldcg(src + (int64_t)(s0 + k) * (128 * R / 4) + (q0 + j) * 128)
-                                        : make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-            for (int j = 0; j < QB; ++j)
-#pragma unroll
-              for (int k = 0; k < 8; ++k) {
-                acc[j].x += v[j][k].x;
-                acc[j].y += v[j][k].y;
-                acc[j].z += v[j][k].z;
-                acc[j].w += v[j][k].w;
-              }
-          }
-          if (f < F) {
-#pragma unroll
-            for (int j = 0; j < QB; ++j) {
-              float4* o = reinterpret_cast<float4*>(p.out[z] + f * R + (q0 + j) * 4);
-              if (p.accumulate) {
-                const float4 old = *o;
-                acc[j].x += old.x;
-                acc[j].y += old.y;
-                acc[j].z += old.z;
-                acc[j].w += old.w;
-              }
-              *o = acc[j];
-            }
-          }
-        }
-        if (tid == 0) p.counters[z][blockIdx.x] = 0u;   // back to zero for the next call
-      }
     }
   }
   __syncthreads();
@@ -341,7 +278,7 @@ k_wgrad(const __grid_constant__ CUtensorMap map_in0, const __grid_constant__ CUt
   if (p.late_wait) pdl_wait();
 }
 
-// one-time per-device setup: shared-memory opt-in and the largest carveout (three CTAs of 61 KB per SM)
+// one-time per-device setup: shared-memory opt-in and the largest carveout
 template <int R, int FW>
 static int wg_prepare() {
   static bool done[FT_MAX_DEVICES] = {};
@@ -354,7 +291,7 @@ static int wg_prepare() {
   return FT_OK;
 }
 
-// CLUSTER shape: how many clusters (1, s, 1) the device holds at once (cached per device and s): a grid that does
+// how many clusters (1, s, 1) the device holds at once (cached per device and s): a grid that does
 // not fit in one wave runs its last clusters alone
 template <int R>
 static int wg_max_active_clusters(int s) {
@@ -395,7 +332,7 @@ static int launch_wg(const CUtensorMap* maps, const WgParams& p, dim3 grid, bool
   cfg.stream = st;
   cudaLaunchAttribute attr[2];
   int na = 0;
-  if (FW == 256 && grid.y > 1) {   // CLUSTER: the M slices of a feature tile form one cluster
+  if (grid.y > 1) {   // the M slices of a feature tile form one cluster
     attr[na].id = cudaLaunchAttributeClusterDimension;
     attr[na].val.clusterDim.x = 1;
     attr[na].val.clusterDim.y = grid.y;
@@ -443,25 +380,21 @@ static int launch_wg_r(int r, const CUtensorMap* maps, const WgParams& p, dim3 g
 }
 
 // which = 1: dA [K x r] = X^T P[:, r_s:];  which = 2: dBt [N x r] = G^T H[:, r_s:];  which = 3: both in
-// ONE launch (blockIdx.z picks the problem).
-// workspace != NULL (the caller's layer workspace, control words zero): the SLOTS shape -- 128-feature tiles, three
-//   CTAs per SM, M slices sized for one wave, combined through slots and arrival counters of the workspace.
-// workspace == NULL: the CLUSTER shape -- 256-feature tiles, at most 8 M slices = one cluster, combined over
-//   distributed shared memory.
-// Either way: no clear kernel, no atomics on the data, a fixed order of additions.
+// ONE launch (blockIdx.z picks the problem).  The M slices (at most 8, the portable cluster size) of a feature
+// tile are one cluster and combine over distributed shared memory in slice order: no clear kernel, no atomics on
+// the data, no workspace, a fixed order of additions.
 // amax_g (which & 2 only): zero word that receives the bit pattern of max |G|.
 // after_kernel: the launch directly follows a kernel of the same call (programmatic edge allowed).
 // beside_prev: see WgParams::late_wait (the caller's promise).
 int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, int64_t N, const void* p_saved,
                  const void* h_saved, int r_t, int r_s, int r, float* dA, float* dBt, int accumulate,
-                 unsigned int* amax_g, void* workspace, bool after_kernel, bool beside_prev, cudaStream_t st) {
+                 unsigned int* amax_g, bool after_kernel, bool beside_prev, cudaStream_t st) {
+  constexpr int FW = 256;
   CUtensorMap maps[4];
   const void* in_all[2] = {x, g};
   const void* lr_all[2] = {p_saved, h_saved};
   const int64_t F_all[2] = {K, N};
   float* out_all[2] = {dA, dBt};
-  const bool slots_shape = workspace != nullptr;
-  const int FW = slots_shape ? 128 : 256;
   WgParams p;
   p.M = M;
   p.r_s = r_s;
@@ -472,37 +405,22 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
   int sel[2], nz = 0;
   for (int z = 0; z < 2; ++z)
     if (which & (1 << z)) sel[nz++] = z;
-  int64_t f_tiles_total = 0, f_tiles_max = 0;
-  for (int i = 0; i < nz; ++i) {
-    const int64_t ft = ceil_div(F_all[sel[i]], FW);
-    f_tiles_total += ft;
-    if (ft > f_tiles_max) f_tiles_max = ft;
-  }
-  int64_t slices = 1;
-  if (slots_shape) {
-    if (f_tiles_max > WS_MAX_FEATURE_TILES) return FT_ERR_UNSUPPORTED_SHAPE;
-    // one wave of three CTAs per SM over all feature tiles (rounded DOWN: a second, mostly empty wave costs more
-    // than slightly longer slices), at least 4 chunks (256 rows) each, and no more slices than the workspace
-    // has slots for
-    slices = (int64_t)3 * sm_count() / f_tiles_total;
-    if (slices > chunks / 4) slices = chunks / 4;
-    if (slices * f_tiles_total > WS_MAX_WGRAD_SLOTS) slices = WS_MAX_WGRAD_SLOTS / f_tiles_total;
-    if (slices < 1) slices = 1;
-  } else {
-    // M slices = cluster size, at most 8, at least 4 chunks each: the count s that minimises waves(s) x chunks
-    // per slice, where waves(s) = clusters of the launch / clusters of size s the device holds at once (one CTA
-    // per SM, and clusters of 3 or more strand a few SMs: 148, 74, 45, 33, 26, 22, 15, 15 on B200)
-    int64_t max_slices = chunks / 4;
-    if (max_slices > 8) max_slices = 8;
-    if (max_slices < 1) max_slices = 1;
-    int64_t best_cost = -1;
-    for (int64_t s = 1; s <= max_slices; ++s) {
-      const int64_t cap = wg_clusters_for(r, (int)s);
-      const int64_t cost = ceil_div(f_tiles_total, cap) * ceil_div(chunks, s);
-      if (best_cost < 0 || cost < best_cost) {
-        best_cost = cost;
-        slices = s;
-      }
+  int64_t f_tiles_total = 0;
+  for (int i = 0; i < nz; ++i) f_tiles_total += ceil_div(F_all[sel[i]], FW);
+  // M slices = cluster size, at most 8, at least 4 chunks (256 rows) each: the count s that minimises
+  // waves(s) x chunks per slice, where waves(s) = clusters of the launch / clusters of size s the device holds at
+  // once (one CTA per SM, and clusters of 3 or more strand a few SMs: 148, 74, 45, 33, 26, 22, 15, 15 on B200) --
+  // a launch that spills into a second wave runs its last clusters alone
+  int64_t max_slices = chunks / 4;
+  if (max_slices > 8) max_slices = 8;
+  if (max_slices < 1) max_slices = 1;
+  int64_t slices = 1, best_cost = -1;
+  for (int64_t s = 1; s <= max_slices; ++s) {
+    const int64_t cap = wg_clusters_for(r, (int)s);
+    const int64_t cost = ceil_div(f_tiles_total, cap) * ceil_div(chunks, s);
+    if (best_cost < 0 || cost < best_cost) {
+      best_cost = cost;
+      slices = s;
     }
   }
   const int cpc = (int)ceil_div(chunks, slices);
@@ -510,8 +428,6 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
   p.n_slices = (int)sl;
   p.chunks_per_cta = cpc;
   unsigned gx = 0;
-  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
-  float* slot_cursor = ws ? reinterpret_cast<float*>(ws + ws_layout(M, r_t).wg_slots_off) : nullptr;
   for (int i = 0; i < 2; ++i) {
     const int z = i < nz ? sel[i] : sel[0];
     int rc = make_tensor_map_2d(&maps[2 * i], in_all[z], 2, (uint64_t)F_all[z], (uint64_t)M, (uint64_t)F_all[z] * 2, 64,
@@ -523,15 +439,8 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
     p.F[i] = F_all[z];
     p.out[i] = out_all[z];
     p.amax_bits[i] = z == 1 ? amax_g : nullptr;
-    p.slots[i] = nullptr;
-    p.counters[i] = nullptr;
     if (i >= nz) continue;
     const unsigned ft = (unsigned)ceil_div(F_all[z], FW);
-    if (slots_shape && sl > 1) {
-      p.slots[i] = slot_cursor;
-      slot_cursor += (size_t)ft * sl * 128 * r;
-      p.counters[i] = reinterpret_cast<uint32_t*>(ws + WS_CTL_WGTILES) + (size_t)z * WS_MAX_FEATURE_TILES;
-    }
     if (ft > gx) gx = ft;
   }
   const dim3 grid(gx, sl, (unsigned)nz);
@@ -541,7 +450,7 @@ int launch_wgrad(int which, const void* x, const void* g, int64_t M, int64_t K, 
   p.dbg = getenv("FT_WG_DBG") ? atoi(getenv("FT_WG_DBG")) : 0;
   if (p.dbg & 2) p.amax_bits[0] = p.amax_bits[1] = nullptr;
 #endif
-  return slots_shape ? launch_wg_r<128>(r, maps, p, grid, pdl, st) : launch_wg_r<256>(r, maps, p, grid, pdl, st);
+  return launch_wg_r<256>(r, maps, p, grid, pdl, st);
 }
 
 }  // namespace ft
