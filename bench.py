@@ -606,6 +606,8 @@ def sweep(B, prepare, dev, graph_us, peaks, full=False):
         return ours, base
 
     out["fusion_ablation_C2"] = fusion_ablation(B, dev, acts, g)
+    out["mlp_fusion_C3"] = mlp_fusion(B, dev, acts, g, graph_us)
+    torch.cuda.empty_cache()
     cfgs = {"C1": (256, 3072, 3072, 32, 16), "C3u": (4608, 3072, 12288, 32, 64), "C3d": (4608, 12288, 3072, 32, 64)}
     out["configs"] = {}
     for name, (M, K, N, r_s, r) in cfgs.items():
@@ -632,6 +634,75 @@ def sweep(B, prepare, dev, graph_us, peaks, full=False):
                                    "bf16_lora_ms": round(tot_base / 1e3, 2),
                                    "speedup_vs_bf16_lora": round(tot_base / tot_ours, 2)}
     return out
+
+
+def mlp_fusion(B, dev, acts, g, graph_us):
+    """NEXT-1 ("further fusing the MLP components provides an additional 1.10x"): the FLUX-shaped
+    MLP pair of BASELINE.json configs[2] (M=4608, 3072 -> 12288 -> GeLU -> 3072, r_s=32, r=64), forward and backward,
+    with and without the MLP fusion.  Unfused = the two LoRA-fused layers with bf16 Y1 and Z in HBM and the GeLU
+    (forward and backward) as torch elementwise kernels.  Fused = ft_mlp_fwd (GeLU, FC2's quantize and
+    down-projection in FC1's GEMM epilogue; Y1 and Z kept as NVFP4 only) and a backward on the 4-bit saved
+    activations: ft_linear_bwd_q4(FC2), ft_gelu_bwd_q4, ft_linear_bwd_q4(FC1)."""
+    import torch
+    import torch.nn.functional as F
+    M, K, N1, N2, r_s, r = 4608, 3072, 12288, 3072, 32, 64
+    r_t = r_s + r
+    X, G2 = acts(M, K), acts(M, N2, grad=True)
+
+    def mk(n, k, ntile):
+        W = (torch.randn(n, k, device=dev, generator=g) * 0.02).to(torch.bfloat16)
+        D = (torch.randn(k, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
+        U = (torch.randn(n, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
+        return B.Layer(W, D, U, r_s, r, ntile=ntile)
+    fc1, fc2 = mk(N1, K, 224), mk(N2, N1, 224)
+    # the same FC1 with its forward scales cut to 192-wide tiles (what ft_mlp_fwd's GEMM runs); weights are random, so
+    # a second random matrix of the same shape serves the timing
+    fc1f = mk(N1, K, 192)
+    bf = torch.bfloat16
+    y1 = torch.empty(M, N1, dtype=bf, device=dev); z = torch.empty_like(y1); dz = torch.empty_like(y1); dy1 = torch.empty_like(y1)
+    y2 = torch.empty(M, N2, dtype=bf, device=dev); dx = torch.empty(M, K, dtype=bf, device=dev)
+    h1 = torch.empty(M, r_t, dtype=bf, device=dev); h2 = torch.empty_like(h1); p1 = torch.empty_like(h1); p2 = torch.empty_like(h1)
+    qx, qz, qy1 = B.QTensor(M, K, device=dev), B.QTensor(M, N1, device=dev), B.QTensor(M, N1, device=dev)
+    qg2, qg1 = B.QTensor(M, N2, device=dev), B.QTensor(M, N1, device=dev)
+    ws = B.new_mlp_workspace(M, max(K, N1), N1, r_t, r_t, dev)
+    ws2 = B.new_workspace(M, N1, N1, r_t, dev)
+    dA1 = torch.empty(K, r, dtype=torch.float32, device=dev); dB1 = torch.empty(N1, r, dtype=torch.float32, device=dev)
+    dA2 = torch.empty(N1, r, dtype=torch.float32, device=dev); dB2 = torch.empty(N2, r, dtype=torch.float32, device=dev)
+    za = torch.empty(1, device=dev); ya = torch.empty(1, device=dev)
+
+    def fwd_unfused():
+        B.ft_linear_fwd(fc1, X, y1, h1, qx, ws2)
+        torch.ops.aten.gelu.out(y1, approximate="tanh", out=z)
+        B.ft_linear_fwd(fc2, z, y2, h2, qz, ws2)
+
+    def bwd_unfused():
+        B.ft_linear_bwd(fc2, z, G2, h2, dz, p2, dA2, dB2, qg2, ws2)
+        torch.ops.aten.gelu_backward.grad_input(dz, y1, approximate="tanh", grad_input=dy1)
+        B.ft_linear_bwd(fc1, X, dy1, h1, dx, p1, dA1, dB1, qg1, ws2)
+    fwd_unfused()
+    torch.cuda.synchronize()
+    za.copy_(z.float().abs().max()); ya.copy_(y1.float().abs().max())     # "the previous step's" amax
+
+    def fwd_fused():
+        B.ft_mlp_fwd(fc1f, fc2, X, za, ya, y2, h1, h2, qx, qz, qy1, ws)
+
+    def bwd_fused():
+        B.ft_linear_bwd_q4(fc2, qz, G2, h2, dz, p2, dA2, dB2, qg2, ws2)
+        B.ft_gelu_bwd_q4(dz, qy1, dz)
+        B.ft_linear_bwd_q4(fc1, qx, dz, h1, dx, p1, dA1, dB1, qg1, ws2)
+    res = {}
+    res["fwd_unfused_us"] = round(graph_us([fwd_unfused], 10), 1)
+    res["fwd_fused_us"] = round(graph_us([fwd_fused], 10), 1)
+    res["fwd_bwd_unfused_us"] = round(graph_us([lambda: (fwd_unfused(), bwd_unfused())], 10), 1)
+    res["fwd_bwd_fused_us"] = round(graph_us([lambda: (fwd_fused(), bwd_fused())], 10), 1)
+    res["fwd_speedup"] = round(res["fwd_unfused_us"] / res["fwd_fused_us"], 3)
+    res["fwd_bwd_speedup"] = round(res["fwd_bwd_unfused_us"] / res["fwd_bwd_fused_us"], 3)
+    res["activation_bytes_kept_unfused"] = 2 * M * K + 2 * 2 * M * N1       # bf16 X, Y1, Z
+    res["activation_bytes_kept_fused"] = int(0.5625 * (M * K + 2 * M * N1))  # Q(X), Q(Y1), Q(Z)
+    res["note"] = ("CUDA graphs, 10 replays; unfused = two LoRA-fused layers + torch GeLU kernels, bf16 Y1 and Z in HBM; fused = "
+                   "ft_mlp_fwd + backward on the 4-bit saved activations (delayed-scaling amax for Q(Z), Q(Y1): reading "
+                   "O-16); paper (other GPUs, whole DiT): MLP fusion +1.10x (PAPER.md:245)")
+    return res
 
 
 def fusion_ablation(B, dev, acts, g):

@@ -80,7 +80,7 @@ typedef struct {
   int32_t block_rows;      /* 1 (activations, gradients) or 16 (weights, 16x16 blocks)  */
   int32_t sf_layout;       /* FT_SF_ROWMAJOR or FT_SF_TILE128x4                          */
   /* optional, weights only (NULL / 0 otherwise): the same scales once more, cut to the GEMM's output-tile
-   * width `ntile` (224): for row tile nt = row / ntile and K=64 step ks two 512-byte groups -- rows
+   * width `ntile` (224, or 192 for the FC1 of ft_mlp_fwd): for row tile nt = row / ntile and K=64 step ks two 512-byte groups -- rows
    * nt*ntile + 0..127 and + 128..ntile-1 of the tile, each in the (r%32)*16 + (r/32)*4 + c%4 order of
    * FT_SF_TILE128x4, rows past the tile or the tensor zero -- at ((nt * cols/64 + ks) * 2 + half) * 512.
    * ft_sf_ntile_bytes() bytes, filled by ft_pack_weight.  With it ft_gemm4 / ft_linear_* may run 256 x ntile
@@ -148,7 +148,7 @@ int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols,
  * value copied), and, if r_kmajor_tiled != NULL, the TILE128x4 expansion of the
  * forward operand's scales (its codes/tensor_dec_scale pointers are not written;
  * point them at r_kmajor's buffers).  For each of the two outputs whose sf_ntile is non-NULL and whose ntile
- * is 224, the tile-cut copy of the scales as well.  N % 64 == 0 and K % 64 == 0. */
+ * is 224 or 192, the tile-cut copy of the scales as well.  N % 64 == 0 and K % 64 == 0. */
 int ft_pack_weight(const ft_qtensor* r_kmajor, ft_qtensor* r_kmajor_tiled,
                    ft_qtensor* r_nmajor, void* stream);
 
@@ -217,6 +217,37 @@ int ft_linear_bwd_q4(const ft_layer* L, const ft_qtensor* qx, const void* g_bf16
                      const void* h_saved_bf16, void* dx_bf16, void* p_saved_bf16, float* dA, float* dBt,
                      int32_t accumulate, ft_qtensor* qg_scratch, void* workspace, size_t workspace_bytes,
                      void* stream);
+
+/* ---- NEXT-1, MLP fusion (sec. 3.3 "MLP Fusion"; reading O-16): the forward of
+ * FC1 -> GeLU -> FC2 with the FC1 GEMM's epilogue doing GeLU and FC2's quantize + down-projection, so that neither
+ * Y1 = FC1(X) nor Z = gelu(Y1) ([M x N1] bf16 each) is written to global memory.
+ *   fc1: K -> N1, its r_kmajor.sf_ntile cut to 192-wide tiles (ntile == 192); fc2: N1 -> N2.
+ *   x_bf16 [M x K] -> y2_bf16 [M x N2].
+ *   z_amax, y1_amax: device floats, the tensor amax the quantizers of Z and of Y1 use (delayed scaling: normally the
+ *     value the previous step left in z_amax_next / y1_amax_next; a GEMM epilogue cannot know max |Z| before its
+ *     last tile).  z_amax_next, y1_amax_next: device floats (or both NULL) that receive THIS step's max |Z|, max |Y1|.
+ *   Outputs kept for backward: h1_saved [M x r_t1] = bf16(X D_f1), h2_saved [M x r_t2] = bf16(Z D_f2),
+ *     qx = Q(X), qz = Q(Z) (FC2's activation operand; its dA uses it, ft_linear_bwd_q4), qy1 = Q(Y1) (the
+ *     pre-activation, consumed by ft_gelu_bwd_q4); all three caller-allocated like qx_scratch of ft_linear_fwd.
+ *   z_debug_bf16, y1_debug_bf16: NULL, or both [M x N1] bf16 buffers that receive copies of Z and Y1 (parity tests:
+ *     the staged comparison of DESIGN.md O-11 needs the bits the quantizers consumed).
+ *   workspace >= ft_mlp_workspace_bytes(M, K, N1, r_t1, r_t2), control words zero (as for every call).
+ * Requirements: K % 64 == 0, N1 % 192 == 0, N2 % 64 == 0, 16 <= r_t2 <= 112, fc1->N == fc2->K == N1.
+ * The GeLU is the tanh form evaluated in fp32 on bf16(Y1), as y sigmoid(2 t) with the hardware's exp2 and
+ * reciprocal approximations (2^-22 relative); Z = bf16(gelu). */
+int ft_mlp_fwd(const ft_layer* fc1, const ft_layer* fc2, const void* x_bf16, int64_t M,
+               const float* z_amax, const float* y1_amax, float* z_amax_next, float* y1_amax_next,
+               void* y2_bf16, void* h1_saved_bf16, void* h2_saved_bf16,
+               ft_qtensor* qx, ft_qtensor* qz, ft_qtensor* qy1, void* z_debug_bf16, void* y1_debug_bf16,
+               void* workspace, size_t workspace_bytes, void* stream);
+size_t ft_mlp_workspace_bytes(int64_t M, int64_t K, int64_t N1, int32_t r_t1, int32_t r_t2);
+/* Byte offset of FC2's pre-scaled intermediate Hs2 [M x r_t2] inside the workspace of ft_mlp_fwd (FC1's Hs1 is at
+ * ft_workspace_hs_offset(M, r_t1)). */
+size_t ft_mlp_workspace_hs2_offset(int64_t M, int32_t r_t1);
+
+/* ---- GeLU backward of the fused MLP: dy1_bf16 [M x N1] = bf16( dz_bf16 * gelu'(dequant(qy1)) ), qy1 = the Q(Y1)
+ * ft_mlp_fwd saved (reading O-16).  dz and dy1 may be the same buffer. */
+int ft_gelu_bwd_q4(const void* dz_bf16, const ft_qtensor* qy1, void* dy1_bf16, void* stream);
 
 /* ---- sizes and diagnostics (host only, no CUDA calls) */
 size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout);

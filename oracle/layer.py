@@ -154,18 +154,26 @@ def wgrad_saved4(qX, G, H, P, r_s):
 # mlp_forward below is written as that composition, so "fused == unfused" holds by construction and the CUDA
 # kernel is what has to match it.
 
-def gelu_tanh(y):
-    """GeLU, tanh form: 0.5 y (1 + tanh( sqrt(2/pi) (y + 0.044715 y^3) )), float64."""
+def _gelu_sigmoid(y):
+    """0.5 (1 + tanh t) = 1 / (1 + exp(-2 t)), t = sqrt(2/pi) (y + 0.044715 y^3), float64.  The same function as
+    the tanh expression, written so that it does not cancel: 1 + tanh(t) loses all its digits in float64 once
+    t < -18 (y < -5.3), where the value is 1e-16 .. 1e-37 -- still a normal bf16 number."""
     y = np.asarray(y, dtype=np.float64)
-    return 0.5 * y * (1.0 + np.tanh(np.sqrt(2.0 / np.pi) * (y + 0.044715 * y * y * y)))
+    t = np.sqrt(2.0 / np.pi) * (y + 0.044715 * y * y * y)
+    with np.errstate(over="ignore"):
+        return 1.0 / (1.0 + np.exp(-2.0 * t))
+
+
+def gelu_tanh(y):
+    """GeLU, tanh form: 0.5 y (1 + tanh( sqrt(2/pi) (y + 0.044715 y^3) )) = y sigmoid(2 t), float64."""
+    return np.asarray(y, dtype=np.float64) * _gelu_sigmoid(y)
 
 
 def gelu_tanh_grad(y):
-    """d/dy of gelu_tanh, float64:  0.5 (1 + t) + 0.5 y (1 - t^2) sqrt(2/pi) (1 + 3 * 0.044715 y^2),  t = tanh(.)."""
+    """d/dy of gelu_tanh, float64: with s = sigmoid(2 t),  s + y s (1 - s) 2 sqrt(2/pi) (1 + 3 * 0.044715 y^2)."""
     y = np.asarray(y, dtype=np.float64)
-    c = np.sqrt(2.0 / np.pi)
-    t = np.tanh(c * (y + 0.044715 * y * y * y))
-    return 0.5 * (1.0 + t) + 0.5 * y * (1.0 - t * t) * c * (1.0 + 3.0 * 0.044715 * y * y)
+    s = _gelu_sigmoid(y)
+    return s + y * s * (1.0 - s) * 2.0 * np.sqrt(2.0 / np.pi) * (1.0 + 3.0 * 0.044715 * y * y)
 
 
 def mlp_forward(X, qR1, D1, U1, qR2, D2, U2, z_amax, y1_amax, Y1_given=None, Z_given=None, H1s_given=None,

@@ -62,6 +62,13 @@ def lib():
         L.ft_linear_bwd_q4.argtypes = [C.POINTER(_Layer), C.POINTER(_QT), vp, i64, vp, vp, vp, vp, vp, i32, C.POINTER(_QT), vp, sz, vp]
         L.ft_sf_bytes.argtypes = [i64, i64, i32, i32]
         L.ft_sf_bytes.restype = sz
+        L.ft_mlp_fwd.argtypes = [C.POINTER(_Layer), C.POINTER(_Layer), vp, i64, vp, vp, vp, vp, vp, vp, vp, C.POINTER(_QT),
+                                 C.POINTER(_QT), C.POINTER(_QT), vp, vp, vp, sz, vp]
+        L.ft_mlp_workspace_bytes.argtypes = [i64, i64, i64, i32, i32]
+        L.ft_mlp_workspace_bytes.restype = sz
+        L.ft_mlp_workspace_hs2_offset.argtypes = [i64, i32]
+        L.ft_mlp_workspace_hs2_offset.restype = sz
+        L.ft_gelu_bwd_q4.argtypes = [vp, C.POINTER(_QT), vp, vp]
         L.ft_sf_ntile_bytes.argtypes = [i64, i64, i32]
         L.ft_sf_ntile_bytes.restype = sz
         L.ft_workspace_bytes.argtypes = [i64, i64, i64, i32]
@@ -183,7 +190,8 @@ def ft_quantize_blockwise(x, out, tensor_amax=None, down=None, h_out=None, hs_ou
 class Layer:
     """ft_layer: Q(R) in both orientations plus the low-rank factors D_f [K x r_t], U_t [N x r_t]."""
 
-    def __init__(self, R_bf16, D_f, U_t, r_s, r, stream=None):
+    def __init__(self, R_bf16, D_f, U_t, r_s, r, stream=None, ntile=224):
+        """ntile: width of the tile-cut copy of the forward operand's scales (224; 192 for the FC1 of ft_mlp_fwd)."""
         _bf16(R_bf16)
         N, K = R_bf16.shape
         self.N, self.K, self.r_s, self.r = N, K, r_s, r
@@ -195,7 +203,7 @@ class Layer:
         # a6: offline quantize (16x16 blocks, row-major S) then re-pack both orientations
         self.q_rowmajor = QTensor(N, K, 16, FT_SF_ROWMAJOR, dev)
         ft_quantize_blockwise(R_bf16, self.q_rowmajor, stream=stream)
-        self.r_kmajor = QTensor(N, K, 16, FT_SF_TILE128x4, dev).with_ntile(224)
+        self.r_kmajor = QTensor(N, K, 16, FT_SF_TILE128x4, dev).with_ntile(ntile)
         self.r_kmajor.codes = self.q_rowmajor.codes
         self.r_kmajor.tensor_dec_scale = self.q_rowmajor.tensor_dec_scale
         self.r_nmajor = QTensor(K, N, 16, FT_SF_TILE128x4, dev).with_ntile(224)
@@ -269,6 +277,34 @@ def ft_linear_bwd_q4(layer, qx, g, h_saved, dx, p_saved, dA, dBt, qg, workspace,
                                   workspace.numel(), _stream(stream)))
     qg.sync_from(q)
     return dx, dA, dBt
+
+
+def new_mlp_workspace(M, K, N1, r_t1, r_t2, device="cuda"):
+    ws = torch.empty(lib().ft_mlp_workspace_bytes(M, K, N1, r_t1, r_t2), dtype=torch.uint8, device=device)
+    return ft_workspace_init(ws)
+
+
+def mlp_workspace_hs2(workspace, M, r_t1, r_t2):
+    off = lib().ft_mlp_workspace_hs2_offset(M, r_t1)
+    return workspace[off:off + M * r_t2 * 2].view(torch.bfloat16).view(M, r_t2)
+
+
+def ft_mlp_fwd(fc1, fc2, x, z_amax, y1_amax, y2, h1, h2, qx, qz, qy1, workspace, z_amax_next=None, y1_amax_next=None,
+               z_debug=None, y1_debug=None, stream=None):
+    """FC1 -> GeLU -> FC2 with the FC1 GEMM's epilogue doing GeLU and FC2's quantize + down-projection (NEXT-1)."""
+    _bf16(x)
+    L1, L2, a, b, c = fc1.c(), fc2.c(), qx.c(), qz.c(), qy1.c()
+    _check(lib().ft_mlp_fwd(C.byref(L1), C.byref(L2), _ptr(x), x.shape[0], _ptr(z_amax), _ptr(y1_amax),
+                            _ptr(z_amax_next), _ptr(y1_amax_next), _ptr(y2), _ptr(h1), _ptr(h2), C.byref(a), C.byref(b),
+                            C.byref(c), _ptr(z_debug), _ptr(y1_debug), _ptr(workspace), workspace.numel(), _stream(stream)))
+    qx.sync_from(a), qz.sync_from(b), qy1.sync_from(c)
+    return y2
+
+
+def ft_gelu_bwd_q4(dz, qy1, out, stream=None):
+    q = qy1.c()
+    _check(lib().ft_gelu_bwd_q4(_ptr(dz), C.byref(q), _ptr(out), _stream(stream)))
+    return out
 
 
 # test / bench hooks of include/fourtune_debug.h (not part of the product interface)

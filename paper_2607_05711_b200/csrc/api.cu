@@ -33,6 +33,26 @@ int launch_wgrad_q4(const uint8_t* codes, const uint8_t* sf, const float* g_dec,
                     const void* p_saved, int r_t, int r_s, int r, float* dA, int accumulate, bool beside_prev,
                     cudaStream_t st);
 
+int launch_gemm4_mlp(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N1, int64_t K, const void* lr_a,
+                     const void* lr_b, int r_t, const void* d2, int r2, const float* g_dec_r2, const float* z_amax_in,
+                     const float* y1_amax_in, ft_qtensor* qz, ft_qtensor* qy1, unsigned int* z_amax_out,
+                     unsigned int* y1_amax_out, void* z_dbg, void* y1_dbg, void* h2, void* hs2, float* slots,
+                     cudaStream_t st);
+int launch_gelu_bwd_q4(const void* dz, const ft_qtensor* qy1, void* out, cudaStream_t st);
+
+// workspace of ft_mlp_fwd: the layer workspace of FC1, then Hs2, then the H2 slots (96 pairs + row tiles)
+struct MlpWs {
+  size_t hs2_off, slots_off, total;
+};
+static MlpWs mlp_ws(int64_t M, int r_t1, int r_t2) {
+  auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+  MlpWs w;
+  w.hs2_off = up(ws_layout(M, r_t1).total);
+  w.slots_off = w.hs2_off + up((size_t)M * r_t2 * 2);
+  w.total = w.slots_off + (size_t)(96 + ceil_div(M, 256)) * 256 * (size_t)r_t2 * 4 + 256;
+  return w;
+}
+
 // ------------------------------------------------------------- device queries
 // SM count of the CURRENT device, cached per device ordinal (a process may drive several GPUs)
 int current_device() {
@@ -334,7 +354,7 @@ int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, v
   if (rk_tiled && !rk_tiled->sf) return FT_ERR_INVALID_ARG;
   const ft_qtensor* outs[2] = {rk_tiled, rn};
   for (int i = 0; i < 2; ++i)
-    if (outs[i] && outs[i]->sf_ntile != nullptr && (outs[i]->ntile != 224 || !aligned16(outs[i]->sf_ntile)))
+    if (outs[i] && outs[i]->sf_ntile != nullptr && ((outs[i]->ntile != 224 && outs[i]->ntile != 192) || !aligned16(outs[i]->sf_ntile)))
       return FT_ERR_INVALID_ARG;
   if (rk->rows % 64 != 0 || rk->cols % 64 != 0 || rk->rows < 64 || rk->cols < 64)
     return FT_ERR_UNSUPPORTED_SHAPE;
@@ -370,6 +390,91 @@ int ft_gemm4(const ft_qtensor* a, const ft_qtensor* b, const void* lr_a_scaled, 
   if (rc != FT_OK) return rc;
   return launch_gemm4(a, b, a->rows, b->rows, a->cols, lr_a_scaled, lr_b, r_t, out_bf16, false,
                       (cudaStream_t)stream);
+}
+
+size_t ft_mlp_workspace_bytes(int64_t M, int64_t K, int64_t N1, int32_t r_t1, int32_t r_t2) {
+  (void)K;
+  (void)N1;
+  if (M < 0 || r_t1 < 0 || r_t2 < 0) return 0;
+  return mlp_ws(M, r_t1, r_t2).total;
+}
+
+size_t ft_mlp_workspace_hs2_offset(int64_t M, int32_t r_t1) { return mlp_ws(M, r_t1, 16).hs2_off; }
+
+int ft_mlp_fwd(const ft_layer* fc1, const ft_layer* fc2, const void* x_bf16, int64_t M, const float* z_amax,
+               const float* y1_amax, float* z_amax_next, float* y1_amax_next, void* y2_bf16, void* h1_saved_bf16,
+               void* h2_saved_bf16, ft_qtensor* qx, ft_qtensor* qz, ft_qtensor* qy1, void* z_debug_bf16,
+               void* y1_debug_bf16, void* workspace, size_t workspace_bytes, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc = check_layer(fc1);
+  if (rc != FT_OK) return rc;
+  rc = check_layer(fc2);
+  if (rc != FT_OK) return rc;
+  if (!x_bf16 || !z_amax || !y1_amax || !y2_bf16 || !h1_saved_bf16 || !h2_saved_bf16 || !qx || !qz || !qy1 || !workspace)
+    return FT_ERR_INVALID_ARG;
+  if ((z_amax_next == nullptr) != (y1_amax_next == nullptr) || (z_debug_bf16 == nullptr) != (y1_debug_bf16 == nullptr))
+    return FT_ERR_INVALID_ARG;
+  const ft_qtensor* qs[3] = {qx, qz, qy1};
+  for (int i = 0; i < 3; ++i)
+    if (!qs[i]->codes || !qs[i]->sf || !qs[i]->tensor_dec_scale || !aligned16(qs[i]->codes) || !aligned16(qs[i]->sf))
+      return FT_ERR_INVALID_ARG;
+  const int r1 = fc1->r_s + fc1->r, r2 = fc2->r_s + fc2->r;
+  const int64_t K = fc1->K, N1 = fc1->N, N2 = fc2->N;
+  if (fc2->K != N1 || M < 1 || N1 % 192 != 0 || r2 < 16 || r2 > 112 || r1 < 16) return FT_ERR_UNSUPPORTED_SHAPE;
+  if (fc1->r_kmajor.sf_ntile == nullptr || fc1->r_kmajor.ntile != 192) return FT_ERR_INVALID_ARG;
+  if (!aligned16(x_bf16) || !aligned16(y2_bf16) || !aligned16(h1_saved_bf16) || !aligned16(h2_saved_bf16) ||
+      !aligned16(workspace))
+    return FT_ERR_INVALID_ARG;
+  const MlpWs mw = mlp_ws(M, r1, r2);
+  if (workspace_bytes < mw.total) return FT_ERR_WORKSPACE_TOO_SMALL;
+  rc = device_check();
+  if (rc != FT_OK) return rc;
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  if (z_amax_next != nullptr) {
+    FT_CUDA_TRY(cudaMemsetAsync(z_amax_next, 0, sizeof(float), st));
+    FT_CUDA_TRY(cudaMemsetAsync(y1_amax_next, 0, sizeof(float), st));
+  }
+  // FC1: a0 + a1 as in ft_linear_fwd
+  void* hs1 = ws + ws_layout(M, r1).hs_off;
+  void* hs2 = ws + mw.hs2_off;
+  qx->rows = M;
+  qx->cols = K;
+  ft_qtensor* outs[3] = {qx, qz, qy1};
+  for (int i = 0; i < 3; ++i) {
+    outs[i]->block_rows = 1;
+    outs[i]->sf_layout = FT_SF_TILE128x4;
+    outs[i]->sf_ntile = nullptr;
+    outs[i]->ntile = 0;
+  }
+  qz->rows = qy1->rows = M;
+  qz->cols = qy1->cols = N1;
+  ft_proj pr;
+  pr.down = fc1->D_f;
+  pr.out = h1_saved_bf16;
+  pr.out_scaled = hs1;
+  pr.other_dec_scale = fc1->r_kmajor.tensor_dec_scale;
+  pr.r_t = r1;
+  rc = launch_quantize_fused(x_bf16, M, K, nullptr, &pr, qx, workspace, false, nullptr, st);
+  if (rc != FT_OK) return rc;
+  // FC1 GEMM with the fused epilogue (GeLU, Q(Z), Q(Y1), H2 partials) and the sums of the H2 partials
+  rc = launch_gemm4_mlp(qx, &fc1->r_kmajor, M, N1, K, hs1, fc1->U_t, r1, fc2->D_f, r2, fc2->r_kmajor.tensor_dec_scale,
+                        z_amax, y1_amax, qz, qy1, reinterpret_cast<unsigned int*>(z_amax_next),
+                        reinterpret_cast<unsigned int*>(y1_amax_next), z_debug_bf16, y1_debug_bf16, h2_saved_bf16, hs2,
+                        reinterpret_cast<float*>(ws + mw.slots_off), st);
+  if (rc != FT_OK) return rc;
+  // FC2: a2 on Q(Z).  The launch directly follows k_finalize_h2, which writes only H2 and Hs2 and whose every CTA
+  // waited for the fused GEMM: the lr_late invariant of gemm_pair.cu holds
+  return launch_gemm4(qz, &fc2->r_kmajor, M, N2, N1, hs2, fc2->U_t, r2, y2_bf16, true, st);
+}
+
+int ft_gelu_bwd_q4(const void* dz_bf16, const ft_qtensor* qy1, void* dy1_bf16, void* stream) {
+  if (!dz_bf16 || !qy1 || !dy1_bf16 || !qy1->codes || !qy1->sf || !qy1->tensor_dec_scale) return FT_ERR_INVALID_ARG;
+  if (qy1->block_rows != 1 || qy1->sf_layout != FT_SF_TILE128x4 || qy1->cols % 16 != 0 || qy1->rows < 1)
+    return FT_ERR_INVALID_ARG;
+  if (!aligned16(dz_bf16) || !aligned16(dy1_bf16)) return FT_ERR_INVALID_ARG;
+  int rc = device_check();
+  if (rc != FT_OK) return rc;
+  return launch_gelu_bwd_q4(dz_bf16, qy1, dy1_bf16, (cudaStream_t)stream);
 }
 
 int ft_linear_fwd(const ft_layer* L, const void* x_bf16, int64_t M, void* y_bf16,

@@ -675,6 +675,91 @@ def _full_size_sampled(B, seed, M, K, N, r_s, r, kind):
     assert rel(dBt4.cpu().numpy().T, w4["dB"]) <= TOL
 
 
+# ------------------------------------------------------------------ NEXT-1: MLP fusion
+MLP_CASES = [   # seed, M, K, N1, N2, r_s, r1, r2 (LoRA rank of FC2; r_t2 = r_s + r2)
+    (81, 300, 320, 384, 256, 16, 16, 32),       # ragged M, partial K stage, two column tiles
+    (82, 1024, 512, 3072, 512, 32, 64, 64),     # r_t2 = 96 (the C3 ranks), 64 tiles: one per pair
+    (83, 2304, 256, 1920, 320, 16, 16, 16),     # 90 tiles on 74 pairs: ranges that cross a row tile
+    (84, 1100, 512, 7680, 256, 32, 32, 80),     # 200 tiles: 2-3 per pair, r_t2 = 112 (the widest H2 accumulator)
+]
+
+
+@pytest.mark.parametrize("seed,M,K,N1,N2,r_s,r1,r2", MLP_CASES)
+def test_mlp_fused_forward(B, seed, M, K, N1, N2, r_s, r1, r2):
+    """ft_mlp_fwd against oracle.layer.mlp_forward (reading O-16), staged as in O-11: every tensor the CUDA path
+    hands from one stage to the next is checked against the oracle's, then fed to the oracle's next stage bit for
+    bit -- Q(X), H1/Hs1, Y1, Z = bf16(gelu(Y1)), Q(Z) and Q(Y1) with the CALLER's (stale) amax, H2/Hs2, Y2, and this
+    step's amax of Z and Y1."""
+    rng = synth.make_rng(seed)
+    X = synth.outlier_normal(rng, M, K)
+    W1, W2 = synth.normal(rng, (N1, K), 0.05), synth.normal(rng, (N2, N1), 0.02)
+    rt1, rt2 = r_s + r1, r_s + r2
+    R1, L11, L12 = range_finder_split(W1, r_s, seed)
+    R2, L21, L22 = range_finder_split(W2, r_s, seed + 1)
+    D1 = np.concatenate([L11, synth.normal(rng, (K, r1), 0.02)], 1).astype(np.float32)
+    U1 = np.concatenate([L12, synth.normal(rng, (r1, N1), 0.02)], 0).astype(np.float32)
+    D2 = np.concatenate([L21, synth.normal(rng, (N1, r2), 0.02)], 1).astype(np.float32)
+    U2 = np.concatenate([L22, synth.normal(rng, (r2, N2), 0.02)], 0).astype(np.float32)
+    fc1 = B.Layer(t16(R1), t16(D1), t16(U1.T), r_s, r1, ntile=192)
+    fc2 = B.Layer(t16(R2), t16(D2), t16(U2.T), r_s, r2)
+    q1, q2 = olayer.quantize_weight(R1), olayer.quantize_weight(R2)
+    # "the previous step's" amax: 1.5 x and 0.8 x this step's (so the scales differ from a fresh quantization, and
+    # some blocks of Y1 saturate)
+    pre = olayer.forward(X, q1, D1, U1, prescale=True)
+    z_amax = np.float32(1.5) * nvfp4.tensor_amax(nvfp4.bf16_round_from_f64(olayer.gelu_tanh(pre["Y"])))
+    y1_amax = np.float32(0.8) * nvfp4.tensor_amax(pre["Y"])
+    dev = "cuda"
+    y2 = torch.zeros(M, N2, dtype=torch.bfloat16, device=dev)
+    h1 = torch.zeros(M, rt1, dtype=torch.bfloat16, device=dev); h2 = torch.zeros(M, rt2, dtype=torch.bfloat16, device=dev)
+    qx, qz, qy1 = B.QTensor(M, K), B.QTensor(M, N1), B.QTensor(M, N1)
+    zd = torch.zeros(M, N1, dtype=torch.bfloat16, device=dev); yd = torch.zeros_like(zd)
+    za = torch.tensor([z_amax], dtype=torch.float32, device=dev); ya = torch.tensor([y1_amax], dtype=torch.float32, device=dev)
+    zn = torch.full((1,), 7.0, dtype=torch.float32, device=dev); yn = torch.full((1,), 7.0, dtype=torch.float32, device=dev)
+    ws = B.new_mlp_workspace(M, K, N1, rt1, rt2)
+    B.ft_mlp_fwd(fc1, fc2, t16(X), za, ya, y2, h1, h2, qx, qz, qy1, ws, z_amax_next=zn, y1_amax_next=yn, z_debug=zd, y1_debug=yd)
+    torch.cuda.synchronize()
+    hs1, hs2 = npf(B.workspace_hs(ws, M, rt1)), npf(B.mlp_workspace_hs2(ws, M, rt1, rt2))
+    Y1g, Zg = npf(yd), npf(zd)
+    # FC1
+    assert_q_equal(qx, nvfp4.quantize_blockwise(X, 1), B.FT_SF_TILE128x4, B)
+    f1 = olayer.forward(X, q1, D1, U1, prescale=True, H_given=hs1)
+    for got, want in ((npf(h1), f1["H"]), (hs1, f1["Hs"])):
+        assert rel(got, want) <= 2e-3 and (got == want).mean() >= 0.99
+    assert rel(Y1g, f1["Y"]) <= TOL and (Y1g == f1["Y"]).mean() >= 0.95
+    aR1 = np.abs(nvfp4.dequantize_unscaled(q1))
+    ad = np.abs(nvfp4.dequantize_unscaled(f1["qX"])) @ aR1.T + np.abs(hs1.astype(np.float64)) @ np.abs(U1.astype(np.float64))
+    elementwise_ok(Y1g, f1["Y"], f1["alpha"] * ad, "Y1")
+    # GeLU on the CUDA path's own Y1: within one bf16 ulp of the float64 evaluation, almost always identical
+    Zo = nvfp4.bf16_round_from_f64(olayer.gelu_tanh(Y1g))
+    assert (Zg == Zo).mean() >= 0.98
+    assert np.all(np.abs(Zg.astype(np.float64) - Zo) <= np.abs(Zo) * 2.0 ** -7 + 1e-30)   # (flush-to-zero below 1e-37)
+    # the two quantizers, on the CUDA path's own bits and the caller's amax: bit for bit
+    assert_q_equal(qz, nvfp4.quantize_blockwise(Zg, 1, amax_t=z_amax), B.FT_SF_TILE128x4, B)
+    assert_q_equal(qy1, nvfp4.quantize_blockwise(Y1g, 1, amax_t=y1_amax), B.FT_SF_TILE128x4, B)
+    assert zn.cpu().numpy()[0] == nvfp4.tensor_amax(Zg) and yn.cpu().numpy()[0] == nvfp4.tensor_amax(Y1g)
+    # FC2 on that Z
+    f2 = olayer.forward(Zg, q2, D2, U2, prescale=True, x_amax=z_amax, H_given=hs2)
+    for got, want in ((npf(h2), f2["H"]), (hs2, f2["Hs"])):
+        assert rel(got, want) <= 2e-3 and (got == want).mean() >= 0.99
+    Y2g = npf(y2)
+    assert rel(Y2g, f2["Y"]) <= TOL and (Y2g == f2["Y"]).mean() >= 0.95
+    aR2 = np.abs(nvfp4.dequantize_unscaled(q2))
+    ad2 = np.abs(nvfp4.dequantize_unscaled(f2["qX"])) @ aR2.T + np.abs(hs2.astype(np.float64)) @ np.abs(U2.astype(np.float64))
+    elementwise_ok(Y2g, f2["Y"], f2["alpha"] * ad2, "Y2")
+    # and the whole thing is the oracle's mlp_forward when it is handed the same staged tensors
+    o = olayer.mlp_forward(X, q1, D1, U1, q2, D2, U2, z_amax=z_amax, y1_amax=y1_amax, Y1_given=Y1g, Z_given=Zg,
+                           H1s_given=hs1, H2s_given=hs2)
+    assert np.array_equal(o["Y2"], f2["Y"]) and np.array_equal(o["qZ"]["codes"], nvfp4.unpack_codes(qz.codes.cpu().numpy()))
+    # GeLU backward on the saved 4-bit pre-activation
+    dz = synth.student_t_grad(rng, M, N1)
+    dy = torch.zeros(M, N1, dtype=torch.bfloat16, device=dev)
+    B.ft_gelu_bwd_q4(t16(dz), qy1, dy)
+    want = olayer.gelu_backward_saved4(dz, o["qY1"])
+    got = npf(dy)
+    assert rel(got, want) <= 2e-3 and (got == want).mean() >= 0.95
+    assert np.all(np.abs(got.astype(np.float64) - want) <= np.abs(want) * 2.0 ** -6 + 1e-12)
+
+
 def test_without_programmatic_launch():
     """FT_PDL=0 switches every programmatic edge (and with it the late-wait modes of the dA kernels and of the
     dgrad GEMM) off: the plain stream-ordered schedule must give the same answers.  Re-runs the fused-backward,

@@ -303,6 +303,15 @@ def test_gelu_tanh_closed_forms_and_derivative():
     fd = (layer.gelu_tanh(y + h) - layer.gelu_tanh(y - h)) / (2 * h)
     assert np.max(np.abs(fd - layer.gelu_tanh_grad(y))) < 1e-8
     assert abs(layer.gelu_tanh_grad(0.0) - 0.5) < 1e-15
+    # the left tail, where 1 + tanh(t) cancels in float64: against y e^{2t} / (1 + e^{2t}) with e^{2t} tiny and exact
+    # to float64 precision, and against the textbook expression wherever that one still has digits (t > -15)
+    yl = np.linspace(-12.0, -3.0, 91)
+    tl = math.sqrt(2.0 / math.pi) * (yl + 0.044715 * yl ** 3)
+    e2 = np.exp(2.0 * tl)
+    assert np.allclose(layer.gelu_tanh(yl), yl * e2 / (1.0 + e2), rtol=1e-13, atol=0)
+    ok = tl > -15
+    assert np.allclose(layer.gelu_tanh(yl[ok]), 0.5 * yl[ok] * (1.0 + np.tanh(tl[ok])), rtol=1e-3, atol=0)
+    assert layer.gelu_tanh(-9.0) < 0 and abs(layer.gelu_tanh(-9.0)) > 1e-30      # not flushed to zero
 
 
 def test_mlp_forward_is_the_two_layers_with_the_quantizer_in_between():
