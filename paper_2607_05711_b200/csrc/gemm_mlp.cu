@@ -16,14 +16,17 @@
 // Tile order: tiles are numbered 256-row tile major and a pair owns a CONTIGUOUS range (at most two row tiles when
 // the range is no longer than a row of tiles), so that H2 partials are flushed once or twice per pair.
 // TMEM: two 192-column accumulators, 16 scale columns, r2 <= 112 columns of H2: 512.
+// 12 epilogue warps (the epilogue is ~19 instructions per element: the MMAs of a tile take ~5.6 k cycles).
 // Shared memory: 4 ring stages of 34 KB, the 48 KB z tile, the 24 KB D_f2 slice (this CTA's r2 / 2 columns).
+#include <cstdlib>
+
 #include "common.cuh"
 #include "quant_math.cuh"
 
 namespace ft {
 
 constexpr int ML_BM = 256, ML_BN = 192;
-constexpr int ML_THREADS = 384;          // 4 control warps + 8 epilogue warps
+constexpr int ML_THREADS = 512;          // 4 control warps + 12 epilogue warps (three groups, one 64-column unit each)
 constexpr int ML_A_BYTES = 128 * 128;
 constexpr int ML_B_BYTES = (ML_BN / 2) * 128;
 constexpr int ML_SFA_BYTES = 4 * 512;
@@ -54,6 +57,9 @@ struct MlpParams {
   __nv_bfloat16* z_dbg;       // NULL in production: bf16 copies of Z and Y1 for the staged parity comparison
   __nv_bfloat16* y1_dbg;
   float* slots;               // [(pairs + row tiles) x 256 x r2] fp32 partial H2 tiles, layout [quad][row][4]
+#ifdef FT_TRACE
+  int dbg;                    // development builds: 1 = no GeLU, 2 = no quantizer arithmetic, 4 = no H2 MMAs, 8 = no stores
+#endif
 };
 
 // sigmoid(2 t) with t = sqrt(2/pi) (u + 0.044715 u^3): 0.5 (1 + tanh t) without the cancellation of 1 + tanh for
@@ -111,9 +117,9 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(&acc_full[a], 1);
-      mbar_init(&acc_empty[a], 16);   // 8 epilogue warps x 2 CTAs (used in the leader only)
+      mbar_init(&acc_empty[a], 24);   // 12 epilogue warps x 2 CTAs (used in the leader only)
     }
-    mbar_init(&z_full, 16);           // the z tile of both CTAs is staged (leader only)
+    mbar_init(&z_full, 24);           // the z tile of both CTAs is staged (leader only)
     mbar_init(&z_free, 1);            // the H2 MMAs have read it (commit, both CTAs)
     mbar_init(&d2_full, 1);           // D_f2 slice landed (leader only)
     mbar_init(&h2_full, 1);           // a segment's H2 accumulator is complete (commit, both CTAs)
@@ -199,6 +205,9 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
         mbar_wait(&d2_full, (uint32_t)j & 1);
         tc_fence_after();
         const bool first = j == 0 || seg_end(j - 1);
+#ifdef FT_TRACE
+        if (!(p.dbg & 4))
+#endif
 #pragma unroll
         for (int u = 0; u < 3; ++u)
 #pragma unroll
@@ -251,8 +260,9 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
     }
   } else if (warp >= 4) {
     // ===================================================== epilogue (both CTAs, own 128 rows)
-    // Two groups of four warps (a warp may read the TMEM lane quarter warp % 4); group g takes the 64-column units
-    // g, g + 2 of the 192-column accumulator.  Thread = one row of the tile.
+    // Three groups of four warps (a warp may read the TMEM lane quarter warp % 4); group g takes the 64-column unit g
+    // of the 192-column accumulator, in two halves of 32 columns.  Thread = one row of the tile.  (Two groups with
+    // two and one unit: 144 us at C3 -- a warp's 2 500 dependent instructions per tile set the pace, not the MMAs.)
     const int q = warp & 3;
     const int grp = (warp - 4) >> 2;
     const int et = (threadIdx.x - 128) & 127;  // 0..127 = row of this CTA's half tile
@@ -266,7 +276,7 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
       mbar_wait(&h2_full, (uint32_t)seg & 1);
       tc_fence_after();
       float* dst = p.slots + (pair_id + mt) * (int64_t)(ML_BM * p.r2) + (rank * 128 + q * 32 + lane) * 4;
-      for (int c0 = grp * 16; c0 < p.r2; c0 += 32) {
+      for (int c0 = grp * 16; c0 < p.r2; c0 += 48) {
         uint32_t v[16];
         tmem_ld16(tmem_base + ((uint32_t)(q * 32) << 16) + ML_H2_COL + c0, v);
         tmem_ld_wait();
@@ -287,62 +297,78 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
       tc_fence_after();
       if (i >= 1) mbar_wait(&z_free, (uint32_t)(i - 1) & 1);   // the H2 MMAs of the tile before have read the staged z
       const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + a * ML_BN;
-#pragma unroll 1
-      for (int u = grp; u < 3; u += 2) {
-        uint32_t v[64];
-        tmem_ld32(t0 + u * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
-        tmem_ld32(t0 + u * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
-        tmem_ld_wait();
-        if (u + 2 >= 3) {   // this warp's last unit is in registers: hand the accumulator back
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive_cluster(map_to_cta(smem_u32(&acc_empty[a]), 0));
-        }
+      {
+        const int u = grp;
         uint8_t* zrow = zs + u * 16384 + et * 128;
         uint32_t cz[8], cy[8], sfz = 0, sfy = 0;
-#pragma unroll
-        for (int b = 0; b < 4; ++b) {       // four 1x16 blocks of the unit
-          uint32_t yb[8], zb[8];
-#pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            yb[j] = pack_bf16x2(__uint_as_float(v[16 * b + 2 * j]) * alpha, __uint_as_float(v[16 * b + 2 * j + 1]) * alpha);
-            zb[j] = pack_bf16x2(gelu_tanh_f32(__uint_as_float(yb[j] << 16)), gelu_tanh_f32(__uint_as_float(yb[j] & 0xFFFF0000u)));
+#pragma unroll 1
+        for (int hh = 0; hh < 2; ++hh) {     // two halves of 32 columns: 32 accumulator words in registers at a time
+          uint32_t v[32];
+          tmem_ld32(t0 + u * 64 + hh * 32, v);
+          tmem_ld_wait();
+          if (hh == 1) {   // this warp's part of the accumulator is in registers: hand it back
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(map_to_cta(smem_u32(&acc_empty[a]), 0));
           }
-          const uint4 y0 = make_uint4(yb[0], yb[1], yb[2], yb[3]), y1 = make_uint4(yb[4], yb[5], yb[6], yb[7]);
-          const uint4 z0 = make_uint4(zb[0], zb[1], zb[2], zb[3]), z1 = make_uint4(zb[4], zb[5], zb[6], zb[7]);
-          // z goes to the staged tile (the A operand of the H2 MMAs): two 16-byte pieces of the swizzled row
-          *reinterpret_cast<uint4*>(zrow + (((2 * b) ^ (et & 7)) << 4)) = z0;
-          *reinterpret_cast<uint4*>(zrow + (((2 * b + 1) ^ (et & 7)) << 4)) = z1;
-          const float az = amax_block16(z0, z1), ay = amax_block16(y0, y1);
-          amax_z2 = __vmaxu2(amax_z2, __float_as_uint(az) >> 16);
-          amax_y2 = __vmaxu2(amax_y2, __float_as_uint(ay) >> 16);
-          const uint32_t sz = block_sf8(az, ts_z.g_enc), sy = block_sf8(ay, ts_y.g_enc);
-          float ez, ey;
-          asm volatile("ld.shared.f32 %0, [%1];" : "=f"(ez) : "r"(enc_z_u + sz * 4));
-          asm volatile("ld.shared.f32 %0, [%1];" : "=f"(ey) : "r"(enc_y_u + sy * 4));
-          cz[2 * b] = quant_bf16x8_fast(z0, ez);
-          cz[2 * b + 1] = quant_bf16x8_fast(z1, ez);
-          cy[2 * b] = quant_bf16x8_fast(y0, ey);
-          cy[2 * b + 1] = quant_bf16x8_fast(y1, ey);
-          sfz |= sz << (8 * b);
-          sfy |= sy << (8 * b);
-          if (p.z_dbg != nullptr && live) {   // test builds of the CALL only: bf16 copies for the staged comparison
-            const int64_t o = row * p.N + nt * ML_BN + u * 64 + b * 16;
-            *reinterpret_cast<uint4*>(p.z_dbg + o) = z0;
-            *reinterpret_cast<uint4*>(p.z_dbg + o + 8) = z1;
-            *reinterpret_cast<uint4*>(p.y1_dbg + o) = y0;
-            *reinterpret_cast<uint4*>(p.y1_dbg + o + 8) = y1;
+#pragma unroll
+          for (int bb = 0; bb < 2; ++bb) {       // two 1x16 blocks of the half
+            const int b = hh * 2 + bb;
+            uint32_t yb[8], zb[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              yb[j] = pack_bf16x2(__uint_as_float(v[16 * bb + 2 * j]) * alpha, __uint_as_float(v[16 * bb + 2 * j + 1]) * alpha);
+              zb[j] = pack_bf16x2(gelu_tanh_f32(__uint_as_float(yb[j] << 16)), gelu_tanh_f32(__uint_as_float(yb[j] & 0xFFFF0000u)));
+#ifdef FT_TRACE
+              if (p.dbg & 1) zb[j] = yb[j];
+#endif
+            }
+            const uint4 y0 = make_uint4(yb[0], yb[1], yb[2], yb[3]), y1 = make_uint4(yb[4], yb[5], yb[6], yb[7]);
+            const uint4 z0 = make_uint4(zb[0], zb[1], zb[2], zb[3]), z1 = make_uint4(zb[4], zb[5], zb[6], zb[7]);
+            // z goes to the staged tile (the A operand of the H2 MMAs): two 16-byte pieces of the swizzled row
+            *reinterpret_cast<uint4*>(zrow + (((2 * b) ^ (et & 7)) << 4)) = z0;
+            *reinterpret_cast<uint4*>(zrow + (((2 * b + 1) ^ (et & 7)) << 4)) = z1;
+            const float az = amax_block16(z0, z1), ay = amax_block16(y0, y1);
+            amax_z2 = __vmaxu2(amax_z2, __float_as_uint(az) >> 16);
+            amax_y2 = __vmaxu2(amax_y2, __float_as_uint(ay) >> 16);
+            const uint32_t sz = block_sf8(az, ts_z.g_enc), sy = block_sf8(ay, ts_y.g_enc);
+            float ez, ey;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(ez) : "r"(enc_z_u + sz * 4));
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(ey) : "r"(enc_y_u + sy * 4));
+#ifdef FT_TRACE
+            if (p.dbg & 2) {
+              cz[2 * bb] = z0.x; cz[2 * bb + 1] = z1.x; cy[2 * bb] = y0.x; cy[2 * bb + 1] = y1.x;
+            } else
+#endif
+            {
+            cz[2 * bb] = quant_bf16x8_fast(z0, ez);
+            cz[2 * bb + 1] = quant_bf16x8_fast(z1, ez);
+            cy[2 * bb] = quant_bf16x8_fast(y0, ey);
+            cy[2 * bb + 1] = quant_bf16x8_fast(y1, ey);
+            }
+            sfz |= sz << (8 * b);
+            sfy |= sy << (8 * b);
+            if (p.z_dbg != nullptr && live) {   // parity tests only: bf16 copies for the staged comparison
+              const int64_t o = row * p.N + nt * ML_BN + u * 64 + b * 16;
+              *reinterpret_cast<uint4*>(p.z_dbg + o) = z0;
+              *reinterpret_cast<uint4*>(p.z_dbg + o + 8) = z1;
+              *reinterpret_cast<uint4*>(p.y1_dbg + o) = y0;
+              *reinterpret_cast<uint4*>(p.y1_dbg + o + 8) = y1;
+            }
+          }
+          // codes: 16 contiguous bytes per row, half and tensor
+#ifdef FT_TRACE
+          if (!(p.dbg & 8))
+#endif
+          if (live) {
+            const int64_t co = row * half_cols + (nt * ML_BN + u * 64 + hh * 32) / 2;
+            *reinterpret_cast<uint4*>(p.codes_z + co) = make_uint4(cz[0], cz[1], cz[2], cz[3]);
+            *reinterpret_cast<uint4*>(p.codes_y1 + co) = make_uint4(cy[0], cy[1], cy[2], cy[3]);
           }
         }
-        // codes: 32 contiguous bytes per row, unit and tensor (a whole sector); scales: one word in the tile layout
+        // scales: one word per row, unit and tensor in the tile layout
         const int64_t so = ((row >> 7) * sf_tiles_n + nt * 3 + u) * 512 + (row & 31) * 16 + ((row & 127) >> 5) * 4;
         if (live) {
-          uint8_t* oz = p.codes_z + row * half_cols + (nt * ML_BN + u * 64) / 2;
-          uint8_t* oy = p.codes_y1 + row * half_cols + (nt * ML_BN + u * 64) / 2;
-          *reinterpret_cast<uint4*>(oz) = make_uint4(cz[0], cz[1], cz[2], cz[3]);
-          *reinterpret_cast<uint4*>(oz + 16) = make_uint4(cz[4], cz[5], cz[6], cz[7]);
-          *reinterpret_cast<uint4*>(oy) = make_uint4(cy[0], cy[1], cy[2], cy[3]);
-          *reinterpret_cast<uint4*>(oy + 16) = make_uint4(cy[4], cy[5], cy[6], cy[7]);
           *reinterpret_cast<uint32_t*>(p.sf_z + so) = sfz;
           *reinterpret_cast<uint32_t*>(p.sf_y1 + so) = sfy;
         } else if (row < ((p.M + 127) & ~(int64_t)127)) {   // padding rows of the last 128-row scale tile read as zero
@@ -526,6 +552,9 @@ int launch_gemm4_mlp(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_
   p.z_dbg = reinterpret_cast<__nv_bfloat16*>(z_dbg);
   p.y1_dbg = reinterpret_cast<__nv_bfloat16*>(y1_dbg);
   p.slots = slots;
+#ifdef FT_TRACE
+  p.dbg = getenv("FT_MLP_DBG") ? atoi(getenv("FT_MLP_DBG")) : 0;
+#endif
   FT_CUDA_TRY(cudaFuncSetAttribute(k_gemm4_mlp, cudaFuncAttributeMaxDynamicSharedMemorySize, ML_SMEM));
   const int64_t tiles_m = ceil_div(M, ML_BM), tiles_n = N1 / ML_BN, T = tiles_m * tiles_n;
   const int64_t max_pairs = sm_count() / 2;
