@@ -72,6 +72,12 @@ __device__ __forceinline__ float gelu_sigmoid_f32(float u) {
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(1.0f + e));
   return s;
 }
+// one 32-byte store (sm_100: 256-bit global accesses); p is 32-byte aligned
+__device__ __forceinline__ void st_global_v8(void* p, uint4 a, uint4 b) {
+  asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w),
+               "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w)
+               : "memory");
+}
 // GeLU, tanh form: 0.5 u (1 + tanh t) = u sigmoid(2 t)
 __device__ __forceinline__ float gelu_tanh_f32(float u) { return u * gelu_sigmoid_f32(u); }
 
@@ -149,18 +155,24 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
     if (elect_one()) {
       int stage = 0;
       uint32_t phase = 0;
+      // The D_f2 slice of tile j goes into the single slice buffer once the H2 MMAs of tile j - 1 have read it (z_free).
+      // Those are issued after the K loop of tile j, so the load is placed ML_STAGES ring stages into tile j + 1: by
+      // then the issuer has consumed a stage of tile j + 1 and z_free(j - 1) has fired -- the wait never stalls the ring
+      // (at the head of the tile the producer sat on z_free while the ring ran empty, once per tile).
+      auto load_d2 = [&](int j) {
+        if (j >= 1) mbar_wait(&z_free, (uint32_t)(j - 1) & 1);
+        const int64_t nt = (t_begin + j) % tiles_n;
+        const uint32_t bar = map_to_cta(smem_u32(&d2_full), 0);
+        if (leader) mbar_expect_tx(&d2_full, 2 * ML_D2_BYTES);
+        for (int u = 0; u < 3; ++u)
+          tma_load_2d_pair(d2s + u * 8192, &map_d2, bar, (int32_t)(rank * (p.r2 / 2)), (int32_t)(nt * ML_BN + u * 64));
+      };
+      const int kt_d2 = min(ML_STAGES, kiters - 1);
       for (int i = 0; i <= n_local; ++i) {
-        if (i >= 1) {
-          // the D_f2 slice of tile j = i - 1: its buffer is free once the H2 MMAs of tile j - 1 have read it
-          const int j = i - 1;
-          if (j >= 1) mbar_wait(&z_free, (uint32_t)(j - 1) & 1);
-          const int64_t nt = (t_begin + j) % tiles_n;
-          const uint32_t bar = map_to_cta(smem_u32(&d2_full), 0);
-          if (leader) mbar_expect_tx(&d2_full, 2 * ML_D2_BYTES);
-          for (int u = 0; u < 3; ++u)
-            tma_load_2d_pair(d2s + u * 8192, &map_d2, bar, (int32_t)(rank * (p.r2 / 2)), (int32_t)(nt * ML_BN + u * 64));
+        if (i == n_local) {
+          load_d2(i - 1);
+          break;
         }
-        if (i == n_local) break;
         const int64_t tile = t_begin + i;
         const int64_t mt = tile / tiles_n, nt = tile % tiles_n;
         const int32_t m0 = (int32_t)(mt * ML_BM + rank * 128);
@@ -189,6 +201,7 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
             stage = 0;
             phase ^= 1;
           }
+          if (kt == kt_d2 && i >= 1) load_d2(i - 1);
         }
       }
     }
@@ -295,17 +308,19 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
       const bool live = row < p.M;
       mbar_wait(&acc_full[a], ((uint32_t)i >> 1) & 1);
       tc_fence_after();
-      if (i >= 1) mbar_wait(&z_free, (uint32_t)(i - 1) & 1);   // the H2 MMAs of the tile before have read the staged z
       const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + a * ML_BN;
       {
         const int u = grp;
         uint8_t* zrow = zs + u * 16384 + et * 128;
-        uint32_t cz[8], cy[8], sfz = 0, sfy = 0;
+        uint32_t cz[4], cy[4], sfz = 0, sfy = 0;
+        uint4 cz_lo = make_uint4(0, 0, 0, 0), cy_lo = cz_lo;
 #pragma unroll 1
         for (int hh = 0; hh < 2; ++hh) {     // two halves of 32 columns: 32 accumulator words in registers at a time
           uint32_t v[32];
           tmem_ld32(t0 + u * 64 + hh * 32, v);
           tmem_ld_wait();
+          // the H2 MMAs of the tile before must have read the staged z before it is overwritten
+          if (hh == 0 && i >= 1) mbar_wait(&z_free, (uint32_t)(i - 1) & 1);
           if (hh == 1) {   // this warp's part of the accumulator is in registers: hand it back
             tc_fence_before();
             __syncwarp();
@@ -356,14 +371,19 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
               *reinterpret_cast<uint4*>(p.y1_dbg + o + 8) = y1;
             }
           }
-          // codes: 16 contiguous bytes per row, half and tensor
+          // codes: the unit's 32 bytes per row and tensor leave as ONE 256-bit store -- a full sector per lane (two
+          // 16-byte stores per sector cost twice the L1 transactions: 23 us of the kernel at C3)
+          if (hh == 0) {
+            cz_lo = make_uint4(cz[0], cz[1], cz[2], cz[3]);
+            cy_lo = make_uint4(cy[0], cy[1], cy[2], cy[3]);
+          } else
 #ifdef FT_TRACE
           if (!(p.dbg & 8))
 #endif
           if (live) {
-            const int64_t co = row * half_cols + (nt * ML_BN + u * 64 + hh * 32) / 2;
-            *reinterpret_cast<uint4*>(p.codes_z + co) = make_uint4(cz[0], cz[1], cz[2], cz[3]);
-            *reinterpret_cast<uint4*>(p.codes_y1 + co) = make_uint4(cy[0], cy[1], cy[2], cy[3]);
+            const int64_t co = row * half_cols + (nt * ML_BN + u * 64) / 2;
+            st_global_v8(p.codes_z + co, cz_lo, make_uint4(cz[0], cz[1], cz[2], cz[3]));
+            st_global_v8(p.codes_y1 + co, cy_lo, make_uint4(cy[0], cy[1], cy[2], cy[3]));
           }
         }
         // scales: one word per row, unit and tensor in the tile layout
