@@ -400,6 +400,22 @@ def run_ours(args):
     kern["step_saved4_us"] = graph_us([step_saved4], 100)
     kern["step_bf16x_us"] = graph_us([step_bf16x], 100)
 
+    # single-copy weights (NEXT-5): the codes of Q(R)^T are rebuilt into a scratch buffer before every backward
+    codes_nmajor = layer.r_nmajor.codes
+    scratch_t = torch.empty_like(codes_nmajor)
+
+    def step_single_copy():
+        B.ft_linear_fwd(layer, X, y, h, qx, ws)
+        B.ft_weight_transpose_codes(layer, scratch_t)
+        B.ft_linear_bwd(layer, X, G, h, dx, p, dA, dBt, qg, ws)
+    layer.r_nmajor.codes = scratch_t
+    kern["step_single_copy_us"] = graph_us([step_single_copy], 100)
+    layer.r_nmajor.codes = codes_nmajor
+    # the transposition alone, over enough distinct destinations that none of it stays in L2
+    scr = copies(scratch_t)
+    kern["transpose_codes_us"] = graph_us([lambda d=d: B.ft_weight_transpose_codes(layer, d) for d in scr])
+    del scr
+
     # the step WITHOUT a graph: 8 launches enqueued by the host each step (tensor maps come from the library's memo)
     def eager_us(fn, n=50):
         for _ in range(5):
@@ -510,6 +526,18 @@ def run_ours(args):
                         "forward pass wrote, so the bf16 X need not be kept for backward (3.56x fewer saved bytes); "
                         "step_us = ft_linear_fwd + ft_linear_bwd_q4 as a CUDA graph, 100 replays; the headline step follows "
                         "Eq. 4 literally (O-12)"},
+            "single_copy_weights": {
+                "step_us": round(kern["step_single_copy_us"], 2), "step_two_copies_us": round(kern["step_bf16x_us"], 2),
+                "transpose_us": round(kern["transpose_codes_us"], 2),
+                "transpose_GBps": round(N * K / (kern["transpose_codes_us"] * 1e-6) / 1e9, 1),
+                "weight_bytes_per_layer_two_copies": int(N * K * (0.5 + 0.5 + 2 / 16)),
+                "weight_bytes_per_layer_single_copy": int(N * K * (0.5 + 2 / 16)),
+                "scratch_bytes_shared_by_all_layers": N * K // 2,
+                "note": "NEXT-5 (PAPER.md:102, :197): one copy of the 4-bit codes per layer; ft_weight_transpose_codes "
+                        "rebuilds the codes of Q(R)^T into one scratch buffer before the layer's backward (N K bytes "
+                        "of traffic: N K / 2 read + N K / 2 written); both scale layouts (N K / 16 each) stay per "
+                        "layer.  The 4-bit MMA takes K-major operands only, so the element transposition cannot be "
+                        "left to the tensor core or to TMA"},
             **extra,
             "paper_context": "2.27x step time / 2.25x memory vs BF16 LoRA on RTX 5090 (PAPER.md:7,207); not the target",
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cpu_cores(), "kind": "oracle",

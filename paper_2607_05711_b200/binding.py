@@ -53,6 +53,7 @@ def lib():
         L.ft_quantize_blockwise.argtypes = [vp, i64, i64, vp, C.POINTER(_Proj), C.POINTER(_QT), i32, C.c_uint64, C.c_uint64,
                                             vp, sz, vp]
         L.ft_pack_weight.argtypes = [C.POINTER(_QT), C.POINTER(_QT), C.POINTER(_QT), vp]
+        L.ft_weight_transpose_codes.argtypes = [C.POINTER(_QT), vp, vp]
         L.ft_linear_fwd.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
         L.ft_linear_bwd_dgrad.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
         L.ft_gemm4.argtypes = [C.POINTER(_QT), C.POINTER(_QT), vp, vp, i32, vp, vp]
@@ -214,6 +215,13 @@ class Layer:
         return _Layer(self.r_kmajor.c(), self.r_nmajor.c(),
                       None if self.D_f is None else self.D_f.data_ptr(),
                       None if self.U_t is None else self.U_t.data_ptr(), self.K, self.N, self.r_s, self.r)
+
+
+def ft_weight_transpose_codes(layer, codes_t, stream=None):
+    """Single-copy weights (NEXT-5): rebuild the codes of Q(R)^T from layer.r_kmajor into codes_t (uint8, K*N/2)."""
+    q = layer.r_kmajor.c()
+    _check(lib().ft_weight_transpose_codes(C.byref(q), _ptr(codes_t), _stream(stream)))
+    return codes_t
 
 
 def ft_linear_fwd(layer, x, y, h_saved, qx, workspace, stream=None):

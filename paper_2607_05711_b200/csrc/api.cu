@@ -22,6 +22,7 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
                           const ft_proj* proj, ft_qtensor* out, void* workspace, bool after_kernel,
                           bool* finalize_last, cudaStream_t st);
 int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, cudaStream_t st);
+int launch_transpose_codes(const uint8_t* src, uint8_t* dst, int64_t N, int64_t K, cudaStream_t st);
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
                  const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, bool lr_late,
                  cudaStream_t st);
@@ -371,6 +372,14 @@ int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, v
     rk_tiled->sf_layout = FT_SF_TILE128x4;
   }
   return launch_pack_weight(rk, rk_tiled, rn, (cudaStream_t)stream);
+}
+
+int ft_weight_transpose_codes(const ft_qtensor* rk, uint8_t* codes_t, void* stream) {
+  if (!rk || !rk->codes || !codes_t || !aligned16(rk->codes) || !aligned16(codes_t)) return FT_ERR_INVALID_ARG;
+  if (rk->rows % 64 != 0 || rk->cols % 64 != 0 || rk->rows < 64 || rk->cols < 64) return FT_ERR_UNSUPPORTED_SHAPE;
+  int rc = device_check();
+  if (rc != FT_OK) return rc;
+  return launch_transpose_codes(rk->codes, codes_t, rk->rows, rk->cols, (cudaStream_t)stream);
 }
 
 int ft_gemm4(const ft_qtensor* a, const ft_qtensor* b, const void* lr_a_scaled, const void* lr_b,

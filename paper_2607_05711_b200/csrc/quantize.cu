@@ -262,23 +262,78 @@ int launch_quantize_generic(const void* x, int64_t rows, int64_t cols, const flo
 }
 
 // --------------------------------------------------------- a6: weight re-packing
-// codes_t[k][n] = codes[n][k] for 4-bit codes: 64x64 code tile through shared memory.
+// Q(R) [N x K/2 bytes] -> Q(R)^T [K x N/2 bytes]: a transposition of 4-bit elements (the same codes
+// serve forward and backward; nothing is re-quantized).  Used offline by ft_pack_weight and, with single-copy weights
+// (SURVEY NEXT-5), once per backward by ft_weight_transpose_codes, so it is written for the HBM roofline: a CTA
+// moves a tile of 256 x 256 elements (32 KB); both its reads and its writes are whole 128-byte row pieces.
+//   warp w, lane t: the 32 rows n = 32 w .. 32 w + 31, the word t of each (elements k = 8 t .. 8 t + 7): four 8x8
+//   element blocks, each transposed in registers by three butterfly stages (PRMT for the 16- and 8-bit stages,
+//   LOP3 for the 4-bit one); the lane then owns, for each of its 8 output rows k, 16 contiguous bytes (32 elements
+//   n) -> one 16-byte store into the staged output tile, chunk index XOR (t & 7) against bank conflicts;
+//   then every output row leaves as eight 16-byte pieces written by eight neighbouring lanes.
+__device__ __forceinline__ void nibble_transpose8x8(uint32_t (&a)[8]) {
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {   // swap the off-diagonal 4x4 blocks
+    const uint32_t x = a[i], y = a[i + 4];
+    a[i] = __byte_perm(x, y, 0x5410);
+    a[i + 4] = __byte_perm(x, y, 0x7632);
+  }
+#pragma unroll
+  for (int b = 0; b < 8; b += 4)
+#pragma unroll
+    for (int i = b; i < b + 2; ++i) {   // 2x2 blocks inside each 4x4
+      const uint32_t x = a[i], y = a[i + 2];
+      a[i] = __byte_perm(x, y, 0x6240);
+      a[i + 2] = __byte_perm(x, y, 0x7351);
+    }
+#pragma unroll
+  for (int i = 0; i < 8; i += 2) {     // single elements inside each 2x2
+    const uint32_t x = a[i], y = a[i + 1];
+    a[i] = (x & 0x0F0F0F0Fu) | ((y & 0x0F0F0F0Fu) << 4);
+    a[i + 1] = ((x >> 4) & 0x0F0F0F0Fu) | (y & 0xF0F0F0F0u);
+  }
+}
+
 __global__ void __launch_bounds__(256) k_transpose_codes(const uint8_t* __restrict__ src,
                                                          uint8_t* __restrict__ dst, int64_t N,
                                                          int64_t K) {
-  __shared__ uint8_t tile[64][65];  // unpacked codes, [n][k]
-  const int64_t n0 = (int64_t)blockIdx.y * 64, k0 = (int64_t)blockIdx.x * 64;
-  for (int i = threadIdx.x; i < 64 * 32; i += 256) {
-    const int n = i / 32, kb = i % 32;
-    const uint8_t b = src[(n0 + n) * (K / 2) + k0 / 2 + kb];
-    tile[n][2 * kb] = b & 0xF;
-    tile[n][2 * kb + 1] = b >> 4;
+  __shared__ __align__(16) uint8_t tile[256 * 128];   // [k][n / 2], 16-byte chunks swizzled by (k >> 3) & 7
+  const int64_t n0 = (int64_t)blockIdx.y * 256, k0 = (int64_t)blockIdx.x * 256;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const bool k_ok = k0 + lane * 8 < K;
+  uint32_t out[8][4];
+#pragma unroll
+  for (int g = 0; g < 4; ++g) {        // 8x8 block g: rows n = 32 warp + 8 g + i
+    uint32_t a[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int64_t n = n0 + warp * 32 + g * 8 + i;
+      a[i] = (k_ok && n < N) ? __ldg(reinterpret_cast<const uint32_t*>(src + n * (K / 2) + k0 / 2) + lane) : 0u;
+    }
+    nibble_transpose8x8(a);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) out[j][g] = a[j];
   }
+#pragma unroll
+  for (int j = 0; j < 8; ++j)          // row k = 8 lane + j, chunk = warp (32 elements n each)
+    *reinterpret_cast<uint4*>(tile + (lane * 8 + j) * 128 + ((warp ^ (lane & 7)) << 4)) =
+        make_uint4(out[j][0], out[j][1], out[j][2], out[j][3]);
   __syncthreads();
-  for (int i = threadIdx.x; i < 64 * 32; i += 256) {
-    const int k = i / 32, nb = i % 32;
-    dst[(k0 + k) * (N / 2) + n0 / 2 + nb] = tile[2 * nb][k] | (tile[2 * nb + 1][k] << 4);
+  const int c = threadIdx.x & 7;
+#pragma unroll
+  for (int it = 0; it < 8; ++it) {
+    const int k = it * 32 + (threadIdx.x >> 3);
+    if (k0 + k < K && n0 + c * 32 < N)
+      *reinterpret_cast<uint4*>(dst + (k0 + k) * (N / 2) + n0 / 2 + c * 16) =
+          *reinterpret_cast<const uint4*>(tile + k * 128 + ((c ^ ((k >> 3) & 7)) << 4));
   }
+}
+
+int launch_transpose_codes(const uint8_t* src, uint8_t* dst, int64_t N, int64_t K, cudaStream_t st) {
+  dim3 grid((unsigned)ceil_div(K, 256), (unsigned)ceil_div(N, 256));
+  k_transpose_codes<<<grid, 256, 0, st>>>(src, dst, N, K);
+  FT_CUDA_TRY(cudaGetLastError());
+  return FT_OK;
 }
 
 // Expand S[N/16][K/16] to per-row TILE128x4 scales for both orientations:
@@ -327,9 +382,8 @@ __global__ void __launch_bounds__(256) k_expand_sf_ntile(const uint8_t* __restri
 int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn,
                        cudaStream_t st) {
   const int64_t N = rk->rows, K = rk->cols;
-  dim3 grid((unsigned)(K / 64), (unsigned)(N / 64));
-  k_transpose_codes<<<grid, 256, 0, st>>>(rk->codes, rn->codes, N, K);
-  FT_CUDA_TRY(cudaGetLastError());
+  const int rc_t = launch_transpose_codes(rk->codes, rn->codes, N, K, st);
+  if (rc_t != FT_OK) return rc_t;
   FT_CUDA_TRY(cudaMemsetAsync(rn->sf, 0, ft_sf_bytes(K, N, 16, FT_SF_TILE128x4), st));
   if (rk_tiled != nullptr)
     FT_CUDA_TRY(cudaMemsetAsync(rk_tiled->sf, 0, ft_sf_bytes(N, K, 16, FT_SF_TILE128x4), st));

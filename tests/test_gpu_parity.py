@@ -208,7 +208,7 @@ def test_quantize_degenerate_inputs(B):
     assert_q_equal(out, nvfp4.quantize_blockwise(x, 1, amax_t=np.float32(2688.0)), 0, B)
 
 
-@pytest.mark.parametrize("N,K", [(64, 64), (256, 512), (3072, 3072)])
+@pytest.mark.parametrize("N,K", [(64, 64), (256, 512), (320, 448), (832, 192), (3072, 3072)])
 def test_weight_quantize_16x16_and_pack(B, N, K):
     rng = synth.make_rng(N + K)
     W = synth.normal(rng, (N, K), 0.02)
@@ -570,6 +570,34 @@ def test_wgrad_saved4_errors(B):
     dA = torch.zeros(K, r, dtype=torch.float32, device="cuda"); dBt = torch.zeros(N, r, dtype=torch.float32, device="cuda")
     with pytest.raises(B.FtError):      # Q(G) has the wrong column count for the X operand
         B.ft_lora_wgrad_q4(L, o["qg"] if N != K else B.QTensor(M, K + 64), o["gt"], o["ht"], o["pt"], dA, dBt)
+
+
+@pytest.mark.parametrize("M,K,N", [(200, 448, 320), (512, 3072, 1024)])
+def test_single_copy_weights(B, M, K, N):
+    """NEXT-5: one copy of the 4-bit codes per layer.  ft_weight_transpose_codes rebuilds the
+    codes of Q(R)^T into a scratch buffer: the bytes ft_pack_weight wrote (themselves compared with the oracle's
+    transposed object in test_weight_quantize_16x16_and_pack), and the dgrad through the scratch is bit-identical."""
+    r_s, r = 16, 16
+    rng = synth.make_rng(M + K + N)
+    W = synth.normal(rng, (N, K), 0.02)
+    D = synth.normal(rng, (K, r_s + r), 0.01)
+    U = synth.normal(rng, (N, r_s + r), 0.01)
+    G = synth.student_t_grad(rng, M, N)
+    L = B.Layer(t16(W), t16(D), t16(U), r_s, r)
+    q = nvfp4.quantize_blockwise(W, 16)
+    want = nvfp4.pack_codes(np.ascontiguousarray(q["codes"].T))
+    scratch = torch.full_like(L.r_nmajor.codes, 0xAB)
+    B.ft_weight_transpose_codes(L, scratch)
+    assert np.array_equal(scratch.cpu().numpy().reshape(K, N // 2), want)
+    ws = B.new_workspace(M, max(K, N), max(K, N), r_s + r, "cuda")
+    outs = []
+    for codes in (L.r_nmajor.codes, scratch):
+        L.r_nmajor.codes = codes
+        dx = torch.zeros(M, K, dtype=torch.bfloat16, device="cuda")
+        p = torch.zeros(M, r_s + r, dtype=torch.bfloat16, device="cuda")
+        B.ft_linear_bwd_dgrad(L, t16(G), dx, p, B.QTensor(M, N), ws)
+        outs.append(dx.view(torch.int16).cpu().numpy())
+    assert np.array_equal(outs[0], outs[1])
 
 
 def test_forward_with_1x16_weight_blocks(B):
