@@ -20,7 +20,10 @@ int launch_quantize_sr(const void* x, int64_t rows, int64_t cols, const float* a
                        uint64_t seed, uint64_t offset, cudaStream_t st);
 int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t,
                           const ft_proj* proj, ft_qtensor* out, void* workspace, bool after_kernel,
-                          bool* finalize_last, cudaStream_t st);
+                          bool* finalize_last, const SumJob* side_job, cudaStream_t st);
+int launch_wgrad_stream(const void* in, const void* l, int64_t M, int64_t F, int r_t, int r_s, int r, float* out,
+                        float* slots, size_t slot_capacity_floats, int* n_slots, unsigned int* amax_in,
+                        float* zero_fill, int64_t zero_fill_n, bool after_kernel, bool beside_prev, cudaStream_t st);
 int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, cudaStream_t st);
 int launch_transpose_codes(const uint8_t* src, uint8_t* dst, int64_t N, int64_t K, cudaStream_t st);
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
@@ -186,7 +189,7 @@ static bool valid_rt(int r_t) { return r_t >= 0 && r_t <= 128 && r_t % 16 == 0; 
 static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_up, int r_t,
                        const void* act, int64_t M, int64_t Kd, int64_t Nd, void* out,
                        void* saved, ft_qtensor* q, void* workspace, size_t ws_bytes,
-                       const float* act_amax, bool after_kernel, cudaStream_t st) {
+                       const float* act_amax, bool after_kernel, const SumJob* side_job, cudaStream_t st) {
   if (!act || !out || !q || !q->codes || !q->sf || !q->tensor_dec_scale || !workspace)
     return FT_ERR_INVALID_ARG;
   if (r_t > 0 && (!saved || !lr_down || !lr_up)) return FT_ERR_INVALID_ARG;
@@ -214,7 +217,7 @@ static int linear_pass(const ft_qtensor* w, const void* lr_down, const void* lr_
   // shared memory (single pass), by a preceding k_amax launch otherwise
   bool finalize_last = false;   // k_finalize_h (which writes only H and Hs) is the last launch of the quantize step
   rc = launch_quantize_fused(act, M, Kd, act_amax, r_t > 0 ? &pr : nullptr, q, workspace, after_kernel,
-                             &finalize_last, st);
+                             &finalize_last, side_job, st);
   if (rc != FT_OK) return rc;
   // lr_late invariant (gemm_pair.cu): the GEMM launch directly follows k_finalize_h of THIS call -- nothing may be
   // enqueued between the two lines above and below
@@ -344,7 +347,7 @@ int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols, const 
     if (round_mode == FT_ROUND_STOCHASTIC) return launch_quantize_sr(x_bf16, rows, cols, amax, out, seed, offset, st);
     return launch_quantize_generic(x_bf16, rows, cols, amax, out, st);
   }
-  return launch_quantize_fused(x_bf16, rows, cols, tensor_amax, proj, out, workspace, pdl_enabled(), nullptr, st);
+  return launch_quantize_fused(x_bf16, rows, cols, tensor_amax, proj, out, workspace, pdl_enabled(), nullptr, nullptr, st);
 }
 
 int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, void* stream) {
@@ -463,7 +466,7 @@ int ft_mlp_fwd(const ft_layer* fc1, const ft_layer* fc2, const void* x_bf16, int
   pr.out_scaled = hs1;
   pr.other_dec_scale = fc1->r_kmajor.tensor_dec_scale;
   pr.r_t = r1;
-  rc = launch_quantize_fused(x_bf16, M, K, nullptr, &pr, qx, workspace, false, nullptr, st);
+  rc = launch_quantize_fused(x_bf16, M, K, nullptr, &pr, qx, workspace, false, nullptr, nullptr, st);
   if (rc != FT_OK) return rc;
   // FC1 GEMM with the fused epilogue (GeLU, Q(Z), Q(Y1), H2 partials) and the sums of the H2 partials
   rc = launch_gemm4_mlp(qx, &fc1->r_kmajor, M, N1, K, hs1, fc1->U_t, r1, fc2->D_f, r2, fc2->r_kmajor.tensor_dec_scale,
@@ -492,7 +495,7 @@ int ft_linear_fwd(const ft_layer* L, const void* x_bf16, int64_t M, void* y_bf16
   int rc = check_layer(L);
   if (rc != FT_OK) return rc;
   return linear_pass(&L->r_kmajor, L->D_f, L->U_t, L->r_s + L->r, x_bf16, M, L->K, L->N, y_bf16,
-                     h_saved_bf16, qx_scratch, workspace, workspace_bytes, nullptr, pdl_enabled(), (cudaStream_t)stream);
+                     h_saved_bf16, qx_scratch, workspace, workspace_bytes, nullptr, pdl_enabled(), nullptr, (cudaStream_t)stream);
 }
 
 int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* dx_bf16,
@@ -501,7 +504,7 @@ int ft_linear_bwd_dgrad(const ft_layer* L, const void* g_bf16, int64_t M, void* 
   int rc = check_layer(L);
   if (rc != FT_OK) return rc;
   return linear_pass(&L->r_nmajor, L->U_t, L->D_f, L->r_s + L->r, g_bf16, M, L->N, L->K, dx_bf16,
-                     p_saved_bf16, qg_scratch, workspace, workspace_bytes, nullptr, pdl_enabled(), (cudaStream_t)stream);
+                     p_saved_bf16, qg_scratch, workspace, workspace_bytes, nullptr, pdl_enabled(), nullptr, (cudaStream_t)stream);
 }
 
 static int check_wgrad(const ft_layer* L, const void* x_bf16, const void* g_bf16, int64_t M, const void* h_saved_bf16,
@@ -574,18 +577,18 @@ static int linear_bwd(const ft_layer* L, const void* x_bf16, const ft_qtensor* q
   const int r_t = L->r_s + L->r;
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
   bool chained = pdl_enabled();   // the first kernel of the call may carry a programmatic edge (it waits at its top)
-  // dA from the saved codes goes through fp32 reductions (k_wgrad_q4 has no slot path): clear it up front
-  if (qx != nullptr && !accumulate) {
-    rc = launch_clear2(dA, (size_t)L->K * L->r * sizeof(float), nullptr, 0, st);
-    if (rc != FT_OK) return rc;
-    chained = true;
-  }
   // G small enough for the single-pass quantizer (<= ~29 MB: it finds the amax itself and reads G once):
   // quantize, GEMM, one wgrad launch for both gradients -- G is read twice either way, with one
   // launch fewer than the schedule below
   if (quantize_single_pass_fits(M, L->N, r_t)) {
+    // dA from the saved codes goes through fp32 reductions (k_wgrad_q4 has no slot path): clear it up front
+    if (qx != nullptr && !accumulate) {
+      rc = launch_clear2(dA, (size_t)L->K * L->r * sizeof(float), nullptr, 0, st);
+      if (rc != FT_OK) return rc;
+      chained = true;
+    }
     rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
-                     workspace, workspace_bytes, nullptr, chained, st);
+                     workspace, workspace_bytes, nullptr, chained, nullptr, st);
     if (rc != FT_OK) return rc;
     if (qx == nullptr)
       return launch_wgrad(3, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
@@ -597,22 +600,28 @@ static int linear_bwd(const ft_layer* L, const void* x_bf16, const ft_qtensor* q
                            false, st);
   }
   // 1. dB^T = G^T (X A): the one pass over G that Eq. 4 needs anyway also yields max |G| (a0), into a control
-  //    word of the workspace (zero by the workspace invariant; the quantize kernel puts it back).  The M slices
-  //    combine over distributed shared memory inside the kernel (a cluster per feature tile): no clear kernel, no memset node.
+  //    word of the workspace (zero by the workspace invariant; the quantize kernel puts it back), and clears dA for
+  //    the reductions of the last launch.  Its M slices store to slots of the workspace; k_finalize_h of step 2
+  //    adds them in slice order (wgrad_stream.cu).  With accumulate they add to dBt directly (nothing to clear).
+  const WsLayout wl = ws_layout(M, r_t);
   unsigned int* amax_g = reinterpret_cast<unsigned int*>(ws + WS_CTL_AMAX_EXT);
-  rc = launch_wgrad(2, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                    accumulate, amax_g, chained, false, st);
+  float* wg_slots = accumulate ? nullptr : reinterpret_cast<float*>(ws + wl.wg_off);
+  int n_slots = 0;
+  rc = launch_wgrad_stream(g_bf16, h_saved_bf16, M, L->N, r_t, L->r_s, L->r, dBt, wg_slots, wl.wg_floats, &n_slots, amax_g,
+                           accumulate ? nullptr : dA, (int64_t)L->K * L->r, chained, false, st);
   if (rc != FT_OK) return rc;
   // 2. a3 + a4 with that amax: Q(G), P = G U_t, dX
+  const SumJob job = {reinterpret_cast<const float4*>(wg_slots), reinterpret_cast<float4*>(dBt), L->N * (int64_t)L->r / 4,
+                      n_slots};
   rc = linear_pass(&L->r_nmajor, L->U_t, L->D_f, r_t, g_bf16, M, L->N, L->K, dx_bf16, p_saved_bf16, qg_scratch,
-                   workspace, workspace_bytes, reinterpret_cast<const float*>(amax_g), true, st);
+                   workspace, workspace_bytes, reinterpret_cast<const float*>(amax_g), true, &job, st);
   if (rc != FT_OK) return rc;
   // 3. dA = X^T (G B^T) needs P.  Nothing it touches depends on the GEMM in front of it (X, P in; dA and its
-  //    out), and every CTA of the GEMM passes its own wait -- P complete -- before triggering: dA
+  //    out), and every CTA of the GEMM passes its own wait -- P complete, dA cleared -- before triggering: dA
   //    starts in the GEMM's tail and waits for the GEMM only before it exits.
   if (qx == nullptr)
-    return launch_wgrad(1, x_bf16, g_bf16, M, L->K, L->N, p_saved_bf16, h_saved_bf16, r_t, L->r_s, L->r, dA, dBt,
-                        accumulate, nullptr, true, true, st);
+    return launch_wgrad_stream(x_bf16, p_saved_bf16, M, L->K, r_t, L->r_s, L->r, dA, nullptr, 0, nullptr, nullptr, nullptr,
+                               0, true, true, st);
   return launch_wgrad_q4(qx->codes, qx->sf, qx->tensor_dec_scale, M, L->K, p_saved_bf16, r_t, L->r_s, L->r, dA, 1,
                          true, st);
 }

@@ -54,8 +54,17 @@ bool pdl_enabled();  // programmatic dependent launch of the GEMM and dA kernels
 constexpr int WS_MAX_QUANT_CTAS = 192;   // one CTA per SM
 constexpr size_t WS_CTL_BYTES = 4096;
 constexpr size_t WS_CTL_AMAX = 0, WS_CTL_BAR = 4, WS_CTL_EXIT = 8, WS_CTL_AMAX_EXT = 16;
+constexpr int WS_WG_TILES = 2 * WS_MAX_QUANT_CTAS;   // dB^T slots: slices x feature tiles of 128 <= 2 CTAs per SM
 struct WsLayout {
-  size_t hs_off, slots_off, total;
+  size_t hs_off, slots_off, wg_off, wg_floats, total;
+};
+// A sum the finalize kernel of the quantize pass runs on the side (wgrad_stream.cu: the M slices of dB^T):
+// out[i] = slots[0][i] + slots[1][i] + ... in slot order, i < n4 float4s.  n_slots == 0: nothing to do.
+struct SumJob {
+  const float4* slots;
+  float4* out;
+  int64_t n4;
+  int n_slots;
 };
 inline WsLayout ws_layout(int64_t M, int r_t) {
   auto up = [](size_t v) { return (v + 255) / 256 * 256; };
@@ -63,7 +72,9 @@ inline WsLayout ws_layout(int64_t M, int r_t) {
   const size_t tiles = (size_t)((M + 127) / 128);
   w.hs_off = WS_CTL_BYTES;
   w.slots_off = w.hs_off + up((size_t)M * (size_t)r_t * 2);
-  w.total = w.slots_off + (WS_MAX_QUANT_CTAS + tiles) * 128 * (size_t)r_t * 4 + 256;
+  w.wg_off = w.slots_off + up((WS_MAX_QUANT_CTAS + tiles) * 128 * (size_t)r_t * 4);
+  w.wg_floats = (size_t)WS_WG_TILES * 128 * (size_t)r_t;
+  w.total = w.wg_off + w.wg_floats * 4 + 256;
   return w;
 }
 

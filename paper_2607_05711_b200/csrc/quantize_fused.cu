@@ -474,11 +474,26 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
 // threads read neighbouring rows of a slot (layout [quad][row][4]).  G = grid size of the quantize launch that filled
 // the slots; P = blockDim.y (1 when a row tile has at most 8 contributors, as on the large shapes).
 template <int R_T>
-__global__ void __launch_bounds__(1024) k_finalize_h(const QFParams p, int G) {
+__global__ void __launch_bounds__(1024) k_finalize_h(const QFParams p, int G, const SumJob job) {
   constexpr int SLOT_F4 = QF_ROWS * R_T / 4;
   __shared__ float4 s_part[8][QF_ROWS];
   pdl_wait();      // the slots and g_dec come from the quantize kernel before us
   pdl_trigger();
+  if (job.n_slots > 0) {   // side job (ft_linear_bwd: the M slices of dB^T, written two kernels ago): slot order
+    const int64_t nthr = (int64_t)gridDim.x * gridDim.y * blockDim.x * blockDim.y;
+    const int64_t me = (((int64_t)blockIdx.y * gridDim.x + blockIdx.x) * blockDim.y + threadIdx.y) * blockDim.x + threadIdx.x;
+    for (int64_t i = me; i < job.n4; i += nthr) {
+      float4 a = __ldcg(job.slots + i);
+      for (int sidx = 1; sidx < job.n_slots; ++sidx) {
+        const float4 o = __ldcg(job.slots + (int64_t)sidx * job.n4 + i);
+        a.x += o.x;
+        a.y += o.y;
+        a.z += o.z;
+        a.w += o.w;
+      }
+      job.out[i] = a;
+    }
+  }
   float inv_alpha = 1.0f;   // Hs = bf16(H * (1 / alpha)), alpha = g_dec(this) * g_dec(other)
   if (p.hs_out != nullptr) inv_alpha = __fdiv_rn(1.0f, __fmul_rn(__ldcg(p.g_dec_out), __ldg(p.other_dec_scale)));
   const int C = p.chunks_per_tile;
@@ -553,7 +568,7 @@ static bool single_pass_geometry(int64_t rows, int64_t cols, int r_t, int nsm, i
 
 template <int R_T>
 static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, const void* x, const float* amax_t,
-                     bool after_kernel, bool* finalize_last, cudaStream_t st) {
+                     bool after_kernel, bool* finalize_last, const SumJob& job, cudaStream_t st) {
   constexpr int NG = (R_T + 63) / 64;
   constexpr int D_BYTES = NG * QF_DG_BYTES;
   const int nsm = sm_count() < QF_MAX_GRID ? sm_count() : QF_MAX_GRID;
@@ -616,7 +631,7 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
       attr[0].val.programmaticStreamSerializationAllowed = 1;
       cfg.attrs = attr;
       cfg.numAttrs = pdl_enabled() ? 1 : 0;
-      FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_finalize_h<(R_T > 0 ? R_T : 16)>, p, grid));
+      FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_finalize_h<(R_T > 0 ? R_T : 16)>, p, grid, job));
       if (finalize_last != nullptr) *finalize_last = true;   // the caller's GEMM may start beside it (gemm_pair.cu)
     }
     return FT_OK;
@@ -668,10 +683,14 @@ bool quantize_single_pass_fits(int64_t rows, int64_t cols, int r_t) {
 }
 
 // after_kernel: a kernel of the same call directly precedes this launch in the stream (programmatic edge allowed).
-// finalize_last (may be NULL): set when the last launch is k_finalize_h, which writes only H and Hs.
+// finalize_last (may be NULL): set when the last launch is k_finalize_h, which writes only H and Hs (and the side job).
+// side_job (may be NULL; needs a projection, i.e. a k_finalize_h launch): a slot sum that kernel runs as well.
 int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float* amax_t, const ft_proj* proj,
-                          ft_qtensor* out, void* workspace, bool after_kernel, bool* finalize_last, cudaStream_t st) {
+                          ft_qtensor* out, void* workspace, bool after_kernel, bool* finalize_last,
+                          const SumJob* side_job, cudaStream_t st) {
   const int r_t = proj ? proj->r_t : 0;
+  if (side_job != nullptr && side_job->n_slots > 0 && r_t == 0) return FT_ERR_INVALID_ARG;
+  const SumJob job = side_job != nullptr ? *side_job : SumJob{nullptr, nullptr, 0, 0};
   if (finalize_last != nullptr) *finalize_last = false;
   CUtensorMap mx, md;
   int rc = make_tensor_map_2d(&mx, x, 2, (uint64_t)cols, (uint64_t)rows, (uint64_t)cols * 2, QF_KC, QF_ROWS,
@@ -705,15 +724,15 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
   p.trace = g_qf_trace;
 #endif
   switch (r_t) {
-    case 0: return launch_qf<0>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
-    case 16: return launch_qf<16>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
-    case 32: return launch_qf<32>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
-    case 48: return launch_qf<48>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
-    case 64: return launch_qf<64>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
-    case 80: return launch_qf<80>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
-    case 96: return launch_qf<96>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
-    case 112: return launch_qf<112>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
-    case 128: return launch_qf<128>(mx, md, p, x, amax_t, after_kernel, finalize_last, st);
+    case 0: return launch_qf<0>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
+    case 16: return launch_qf<16>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
+    case 32: return launch_qf<32>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
+    case 48: return launch_qf<48>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
+    case 64: return launch_qf<64>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
+    case 80: return launch_qf<80>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
+    case 96: return launch_qf<96>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
+    case 112: return launch_qf<112>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
+    case 128: return launch_qf<128>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
     default: return FT_ERR_UNSUPPORTED_SHAPE;
   }
 }
