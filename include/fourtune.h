@@ -141,6 +141,27 @@ int ft_quantize_blockwise(const void* x_bf16, int64_t rows, int64_t cols,
                           ft_qtensor* out, int32_t round_mode, uint64_t seed, uint64_t offset,
                           void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- ft_quantize_blockwise without a caller workspace and without any device allocation: for callers that cannot
+ * call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid it).  The scratch the
+ * pass needs (control words + the fp32 partial sums of the fused projection) lives in a static device array of
+ * ft_static_scratch_bytes() = 8 MiB inside the library, held by every GPU that loads the library until the process
+ * exits.  Same kernels, same results, same arguments as ft_quantize_blockwise with block_rows == 1 and
+ * FT_ROUND_NEAREST_EVEN (tensor_amax == NULL: the library finds it).  x, proj->down in; out (codes,
+ * sf, tensor_dec_scale), proj->out, proj->out_scaled are the caller's device buffers.
+ * Limit: ft_static_scratch_needed(rows, r_t) <= ft_static_scratch_bytes(): any size without a projection; with one,
+ *   rows <= 5450 at r_t = 64 (the 4608-token FLUX activations fit), rows <= 27 000 at r_t = 32, never for r_t >= 96
+ *   (the partial sums take 192 slots of 128 x r_t floats).  Beyond it the call returns FT_ERR_WORKSPACE_TOO_SMALL
+ *   and launches nothing (use ft_quantize_blockwise with a workspace).
+ * The call allocates nothing (no cudaMalloc / cudaFree, no allocating library routine); it enqueues one 4 KB memset
+ *   node (the control words) and the kernels on `stream`.
+ * All calls on a device share the one array: calls that may OVERLAP on the GPU (different streams without a
+ *   dependency between them) race on it -- serialise them.  Not interchangeable with a caller workspace inside one
+ *   layer call: ft_linear_* still take theirs. */
+int ft_quantize_blockwise_static(const void* x_bf16, int64_t rows, int64_t cols, const float* tensor_amax,
+                                 const ft_proj* proj, ft_qtensor* out, void* stream);
+size_t ft_static_scratch_bytes(void);
+size_t ft_static_scratch_needed(int64_t rows, int32_t r_t);
+
 /* ---- a6 helper: build Q(R)^T ([K x N], N contiguous) from Q(R) ([N x K]) by
  * moving nibbles and scales; nothing is re-quantized.
  * r_kmajor: block_rows 16, sf_layout FT_SF_ROWMAJOR (S[N/16][K/16]).

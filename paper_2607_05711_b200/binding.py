@@ -53,6 +53,10 @@ def lib():
         L.ft_quantize_blockwise.argtypes = [vp, i64, i64, vp, C.POINTER(_Proj), C.POINTER(_QT), i32, C.c_uint64, C.c_uint64,
                                             vp, sz, vp]
         L.ft_pack_weight.argtypes = [C.POINTER(_QT), C.POINTER(_QT), C.POINTER(_QT), vp]
+        L.ft_quantize_blockwise_static.argtypes = [vp, i64, i64, vp, C.POINTER(_Proj), C.POINTER(_QT), vp]
+        L.ft_static_scratch_bytes.restype = sz
+        L.ft_static_scratch_needed.argtypes = [i64, i32]
+        L.ft_static_scratch_needed.restype = sz
         L.ft_weight_transpose_codes.argtypes = [C.POINTER(_QT), vp, vp]
         L.ft_linear_fwd.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
         L.ft_linear_bwd_dgrad.argtypes = [C.POINTER(_Layer), vp, i64, vp, vp, C.POINTER(_QT), vp, sz, vp]
@@ -185,6 +189,23 @@ def ft_quantize_blockwise(x, out, tensor_amax=None, down=None, h_out=None, hs_ou
                                        None if proj is None else C.byref(proj), C.byref(q),
                                        round_mode, seed, offset, _ptr(workspace), workspace.numel(),
                                        _stream(stream)))
+    return out
+
+
+def ft_quantize_blockwise_static(x, out, tensor_amax=None, down=None, h_out=None, hs_out=None, other_dec_scale=None,
+                                 stream=None):
+    """ft_quantize_blockwise on the library's static scratch array: no workspace argument, no device allocation."""
+    _bf16(x)
+    rows, cols = x.shape
+    proj = None
+    if down is not None:
+        _bf16(down)
+        proj = _Proj(down.data_ptr(), None if h_out is None else h_out.data_ptr(),
+                     None if hs_out is None else hs_out.data_ptr(),
+                     None if other_dec_scale is None else other_dec_scale.data_ptr(), down.shape[1])
+    q = out.c()
+    _check(lib().ft_quantize_blockwise_static(_ptr(x), rows, cols, _ptr(tensor_amax),
+                                              None if proj is None else C.byref(proj), C.byref(q), _stream(stream)))
     return out
 
 

@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfourtune.so")
-SOURCES = ["api.cu", "quantize.cu", "quantize_fused.cu", "gemm.cu", "gemm_pair.cu", "gemm_mlp.cu", "wgrad.cu", "wgrad_stream.cu", "wgrad_q4.cu"]
+SOURCES = ["api.cu", "quantize.cu", "quantize_fused.cu", "gemm.cu", "gemm_pair.cu", "gemm_mlp.cu", "wgrad.cu", "wgrad_stream.cu", "wgrad_q4.cu", "no_alloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
