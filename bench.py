@@ -29,10 +29,11 @@ METRIC = "W4A4G4 linear fwd+bwd TFLOPS (4*M*N*K per step / step time)"
 UNIT = "TFLOP/s"
 FP4_OVER_BF16 = 4.0   # nominal dense ratio 9 / 2.25 PFLOP/s (B200_PROFILING.md)
 FP4_NOMINAL_TFLOPS = 9000.0   # dense NVFP4, B200 (B200_PROFILING.md): the peak north_star's 60 % bar refers to
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture of the C2 step
-# summarised in profiles/r02_full_summary.md (ncu flushes the caches before every launch: cold-cache figures)
-NCU_DRAM_TRAFFIC = {"gemm_fwd": None, "gemm_dgrad": None, "quantize_X": None, "quantize_G": None,
-                    "wgrad_dBt": None, "wgrad_dA": None}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes) from the ncu --set full capture of the C2 step
+# summarised in profiles/r02_full_summary.md (ncu flushes the caches before every launch: cold-cache figures; the
+# quantize entries include their k_finalize_h launch)
+NCU_DRAM_TRAFFIC = {"gemm_fwd": 61.37e6, "gemm_dgrad": 43.54e6, "quantize_X": 34.66e6, "quantize_G": 102.83e6,
+                    "wgrad_dBt": 89.32e6, "wgrad_dA": 29.32e6}
 PROBE_SRC = os.path.join(ROOT, "bench_fp4_probe.cu")
 PROBE_BIN = os.path.join(ROOT, "build", "bench_fp4_probe")
 
@@ -466,7 +467,9 @@ def run_ours(args):
             gbs = nbytes / us / 1e3
             return {"kernel": kernel, "step": step, "bound": "hbm", "work": nbytes, "work_unit": "bytes", "us": round(us, 2),
                     "achieved": gbs, "unit": "GB/s", "peak": peaks["hbm"], "frac": gbs / peaks["hbm"],
-                    "frac_of_nominal_8TBps": gbs / 8000.0, "traffic": NCU_DRAM_TRAFFIC[key]}
+                    "frac_of_nominal_8TBps": gbs / 8000.0,
+                    "traffic": None if key is None else (NCU_DRAM_TRAFFIC["wgrad_dBt"] + NCU_DRAM_TRAFFIC["wgrad_dA"]
+                                                         if key == "wgrad_step" else NCU_DRAM_TRAFFIC[key])}
         qb = 2.5625 + 4.0 * r_t / K                       # codes + scales + H, Hs and the D slice per element of X
         qbg = 2.5625 + 4.0 * r_t / N
         roofs = [
@@ -476,8 +479,11 @@ def run_ours(args):
                       qb * M * K, kern["quantize_X_a0a1_us"], "quantize_X"),
             hbm_entry("k_quantize_fused<64,streaming> + k_finalize_h (G, amax given)", "a3", qbg * M * N,
                       kern["quantize_G_a3_us"], "quantize_G"),
-            hbm_entry("k_wgrad<32> (dA and dB^T in one launch: reads X and G once)", "a5", 2.0 * M * (K + N),
-                      kern["wgrad_dA_dBt_us"], "wgrad_dBt"),
+            hbm_entry("ft_lora_wgrad: k_wgrad<32,256> (dA and dB^T in one launch of cluster CTAs: reads X and G once)",
+                      "a5", 2.0 * M * (K + N), kern["wgrad_dA_dBt_us"], None),
+            hbm_entry("k_wgrad_s<32> dB^T (+ amax of G, clears dA) and dA inside ft_linear_bwd: bwd_us - a3 - a4 (derived: "
+                      "the dA launch runs partly beside the dgrad GEMM's tail)", "a5 in the step", 2.0 * M * (K + N),
+                      kern["bwd_us"] - kern["quantize_G_a3_us"] - kern["gemm_dgrad_us"], "wgrad_step"),
         ]
         gemm_us = 0.5 * (kern["gemm_fwd_us"] + kern["gemm_dgrad_us"])
         gemm_tflops = gemm_flop / (gemm_us * 1e-6) / 1e12
@@ -509,7 +515,7 @@ def run_ours(args):
                          "frac_of_derived": gemm_tflops / fp4_derived,
                          "derived_peak": fp4_derived,
                          "derived_note": "measured bf16 burst %.1f x nominal fp4/bf16 ratio 4 (of %s)" % (peaks["bf16"], peaks["source"]),
-                         "traffic": NCU_DRAM_TRAFFIC["gemm_fwd"]},
+                         "traffic": 0.5 * (NCU_DRAM_TRAFFIC["gemm_fwd"] + NCU_DRAM_TRAFFIC["gemm_dgrad"])},
             "roofline_kernels": roofs,
             "fp4_probe": probe,
             "kernels_us": {k: round(v, 2) for k, v in kern.items()},

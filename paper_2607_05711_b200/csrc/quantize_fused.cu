@@ -24,7 +24,7 @@
 // row over its slots in CTA order and writes bf16 H and Hs = H * (1 / alpha): no atomics on the data, a
 // fixed summation order (the same bits on every run), thousands of threads with one L2 round trip each, and
 // the GEMM that follows runs its 4-bit stages beside it (gemm_pair.cu, lr_late).  Measured in round 2 and
-// dropped (profiles/r02_quantize_trace.md): the sums inside this kernel -- by the CTA whose arrival completes
+// dropped (profiles/r02_experiments.md, B2): the sums inside this kernel -- by the CTA whose arrival completes
 // a row tile (36 finalizers, each a chain of L2 round trips: 6-11 us of tail at C2), or by every CTA behind a
 // grid barrier (imbalance + drain + fence + poll + sum: 6-8 us of tail that nothing can overlap); fp32
 // reductions into one accumulator (REDG issues at ~1.3 cycles per lane and word).
