@@ -2,9 +2,9 @@
 """bench.py -- W4A4G4 triple-branch linear, fwd + bwd, on synthetic FLUX.1-dev-shaped input.
 
 A step = one pass of the whole hot path (rows a0-a5) over one batch:
-    ft_linear_fwd (one kernel: tensor amax + quantize + down-projection of X; 4-bit GEMM + up-projection)
-    ft_linear_bwd (dB^T with the amax of G as a by-product; quantize + down-projection of G; 4-bit GEMM
-                   with Q(R)^T; dA)
+    ft_linear_fwd (one kernel: tensor amax + quantize + down-projection of X; its slot sums; 4-bit GEMM + up-projection)
+    ft_linear_bwd (dB^T partials with the amax of G as a by-product; quantize + down-projection of G; slot sums of P and
+                   dB^T; 4-bit GEMM with Q(R)^T; dA)                                       -- 8 kernel launches
 Workload at N=1: BASELINE.json configs[1] (C2): fused QKV projection M=4608, K=3072, N=9216,
 stabilizer rank 32, LoRA rank 32.  N>1: every rank runs the same layer on its own batch of 4608
 tokens (weak scaling) and all-reduces the LoRA gradients (NCCL), the path's only exchange.
