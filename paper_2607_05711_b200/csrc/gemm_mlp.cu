@@ -72,12 +72,6 @@ __device__ __forceinline__ float gelu_sigmoid_f32(float u) {
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(s) : "f"(1.0f + e));
   return s;
 }
-// one 32-byte store (sm_100: 256-bit global accesses); p is 32-byte aligned
-__device__ __forceinline__ void st_global_v8(void* p, uint4 a, uint4 b) {
-  asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(p), "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w),
-               "r"(b.x), "r"(b.y), "r"(b.z), "r"(b.w)
-               : "memory");
-}
 // GeLU, tanh form: 0.5 u (1 + tanh t) = u sigmoid(2 t)
 __device__ __forceinline__ float gelu_tanh_f32(float u) { return u * gelu_sigmoid_f32(u); }
 
