@@ -4,7 +4,7 @@
 // tile.  Each CTA stages its own 128 rows of A and its own BN/2-row half of B, so a CTA moves
 // 128 + BN/2 operand rows through its shared memory per 128 x BN of output.  Ring: 5 stages of one K = 256 step.
 // What paces the main loop (round 2, clock64 around the issuing thread's waits and FT_TRACE ablations,
-// profiles/r02_experiments.md A3/B6): the single issuing thread spends ~530 cycles per stage whatever the tile width
+// profiles/r02_experiments.md B6, B7): the single issuing thread spends ~530 cycles per stage whatever the tile width
 // (a barrier wait of >= 100, 16 tcgen05 instructions, a multicast commit, the loop) against 512 (BN = 256) or 448
 // (BN = 224) cycles of MMA; on top of that the forward pass, which writes a 256 x 224 tile every 13 stages, waits
 // ~80 cycles per stage longer for its operands while the output is being stored (no stores: 69 k instead of 80 k
@@ -143,8 +143,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
     // ===================================================== TMA producers (both CTAs): warp 0 loads A and its scales,
     // warp 3 loads B and its scales.  One thread pays ~95 cycles per TMA instruction it issues (plus ~40 for the
     // expect-arrive and >= 55 for the wait): five loads per K=256 stage from one thread are ~600 cycles of issue
-    // against 512 cycles of MMA -- that, not bytes, was what the main loop waited for (profiles/r02_experiments.md
-    // A3).  Two threads in different warps issue side by side.
+    // against 512 cycles of MMA (profiles/r02_experiments.md B7).  Two threads in different warps issue side by side.
     if (elect_one()) {
       const bool load_a = warp == 0;
       int stage = 0;
