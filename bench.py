@@ -206,7 +206,7 @@ def run_ours(args):
     R, L1, L2t = prepare.random_range_split(Wt, r_s, seed=w["seed"])     # offline (Eq. 1)
     D_f = torch.cat([L1, A], 1).contiguous()
     U_t = torch.cat([L2t, Bt], 1).contiguous()
-    layer = B.Layer(R, D_f, U_t, r_s, r)                                 # offline: Q(R), both packings
+    layer = B.Layer(R, D_f, U_t, r_s, r, tokens=M)                       # offline: Q(R), both packings; tile-cut scales for M tokens
     X, G = Xh.to(dev), Gh.to(dev)
     y = torch.empty(M, N, dtype=torch.bfloat16, device=dev)
     dx = torch.empty(M, K, dtype=torch.bfloat16, device=dev)
@@ -613,7 +613,7 @@ def sweep(B, prepare, dev, graph_us, peaks, full=False):
         W = (torch.randn(N, K, device=dev, generator=g) * 0.02).to(torch.bfloat16)
         D_f = (torch.randn(K, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
         U_t = (torch.randn(N, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
-        layer = B.Layer(W, D_f, U_t, r_s, r)
+        layer = B.Layer(W, D_f, U_t, r_s, r, tokens=M)
         y = torch.empty(M, N, dtype=torch.bfloat16, device=dev)
         dx = torch.empty(M, K, dtype=torch.bfloat16, device=dev)
         h = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)
@@ -752,7 +752,7 @@ def fusion_ablation(B, dev, acts, g):
     W = (torch.randn(N, K, device=dev, generator=g) * 0.02).to(torch.bfloat16)
     D_f = (torch.randn(K, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
     U_t = (torch.randn(N, r_t, device=dev, generator=g) * 0.01).to(torch.bfloat16)
-    layer = B.Layer(W, D_f, U_t, r_s, r)
+    layer = B.Layer(W, D_f, U_t, r_s, r, tokens=M)
     y = torch.empty(M, N, dtype=torch.bfloat16, device=dev)
     dx = torch.empty(M, K, dtype=torch.bfloat16, device=dev)
     h = torch.empty(M, r_t, dtype=torch.bfloat16, device=dev)

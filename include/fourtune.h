@@ -80,7 +80,7 @@ typedef struct {
   int32_t block_rows;      /* 1 (activations, gradients) or 16 (weights, 16x16 blocks)  */
   int32_t sf_layout;       /* FT_SF_ROWMAJOR or FT_SF_TILE128x4                          */
   /* optional, weights only (NULL / 0 otherwise): the same scales once more, cut to the GEMM's output-tile
-   * width `ntile` (224, or 192 for the FC1 of ft_mlp_fwd): for row tile nt = row / ntile and K=64 step ks two 512-byte groups -- rows
+   * width `ntile` (224 or 240, or 192 for the FC1 of ft_mlp_fwd): for row tile nt = row / ntile and K=64 step ks two 512-byte groups -- rows
    * nt*ntile + 0..127 and + 128..ntile-1 of the tile, each in the (r%32)*16 + (r/32)*4 + c%4 order of
    * FT_SF_TILE128x4, rows past the tile or the tensor zero -- at ((nt * cols/64 + ks) * 2 + half) * 512.
    * ft_sf_ntile_bytes() bytes, filled by ft_pack_weight.  With it ft_gemm4 / ft_linear_* may run 256 x ntile
@@ -169,7 +169,7 @@ size_t ft_static_scratch_needed(int64_t rows, int32_t r_t);
  * value copied), and, if r_kmajor_tiled != NULL, the TILE128x4 expansion of the
  * forward operand's scales (its codes/tensor_dec_scale pointers are not written;
  * point them at r_kmajor's buffers).  For each of the two outputs whose sf_ntile is non-NULL and whose ntile
- * is 224 or 192, the tile-cut copy of the scales as well.  N % 64 == 0 and K % 64 == 0. */
+ * is 224, 240 or 192, the tile-cut copy of the scales as well.  N % 64 == 0 and K % 64 == 0. */
 int ft_pack_weight(const ft_qtensor* r_kmajor, ft_qtensor* r_kmajor_tiled,
                    ft_qtensor* r_nmajor, void* stream);
 
@@ -283,6 +283,11 @@ int ft_gelu_bwd_q4(const void* dz_bf16, const ft_qtensor* qy1, void* dy1_bf16, v
 /* ---- sizes and diagnostics (host only, no CUDA calls) */
 size_t ft_sf_bytes(int64_t rows, int64_t cols, int32_t block_rows, int32_t layout);
 size_t ft_sf_ntile_bytes(int64_t rows, int64_t cols, int32_t ntile);   /* ft_qtensor::sf_ntile */
+/* The tile width worth packing ft_qtensor::sf_ntile for, for a weight operand [N x K] that will meet M tokens
+ * (with a low-rank term of rank r_t): 224 or 240, or 0 if the GEMM will use its 256-wide tiles anyway (which need
+ * no tile-cut scales).  Host only (the library's cost model of its own schedule on the current device); any of the
+ * three choices gives the same results, only the speed differs. */
+int32_t ft_gemm_best_ntile(int64_t M, int64_t N, int64_t K, int32_t r_t);
 size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t);
 /* Zero the control words at the head of a workspace (one 4 KB memset on `stream`).  Needed once per buffer,
  * before its first use, unless the caller zero-filled it; never per call.  Also the way to recover a workspace

@@ -11,7 +11,7 @@ extern "C" {
 /* GEMM variant: 0 = default (the library picks the CTA-pair kernel and its tile width per shape);
  * 128, 192, 256 = the 1-CTA kernel with that N tile (kept as a cross-check of the pair kernel);
  * 1000 + bn = the CTA-pair kernel with tile width bn (bn = 256: scale columns overlaid on the draining
- * accumulator; bn = 224: scale columns of their own; falls back to 256 if the weight operand carries no
+ * accumulator; bn = 224 / 240: scale columns of their own; falls back to 256 if the weight operand carries no
  * scales cut to that width). */
 int ft_debug_set_gemm_tile_n(int bn);
 /* quantizer route: 0 = default (single-pass amax + quantize when the tensor fits the SMs' shared memory),

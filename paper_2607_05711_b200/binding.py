@@ -75,6 +75,8 @@ def lib():
         L.ft_mlp_workspace_hs2_offset.restype = sz
         L.ft_gelu_bwd_q4.argtypes = [vp, C.POINTER(_QT), vp, vp]
         L.ft_sf_ntile_bytes.argtypes = [i64, i64, i32]
+        L.ft_gemm_best_ntile.argtypes = [i64, i64, i64, i32]
+        L.ft_gemm_best_ntile.restype = i32
         L.ft_sf_ntile_bytes.restype = sz
         L.ft_workspace_bytes.argtypes = [i64, i64, i64, i32]
         L.ft_workspace_bytes.restype = sz
@@ -212,8 +214,10 @@ def ft_quantize_blockwise_static(x, out, tensor_amax=None, down=None, h_out=None
 class Layer:
     """ft_layer: Q(R) in both orientations plus the low-rank factors D_f [K x r_t], U_t [N x r_t]."""
 
-    def __init__(self, R_bf16, D_f, U_t, r_s, r, stream=None, ntile=224):
-        """ntile: width of the tile-cut copy of the forward operand's scales (224; 192 for the FC1 of ft_mlp_fwd)."""
+    def __init__(self, R_bf16, D_f, U_t, r_s, r, stream=None, ntile=224, tokens=None):
+        """ntile: width of the tile-cut copy of the forward operand's scales (224 or 240; 192 for the FC1 of ft_mlp_fwd).
+        tokens: the M this layer will run at; given, the library's cost model (ft_gemm_best_ntile) picks the widths
+        for both operands (same results either way, only the GEMM's tile schedule differs)."""
         _bf16(R_bf16)
         N, K = R_bf16.shape
         self.N, self.K, self.r_s, self.r = N, K, r_s, r
@@ -225,10 +229,14 @@ class Layer:
         # a6: offline quantize (16x16 blocks, row-major S) then re-pack both orientations
         self.q_rowmajor = QTensor(N, K, 16, FT_SF_ROWMAJOR, dev)
         ft_quantize_blockwise(R_bf16, self.q_rowmajor, stream=stream)
+        nt_bwd = ntile if ntile in (224, 240) else 224
+        if tokens is not None:
+            ntile = lib().ft_gemm_best_ntile(tokens, N, K, r_s + r) or 224
+            nt_bwd = lib().ft_gemm_best_ntile(tokens, K, N, r_s + r) or 224
         self.r_kmajor = QTensor(N, K, 16, FT_SF_TILE128x4, dev).with_ntile(ntile)
         self.r_kmajor.codes = self.q_rowmajor.codes
         self.r_kmajor.tensor_dec_scale = self.q_rowmajor.tensor_dec_scale
-        self.r_nmajor = QTensor(K, N, 16, FT_SF_TILE128x4, dev).with_ntile(224)
+        self.r_nmajor = QTensor(K, N, 16, FT_SF_TILE128x4, dev).with_ntile(nt_bwd)
         qk, qkt, qn = self.q_rowmajor.c(), self.r_kmajor.c(), self.r_nmajor.c()
         _check(lib().ft_pack_weight(C.byref(qk), C.byref(qkt), C.byref(qn), _stream(stream)))
 

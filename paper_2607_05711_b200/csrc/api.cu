@@ -26,6 +26,7 @@ int launch_wgrad_stream(const void* in, const void* l, int64_t M, int64_t F, int
                         float* zero_fill, int64_t zero_fill_n, bool after_kernel, bool beside_prev, cudaStream_t st);
 int launch_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, cudaStream_t st);
 int launch_transpose_codes(const uint8_t* src, uint8_t* dst, int64_t N, int64_t K, cudaStream_t st);
+int best_pair_ntile(int64_t M, int64_t N, int64_t K, int r_t);
 int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N, int64_t K,
                  const void* lr_a_scaled, const void* lr_b, int r_t, void* out_bf16, bool lr_late,
                  cudaStream_t st);
@@ -280,6 +281,11 @@ size_t ft_sf_ntile_bytes(int64_t rows, int64_t cols, int32_t ntile) {
   return (size_t)(ceil_div(rows, ntile) * ceil_div(cols, 64) * 1024);
 }
 
+int32_t ft_gemm_best_ntile(int64_t M, int64_t N, int64_t K, int32_t r_t) {
+  if (M < 1 || N < 64 || K < 64 || r_t < 0) return 0;
+  return best_pair_ntile(M, N, K, r_t);
+}
+
 size_t ft_workspace_bytes(int64_t M, int64_t K, int64_t N, int32_t r_t) {
   (void)K;
   (void)N;
@@ -358,7 +364,7 @@ int ft_pack_weight(const ft_qtensor* rk, ft_qtensor* rk_tiled, ft_qtensor* rn, v
   if (rk_tiled && !rk_tiled->sf) return FT_ERR_INVALID_ARG;
   const ft_qtensor* outs[2] = {rk_tiled, rn};
   for (int i = 0; i < 2; ++i)
-    if (outs[i] && outs[i]->sf_ntile != nullptr && ((outs[i]->ntile != 224 && outs[i]->ntile != 192) || !aligned16(outs[i]->sf_ntile)))
+    if (outs[i] && outs[i]->sf_ntile != nullptr && ((outs[i]->ntile != 224 && outs[i]->ntile != 240 && outs[i]->ntile != 192) || !aligned16(outs[i]->sf_ntile)))
       return FT_ERR_INVALID_ARG;
   if (rk->rows % 64 != 0 || rk->cols % 64 != 0 || rk->rows < 64 || rk->cols < 64)
     return FT_ERR_UNSUPPORTED_SHAPE;

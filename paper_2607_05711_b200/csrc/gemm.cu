@@ -298,7 +298,7 @@ int launch_gemm4(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64_t N,
 }  // namespace ft
 
 extern "C" int ft_debug_set_gemm_tile_n(int bn) {
-  if (bn == 1224 || bn == 1256) {   // the CTA-pair kernel with a forced tile width
+  if (bn == 1224 || bn == 1240 || bn == 1256) {   // the CTA-pair kernel with a forced tile width
     ft::g_force_bn = 0;
     ft::g_pair_bn = bn - 1000;
     return FT_OK;

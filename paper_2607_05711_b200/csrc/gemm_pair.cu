@@ -57,7 +57,8 @@ struct PairCfg {
   static constexpr int STAGES = 5;
   static constexpr int SMEM = STAGES * STAGE_BYTES + 1024;
   static constexpr uint32_t SF_COL = OVERLAY ? 0 : 2 * BN;   // TMEM column of the scales (OVERLAY: per tile)
-  static_assert(BN % 32 == 0 && BN <= 256 && (OVERLAY || 2 * BN + 64 <= 512), "tile width");
+  static constexpr bool SF_PER_STEP = !OVERLAY && 2 * BN + 64 <= 512;   // 16 scale columns for each K=64 step of a stage
+  static_assert(BN % 16 == 0 && BN <= 256 && (OVERLAY || 2 * BN + 16 <= 512), "tile width");
   static_assert(STAGE_BYTES % 1024 == 0, "stage buffers stay 1024-byte aligned");
 };
 
@@ -99,7 +100,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
   const int klr = (p.r_t + 63) / 64;
   const int kiters = k4 + klr;
   const int64_t sf_tiles_k = p.K / 64;
-  // width of tile column nt: BN, or what is left of N (a multiple of 32: N % 64 == 0, BN % 32 == 0)
+  // width of tile column nt: BN, or what is left of N (a multiple of 16: N % 64 == 0, BN % 16 == 0)
   auto n_eff_of = [&](int64_t nt) { return (int)min((int64_t)BN, p.N - nt * BN); };
 
   if (threadIdx.x == 0) {
@@ -262,8 +263,8 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
           const uint64_t dfa = make_smem_desc(ssfa, 128, 0, 0), dfb = make_smem_desc(ssfb, 128, 0, 0);
           // B scales of step k: OVERLAY: 512 B at k * 512 of each of the two 2 KB scale tiles;
           // else 1 KB (both halves) at k * 1024
-          // BN < 256: every K=64 step of a stage has its own 16 scale columns (2 BN + 64 <= 512), so the copies of
-          // step k + 1 need not wait until the MMA of step k has read its scales
+          // BN <= 224: every K=64 step of a stage has its own 16 scale columns (2 BN + 64 <= 512), so the copies of
+          // step k + 1 need not wait until the MMA of step k has read its scales (measured: no difference)
           auto step = [&](int k, uint32_t acc) {
             if constexpr (OVERLAY) {
               tc_cp_sf_pair(sfa_t, dfa + (uint64_t)(k * 32));
@@ -271,7 +272,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
               tc_cp_sf_pair(sfb_t + 4, dfb + (uint64_t)(128 + k * 32));
               mma_nvf4_pair(acc_t, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc4, sfa_t, sfb_t, acc);
             } else {
-              const uint32_t fa = sfa_t + 16 * k, fb = fa + 8;
+              const uint32_t fa = sfa_t + (Cfg::SF_PER_STEP ? 16 * k : 0), fb = fa + 8;
               tc_cp_sf_pair(fa, dfa + (uint64_t)(k * 32));
               tc_cp_sf_pair(fb, dfb + (uint64_t)(k * 64));
               tc_cp_sf_pair(fb + 4, dfb + (uint64_t)(k * 64 + 32));
@@ -374,7 +375,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
 #pragma unroll 1
       for (int u = grp; u < n_units; u += 2) {
         const int c0 = u * 64;
-        const bool narrow = n_eff - c0 <= 32;   // a 32-column unit (only the last one of a 224-wide or ragged tile)
+        const int w = min(64, n_eff - c0);   // unit width: 64, or what is left of the tile (a multiple of 16)
         uint32_t v[64];
         if (OVERLAY && u == 0) {
           // columns 0-15 of this accumulator are the next tile's scale-factor buffer: read them first and
@@ -384,11 +385,14 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster(map_to_cta(smem_u32(&sf_free[a]), 0));
-          tmem_ld16(t0 + 16, *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
-        } else {
+          if (w > 16) tmem_ld16(t0 + 16, *reinterpret_cast<uint32_t(*)[16]>(&v[16]));
+        } else if (w >= 32) {
           tmem_ld32(t0 + c0, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
+        } else {
+          tmem_ld16(t0 + c0, *reinterpret_cast<uint32_t(*)[16]>(&v[0]));
         }
-        if (!narrow) tmem_ld32(t0 + c0 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
+        if (w == 64) tmem_ld32(t0 + c0 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
+        else if (w == 48) tmem_ld16(t0 + c0 + 32, *reinterpret_cast<uint32_t(*)[16]>(&v[32]));
         tmem_ld_wait();
         if (u == last_u) {   // this warp's part of the accumulator is in registers: hand it back
           tc_fence_before();
@@ -396,7 +400,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
           if (lane == 0) mbar_arrive_cluster(map_to_cta(smem_u32(&acc_empty[a]), 0));
           released = true;
         }
-        // bf16( alpha * acc ): a thread holds 64 (32) consecutive columns of one row = 128 (64) bytes, stored as
+        // bf16( alpha * acc ): a thread holds up to 64 consecutive columns of one row = 128 bytes, stored as
         // 256-bit pieces: every store instruction fills whole 32-byte sectors.  (Staging the tile in shared memory
         // for a TMA store put the output through the shared-memory ports and the TMA unit that the operand loads
         // need: the forward pass, one 256 x 224 tile per 13 stages, ran 21 % slower for it.)
@@ -412,7 +416,7 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
 #endif
         if (grow < p.M) {
           __nv_bfloat16* dst = p.out + grow * p.N + n0 + c0;
-          const int pieces = narrow ? 2 : 4;
+          const int pieces = w / 16;
 #pragma unroll
           for (int j = 0; j < 4; ++j) {
             if (j < pieces) {
@@ -459,27 +463,34 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
 
 int g_pair_bn = 0;   // test / bench hook: 0 = choose per shape, else force this pair tile width
 
-// Tile width for an [M x N] output with reduction length K and a rank-r_t stage, from a cost model of the
-// persistent schedule: rounds of n_pairs tiles, each tile K/64 MMAs of BN/2 cycles (+ the low-rank MMAs) plus,
-// for BN = 256, the ~1.9 k-cycle hand-over of the overlaid scale columns; narrower tiles move ~4 % more operand
-// bytes per MAC through shared memory.
+// Tile width of the pair kernel for a shape: 256, or the width `ntile_avail` (224 / 240) the weight's tile-cut scales
+// were packed for.  Cost model of the persistent schedule (profiles/r02_experiments.md B6): rounds of n_pairs
+// tiles; a K=256 stage costs the issuing thread ~530 cycles or the MMAs' 4 x BN/2, whichever is more; BN = 256 pays
+// the ~1.7 k-cycle hand-over of the overlaid scale columns per tile, the others ~270.
+static double pair_cost(int bn, int64_t M, int64_t N, int64_t K, int r_t, int64_t pairs) {
+  const double stage4 = 4.0 * (bn / 2) > 530.0 ? 4.0 * (bn / 2) : 530.0;
+  double lr = 0.0;   // low-rank stages: up to four K=16 bf16 MMAs of BN/2 cycles each, or the thread's ~300
+  for (int c = 0; c < r_t; c += 64) {
+    const double mma = ((r_t - c < 64 ? r_t - c : 64) / 16) * (bn / 2.0);
+    lr += mma > 300.0 ? mma : 300.0;
+  }
+  const double per_tile = (double)ceil_div(K, 256) * stage4 + lr + (bn == 256 ? 1700.0 : 270.0);
+  const int64_t tiles = ceil_div(M, P_BM) * ceil_div(N, bn);   // a ragged last column tile costs a whole tile's issue time
+  return (double)ceil_div(tiles, pairs) * per_tile;
+}
 static int choose_pair_bn(int64_t M, int64_t N, int64_t K, int r_t, int ntile_avail) {
   if (g_pair_bn != 0) return g_pair_bn;
-  if (ntile_avail != 224) return 256;
+  if (ntile_avail != 224 && ntile_avail != 240) return 256;
   const int64_t pairs = sm_count() / 2;
-  auto cost = [&](int bn) {
-    const double per_tile = (double)(K / 64 + (r_t + 15) / 16) * (bn / 2) * (bn == 256 ? 1.0 : 1.04) +
-                            (bn == 256 ? 1900.0 : 250.0);
-    const int64_t tiles_m = ceil_div(M, P_BM), full_n = N / bn, rest = N - full_n * bn;
-    const int64_t full_tiles = tiles_m * full_n;
-    const double rounds_full = (double)ceil_div(full_tiles, pairs);
-    // the ragged column of tiles runs in the slack of the last round if there is any
-    const int64_t slack = (int64_t)rounds_full * pairs - full_tiles;
-    const int64_t spill = tiles_m > slack ? tiles_m - slack : 0;
-    const double ragged = rest == 0 ? 0.0 : (double)ceil_div(spill, pairs) * rest / bn;
-    return (rounds_full + ragged) * per_tile;
-  };
-  return cost(224) < cost(256) ? 224 : 256;
+  return pair_cost(ntile_avail, M, N, K, r_t, pairs) < pair_cost(256, M, N, K, r_t, pairs) ? ntile_avail : 256;
+}
+// the tile-cut scale layout worth packing for a weight that will meet M tokens: 224, 240, or 0 (256-wide tiles win)
+int best_pair_ntile(int64_t M, int64_t N, int64_t K, int r_t) {
+  const int64_t pairs = sm_count() / 2;
+  const double c224 = pair_cost(224, M, N, K, r_t, pairs), c240 = pair_cost(240, M, N, K, r_t, pairs),
+               c256 = pair_cost(256, M, N, K, r_t, pairs);
+  if (c256 <= c224 && c256 <= c240) return 0;
+  return c240 < c224 ? 240 : 224;
 }
 
 template <int BN>
@@ -549,6 +560,7 @@ int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64
   int bn = choose_pair_bn(M, N, K, r_t, avail);
   if (bn != 256 && bn != avail) bn = 256;   // no scale layout for that width: the 256-wide kernel takes the standard one
   if (bn == 224) return launch_pair_bn<224>(a, b, M, N, K, lr_a, lr_b, r_t, out, lr_late, st);
+  if (bn == 240) return launch_pair_bn<240>(a, b, M, N, K, lr_a, lr_b, r_t, out, lr_late, st);
   return launch_pair_bn<256>(a, b, M, N, K, lr_a, lr_b, r_t, out, lr_late, st);
 }
 

@@ -288,13 +288,13 @@ def test_fused_projection_random_shapes(B, qmode):
 
 
 # ------------------------------------------------------------------ a2 / a4 / a5: the layer
-def make_layer(B, seed, M, K, N, r_s, r, x_kind="outlier"):
+def make_layer(B, seed, M, K, N, r_s, r, x_kind="outlier", ntile=224):
     d = synth.layer_inputs(seed, M, K, N, max(r, 1), x_kind)
     R, L1, L2 = olayer.prepare_weight(d["W"], r_s)
     D_f = np.concatenate([L1, d["A"][:, :r]], 1).astype(np.float32)
     U_f = np.concatenate([L2, d["B"][:r, :]], 0).astype(np.float32)
     r_t = r_s + r
-    L = B.Layer(t16(R), t16(D_f) if r_t else None, t16(U_f.T) if r_t else None, r_s, r)
+    L = B.Layer(t16(R), t16(D_f) if r_t else None, t16(U_f.T) if r_t else None, r_s, r, ntile=ntile)
     return d, R, D_f, U_f, L
 
 
@@ -314,14 +314,14 @@ def range_finder_split(W, r_s, seed):
     return R, L1, L2
 
 
-def make_layer_fast(B, seed, M, K, N, r_s, r, x_kind="outlier"):
+def make_layer_fast(B, seed, M, K, N, r_s, r, x_kind="outlier", ntile=224):
     """make_layer with the range-finder split: for shapes where the full SVD of W would dominate the test."""
     d = synth.layer_inputs(seed, M, K, N, max(r, 1), x_kind)
     R, L1, L2 = range_finder_split(d["W"], r_s, seed)
     D_f = np.concatenate([L1, d["A"][:, :r]], 1).astype(np.float32)
     U_f = np.concatenate([L2, d["B"][:r, :]], 0).astype(np.float32)
     r_t = r_s + r
-    L = B.Layer(t16(R), t16(D_f) if r_t else None, t16(U_f.T) if r_t else None, r_s, r)
+    L = B.Layer(t16(R), t16(D_f) if r_t else None, t16(U_f.T) if r_t else None, r_s, r, ntile=ntile)
     return d, R, D_f, U_f, L
 
 
@@ -354,7 +354,7 @@ def run_layer(B, L, X, G, M, K, N, r_t, r, fused_bwd=False):
                 xt=xt, gt=gt, ht=h, pt=p)
 
 
-LAYER_CASES = [  # seed, M, K, N, r_s, r, tile_n (fourtune_debug.h: 0 auto, 128/192/256 1-CTA, 1224/1256 pair kernel)
+LAYER_CASES = [  # seed, M, K, N, r_s, r, tile_n (fourtune_debug.h: 0 auto, 128/192/256 1-CTA, 1224/1240/1256 pair kernel)
     (11, 1, 64, 64, 0, 0, 0), (12, 128, 256, 128, 0, 0, 256), (13, 130, 320, 192, 16, 16, 0),
     (14, 256, 512, 384, 16, 16, 192), (15, 200, 1024, 768, 32, 64, 256), (16, 300, 576, 448, 32, 32, 128),
     (17, 129, 2048, 640, 0, 16, 192),
@@ -362,14 +362,16 @@ LAYER_CASES = [  # seed, M, K, N, r_s, r, tile_n (fourtune_debug.h: 0 auto, 128/
     # + 192), 768 (3 x 224 + 96: a 32-column unit in a ragged tile), K with a partial stage; and the 256-wide one forced
     (18, 1, 64, 64, 0, 0, 1224), (19, 130, 320, 192, 16, 16, 1224), (20, 300, 576, 448, 32, 32, 1224),
     (21, 129, 2048, 640, 0, 16, 1224), (22, 200, 1024, 768, 32, 64, 1224), (23, 260, 448, 1024, 16, 96, 1224),
-    (24, 300, 576, 448, 32, 32, 1256), (25, 200, 1024, 768, 32, 64, 1256)]
+    (24, 300, 576, 448, 32, 32, 1256), (25, 200, 1024, 768, 32, 64, 1256),
+    (26, 1, 64, 64, 0, 0, 1240), (27, 130, 320, 192, 16, 16, 1240), (28, 300, 576, 448, 32, 32, 1240),
+    (29, 129, 2048, 640, 0, 16, 1240), (30, 260, 448, 1024, 16, 96, 1240), (31, 200, 1024, 960, 32, 64, 1240)]
 
 
 @pytest.mark.parametrize("seed,M,K,N,r_s,r,bn", LAYER_CASES)
 def test_layer_small(B, seed, M, K, N, r_s, r, bn):
     B.debug_set_gemm_tile_n(bn)
     try:
-        d, R, D_f, U_f, L = make_layer(B, seed, M, K, N, r_s, r)
+        d, R, D_f, U_f, L = make_layer(B, seed, M, K, N, r_s, r, ntile=240 if bn == 1240 else 224)
         out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r)
     finally:
         B.debug_set_gemm_tile_n(0)
@@ -454,14 +456,14 @@ MULTI_TILE_CASES = [   # seed, M, K, N, r_s, r
 ]
 
 
-@pytest.mark.parametrize("bn", [1224, 1256], ids=["pair224", "pair256"])
+@pytest.mark.parametrize("bn", [1224, 1240, 1256], ids=["pair224", "pair240", "pair256"])
 @pytest.mark.parametrize("seed,M,K,N,r_s,r", MULTI_TILE_CASES)
 def test_layer_multi_tile_per_cta_pair(B, seed, M, K, N, r_s, r, bn):
     """Both tile widths of the CTA-pair GEMM: 256 (scale columns overlaid on the draining accumulator, hand-over
     per tile) and 224 (scale columns of their own, ragged last tile of every row of tiles)."""
     B.debug_set_gemm_tile_n(bn)
     try:
-        d, R, D_f, U_f, L = make_layer_fast(B, seed, M, K, N, r_s, r)
+        d, R, D_f, U_f, L = make_layer_fast(B, seed, M, K, N, r_s, r, ntile=240 if bn == 1240 else 224)
         out = run_layer(B, L, d["X"], d["dY"], M, K, N, r_s + r, r, fused_bwd=r > 0)
     finally:
         B.debug_set_gemm_tile_n(0)
