@@ -803,6 +803,49 @@ def test_without_programmatic_launch():
     assert r.returncode == 0 and " passed" in r.stdout, r.stdout[-2000:] + r.stderr[-2000:]
 
 
+def test_step_under_cuda_graph_capture_ragged_m(B):
+    """A forward + backward step with ragged M on the streaming route (G too large for the single-pass quantizer),
+    captured into a CUDA graph and replayed: the same bits as the eager step (programmatic edges, the cooperative
+    single-pass launch for X and the cluster launches all have to survive capture; nothing in a call may touch the
+    host after validation)."""
+    M, K, N, r_s, r = 4500, 512, 4096, 32, 32      # 35.2 rows of 128: a ragged last row tile; G = 36.9 MB
+    r_t = r_s + r
+    d, R, D_f, U_f, L = make_layer(B, 63, M, K, N, r_s, r)
+    x, g = t16(d["X"]), t16(d["dY"])
+    y = torch.zeros(M, N, dtype=torch.bfloat16, device="cuda"); dx = torch.zeros(M, K, dtype=torch.bfloat16, device="cuda")
+    h = torch.zeros(M, r_t, dtype=torch.bfloat16, device="cuda"); p = torch.zeros_like(h)
+    ws = B.new_workspace(M, max(K, N), max(K, N), r_t, "cuda")
+    qx, qg = B.QTensor(M, K), B.QTensor(M, N)
+    dA = torch.zeros(K, r, dtype=torch.float32, device="cuda"); dBt = torch.zeros(N, r, dtype=torch.float32, device="cuda")
+    outs = (y, dx, h, p, qx.codes, qx.sf, qg.codes, qg.sf, dBt)
+
+    def step():
+        B.ft_linear_fwd(L, x, y, h, qx, ws)
+        B.ft_linear_bwd(L, x, g, h, dx, p, dA, dBt, qg, ws)
+
+    step()
+    torch.cuda.synchronize()
+    want = [t.clone() for t in outs]
+    want_dA = dA.clone()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        step()                                     # warm the stream (tensor-map memo, function attributes)
+        side.synchronize()
+        with torch.cuda.graph(graph, stream=side):
+            step()
+    for rep in range(3):
+        for t in outs:
+            t.zero_()
+        dA.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        for j, (t, w) in enumerate(zip(outs, want)):
+            assert torch.equal(t, w), (rep, j)
+        assert rel(dA.cpu().numpy(), want_dA.cpu().numpy()) <= 1e-5
+
+
 def test_back_to_back_steps_without_sync(B):
     """The programmatic-launch shortcuts (dgrad GEMM started beside k_finalize_h, dA kernels started beside the
     GEMM with their wait at the end, clear kernels with programmatic edges) must not let a step see a neighbour's
