@@ -18,6 +18,7 @@
 // TMEM: two 192-column accumulators, 16 scale columns, r2 <= 112 columns of H2: 512.
 // 12 epilogue warps (the epilogue is ~19 instructions per element: the MMAs of a tile take ~5.6 k cycles).
 // Shared memory: 4 ring stages of 34 KB, the 48 KB z tile, the 24 KB D_f2 slice (this CTA's r2 / 2 columns).
+#include <cstdio>
 #include <cstdlib>
 
 #include "common.cuh"
@@ -112,7 +113,7 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
     prefetch_tmap(&map_sfb);
     prefetch_tmap(&map_d2);
     for (int s = 0; s < ML_STAGES; ++s) {
-      mbar_init(&full_bar[s], 1);
+      mbar_init(&full_bar[s], 2);   // the leader's two producer threads
       mbar_init(&empty_bar[s], 1);
     }
     for (int a = 0; a < 2; ++a) {
@@ -144,9 +145,12 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
   pdl_wait();      // everything this kernel reads comes from the quantize pass before it (and k_finalize_h: Hs)
   pdl_trigger();
 
-  if (warp == 0) {
-    // ===================================================== TMA producer (both CTAs)
+  if (warp == 0 || warp == 3) {
+    // ===================================================== TMA producers (both CTAs): warp 0 loads A (X codes, Hs) and its
+    // scales, warp 3 loads B (weight codes, U) with its scales and the D_f2 slices.  A thread pays ~95 cycles per TMA
+    // instruction it issues: four per stage from one thread were 600 of the K loop's cycles per stage (gemm_pair.cu).
     if (elect_one()) {
+      const bool load_a = warp == 0;
       int stage = 0;
       uint32_t phase = 0;
       // The D_f2 slice of tile j goes into the single slice buffer once the H2 MMAs of tile j - 1 have read it (z_free).
@@ -164,38 +168,44 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
       const int kt_d2 = min(ML_STAGES, kiters - 1);
       for (int i = 0; i <= n_local; ++i) {
         if (i == n_local) {
-          load_d2(i - 1);
+          if (!load_a) load_d2(i - 1);
           break;
         }
         const int64_t tile = t_begin + i;
         const int64_t mt = tile / tiles_n, nt = tile % tiles_n;
         const int32_t m0 = (int32_t)(mt * ML_BM + rank * 128);
         const int32_t nb0 = (int32_t)(nt * ML_BN + rank * (ML_BN / 2));
-        const int64_t sfa_rt = mt * 2 + rank;
+        const int32_t sfa_row = (int32_t)((mt * 2 + rank) * sf_tiles_k), sfb_row = (int32_t)(nt * sf_tiles_k);
         for (int kt = 0; kt < kiters; ++kt) {
           mbar_wait(&empty_bar[stage], phase ^ 1);
           uint8_t* sa = smem + stage * ML_STAGE_BYTES;
           uint8_t* sb = sa + ML_A_BYTES;
           const uint32_t bar = map_to_cta(smem_u32(&full_bar[stage]), 0);
           if (kt < k4) {
-            if (leader) mbar_expect_tx(&full_bar[stage], 2 * ML_STAGE_BYTES);
-            tma_load_2d_pair(sa, &map_a, bar, kt * 128, m0);
-            tma_load_2d_pair(sb, &map_b, bar, kt * 128, nb0);
-            uint8_t* ssfa = sb + ML_B_BYTES;
-            uint8_t* ssfb = ssfa + ML_SFA_BYTES;
-            tma_load_2d_pair(ssfa, &map_sfa, bar, 0, (int32_t)(sfa_rt * sf_tiles_k + kt * 4));
-            tma_load_2d_pair(ssfb, &map_sfb, bar, 0, (int32_t)(nt * sf_tiles_k + kt * 4));
+            if (load_a) {
+              if (leader) mbar_expect_tx(&full_bar[stage], 2 * (ML_A_BYTES + ML_SFA_BYTES));
+              tma_load_2d_pair(sa, &map_a, bar, kt * 128, m0);
+              tma_load_2d_pair(sb + ML_B_BYTES, &map_sfa, bar, 0, sfa_row + kt * 4);
+            } else {
+              if (leader) mbar_expect_tx(&full_bar[stage], 2 * (ML_B_BYTES + ML_SFB_BYTES));
+              tma_load_2d_pair(sb, &map_b, bar, kt * 128, nb0);
+              tma_load_2d_pair(sb + ML_B_BYTES + ML_SFA_BYTES, &map_sfb, bar, 0, sfb_row + kt * 4);
+            }
           } else {
             const int c0 = (kt - k4) * 64;
-            if (leader) mbar_expect_tx(&full_bar[stage], 2 * (ML_A_BYTES + ML_B_BYTES));
-            tma_load_2d_pair(sa, &map_h, bar, c0, m0);
-            tma_load_2d_pair(sb, &map_u, bar, c0, nb0);
+            if (load_a) {
+              if (leader) mbar_expect_tx(&full_bar[stage], 2 * ML_A_BYTES);
+              tma_load_2d_pair(sa, &map_h, bar, c0, m0);
+            } else {
+              if (leader) mbar_expect_tx(&full_bar[stage], 2 * ML_B_BYTES);
+              tma_load_2d_pair(sb, &map_u, bar, c0, nb0);
+            }
           }
           if (++stage == ML_STAGES) {
             stage = 0;
             phase ^= 1;
           }
-          if (kt == kt_d2 && i >= 1) load_d2(i - 1);
+          if (!load_a && kt == kt_d2 && i >= 1) load_d2(i - 1);
         }
       }
     }
@@ -207,9 +217,18 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
       const uint32_t sfa_t = tmem_base + ML_SF_COL, sfb_t = sfa_t + 8, h2_t = tmem_base + ML_H2_COL;
       const uint32_t zs_u = smem_u32(zs), d2_u = smem_u32(d2s);
       // H2 (+)= z tile [256 x 192] * D_f2 slice [192 x r2]: 12 MMAs of K = 16 on the staged tile of local tile j
+#ifdef FT_TRACE
+      long long tr_k = 0, tr_zw = 0, tr_dw = 0, tr_h2 = 0, tr_acc = 0, tr_t = clock64();
+      const long long tr_start = tr_t;
+#define MLP_TR(x) do { const long long now_ = clock64(); (x) += now_ - tr_t; tr_t = now_; } while (0)
+#else
+#define MLP_TR(x) do { } while (0)
+#endif
       auto h2_step = [&](int j) {
         mbar_wait(&z_full, (uint32_t)j & 1);
+        MLP_TR(tr_zw);
         mbar_wait(&d2_full, (uint32_t)j & 1);
+        MLP_TR(tr_dw);
         tc_fence_after();
         const bool first = j == 0 || seg_end(j - 1);
 #ifdef FT_TRACE
@@ -224,6 +243,7 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
                           (first && u == 0 && k == 0) ? 0u : 1u);
         tc_commit_pair(&z_free, 3);                 // the z tile and the slice may be overwritten
         if (seg_end(j)) tc_commit_pair(&h2_full, 3);   // the row tile's partial H2 is complete
+        MLP_TR(tr_h2);
       };
       int stage = 0;
       uint32_t phase = 0;
@@ -232,6 +252,7 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
         const uint32_t acc_t = tmem_base + a * ML_BN;
         mbar_wait(&acc_empty[a], (((uint32_t)i >> 1) & 1) ^ 1);   // tile i-2 drained
         tc_fence_after();
+        MLP_TR(tr_acc);
         for (int kt = 0; kt < kiters; ++kt) {
           mbar_wait(&full_bar[stage], phase);
           tc_fence_after();
@@ -261,9 +282,16 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
             phase ^= 1;
           }
         }
+        MLP_TR(tr_k);
         if (i >= 1) h2_step(i - 1);   // the z tile of the tile before is staged by now (its epilogue ran beside this tile)
       }
       h2_step(n_local - 1);
+#ifdef FT_TRACE
+      if (pair_id == 0 || pair_id == 41)
+        printf("mlp pair %d: %d tiles, per tile: acc_empty wait %.0f, K loop %.0f, z_full wait %.0f, d2_full wait %.0f, H2 issue %.0f; total %lld cycles\n",
+               (int)pair_id, n_local, (double)tr_acc / n_local, (double)tr_k / n_local, (double)tr_zw / n_local, (double)tr_dw / n_local,
+               (double)tr_h2 / n_local, clock64() - tr_start);
+#endif
     }
   } else if (warp >= 4) {
     // ===================================================== epilogue (both CTAs, own 128 rows)
@@ -278,6 +306,9 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
     const int64_t half_cols = p.N / 2, sf_tiles_n = p.N / 64;
     uint32_t amax_z2 = 0, amax_y2 = 0;   // running max of the bf16 magnitudes, two per word
     int seg = 0;                         // segments whose H2 accumulator this thread has drained
+#ifdef FT_TRACE
+    long long e_accw = 0, e_ld = 0, e_zfw = 0, e_math = 0, e_drain = 0;
+#endif
     // drain the H2 accumulator of the row tile mt to this pair's slot: 16-column pieces alternate between the groups
     auto drain_h2 = [&](int64_t mt) {
       mbar_wait(&h2_full, (uint32_t)seg & 1);
@@ -300,8 +331,15 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
       const int64_t mt = tile / tiles_n, nt = tile % tiles_n;
       const int64_t row = mt * ML_BM + rank * 128 + et;
       const bool live = row < p.M;
+#ifdef FT_TRACE
+      long long e_t = clock64();
+#define EPI_TR(x) do { const long long now_ = clock64(); (x) += now_ - e_t; e_t = now_; } while (0)
+#else
+#define EPI_TR(x) do { } while (0)
+#endif
       mbar_wait(&acc_full[a], ((uint32_t)i >> 1) & 1);
       tc_fence_after();
+      EPI_TR(e_accw);
       const uint32_t t0 = tmem_base + ((uint32_t)(q * 32) << 16) + a * ML_BN;
       {
         const int u = grp;
@@ -314,7 +352,9 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
           tmem_ld32(t0 + u * 64 + hh * 32, v);
           tmem_ld_wait();
           // the H2 MMAs of the tile before must have read the staged z before it is overwritten
+          if (hh == 0) EPI_TR(e_ld);
           if (hh == 0 && i >= 1) mbar_wait(&z_free, (uint32_t)(i - 1) & 1);
+          if (hh == 0) EPI_TR(e_zfw);
           if (hh == 1) {   // this warp's part of the accumulator is in registers: hand it back
             tc_fence_before();
             __syncwarp();
@@ -327,7 +367,11 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
               yb[j] = pack_bf16x2(__uint_as_float(v[16 * bb + 2 * j]) * alpha, __uint_as_float(v[16 * bb + 2 * j + 1]) * alpha);
+#if defined(FT_MLP_CT) && (FT_MLP_CT & 1)
+              zb[j] = yb[j];   // development builds: no GeLU at all (compile time)
+#else
               zb[j] = pack_bf16x2(gelu_tanh_f32(__uint_as_float(yb[j] << 16)), gelu_tanh_f32(__uint_as_float(yb[j] & 0xFFFF0000u)));
+#endif
 #ifdef FT_TRACE
               if (p.dbg & 1) zb[j] = yb[j];
 #endif
@@ -337,6 +381,10 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
             // z goes to the staged tile (the A operand of the H2 MMAs): two 16-byte pieces of the swizzled row
             *reinterpret_cast<uint4*>(zrow + (((2 * b) ^ (et & 7)) << 4)) = z0;
             *reinterpret_cast<uint4*>(zrow + (((2 * b + 1) ^ (et & 7)) << 4)) = z1;
+#if defined(FT_MLP_CT) && (FT_MLP_CT & 2)
+            cz[2 * bb] = z0.x; cz[2 * bb + 1] = z1.x; cy[2 * bb] = y0.x; cy[2 * bb + 1] = y1.x;   // no quantizer at all
+            continue;
+#endif
             const float az = amax_block16(z0, z1), ay = amax_block16(y0, y1);
             amax_z2 = __vmaxu2(amax_z2, __float_as_uint(az) >> 16);
             amax_y2 = __vmaxu2(amax_y2, __float_as_uint(ay) >> 16);
@@ -392,12 +440,19 @@ k_gemm4_mlp(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ C
       }
       // the H2 accumulator of a row tile that ended with the tile before must be out before the H2 MMAs of THIS
       // tile (which follow this warp's z_full arrival) overwrite it
+      EPI_TR(e_math);
       if (i >= 1 && seg_end(i - 1)) drain_h2((t_begin + i - 1) / tiles_n);
+      EPI_TR(e_drain);
       fence_proxy_async();   // the staged z is read by the tensor core (async proxy)
       __syncwarp();
       if (lane == 0) mbar_arrive_cluster(map_to_cta(smem_u32(&z_full), 0));
     }
     drain_h2((t_begin + n_local - 1) / tiles_n);
+#ifdef FT_TRACE
+    if (pair_id == 0 && rank == 0 && (warp == 4 || warp == 9) && lane == 0)
+      printf("mlp epilogue warp %d: per tile: acc_full wait %.0f, first tmem load %.0f, z_free wait %.0f, math+stores %.0f, drain_h2 %.0f\n",
+             warp, (double)e_accw / n_local, (double)e_ld / n_local, (double)e_zfw / n_local, (double)e_math / n_local, (double)e_drain / n_local);
+#endif
     // this step's tensor amax of Z and Y1 (for the next step's scaling)
     if (p.z_amax_out != nullptr) {
       uint32_t bz = max(amax_z2 & 0xFFFFu, amax_z2 >> 16), by = max(amax_y2 & 0xFFFFu, amax_y2 >> 16);
