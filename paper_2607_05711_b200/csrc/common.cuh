@@ -54,6 +54,11 @@ bool pdl_enabled();  // programmatic dependent launch of the GEMM and dA kernels
 constexpr int WS_MAX_QUANT_CTAS = 192;   // one CTA per SM
 constexpr size_t WS_CTL_BYTES = 4096;
 constexpr size_t WS_CTL_AMAX = 0, WS_CTL_BAR = 4, WS_CTL_EXIT = 8, WS_CTL_AMAX_EXT = 16;
+// per row tile of the quantize pass: how many CTAs have stored their partial H tile (k_finalize_h starts a tile's sum
+// as soon as the count is complete), and how many finalize blocks of the tile are done (the last one zeroes both)
+constexpr int WS_CTL_MAX_TILES = 480;
+constexpr size_t WS_CTL_TILE_CNT = 64, WS_CTL_TILE_DONE = WS_CTL_TILE_CNT + 4 * WS_CTL_MAX_TILES;
+static_assert(WS_CTL_TILE_DONE + 4 * WS_CTL_MAX_TILES <= WS_CTL_BYTES, "control words");
 constexpr int WS_WG_TILES = 2 * WS_MAX_QUANT_CTAS;   // dB^T slots: slices x feature tiles of 128 <= 2 CTAs per SM
 struct WsLayout {
   size_t hs_off, slots_off, wg_off, wg_floats, total;

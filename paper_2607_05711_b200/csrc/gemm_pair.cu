@@ -432,6 +432,8 @@ k_gemm4_pair(const __grid_constant__ CUtensorMap map_a, const __grid_constant__ 
 #ifdef FT_TRACE
               if (p.dbg & 8) {   // timing only: conversion, no stores
                 if ((lo.x ^ hi.w) == 0x12345677u) p.out[1] = __float2bfloat16(1.0f);
+              } else if (p.dbg & 16) {   // timing only: the same stores into a per-CTA region that stays in L2
+                st_global_v8(p.out + ((int64_t)(blockIdx.x * 128 + et)) * p.N + c0 + 16 * j, lo, hi);
               } else
 #endif
               if (p.out_align32) {

@@ -22,8 +22,10 @@
 // warps: the ring stalls for the 1-2 us of every drain; with a projection the main loop now ends when the
 // projection-less one does).  k_finalize_h, launched behind the kernel with a programmatic edge, sums every
 // row over its slots in CTA order and writes bf16 H and Hs = H * (1 / alpha): no atomics on the data, a
-// fixed summation order (the same bits on every run), thousands of threads with one L2 round trip each, and
-// the GEMM that follows runs its 4-bit stages beside it (gemm_pair.cu, lr_late).  Measured in round 2 and
+// fixed summation order (the same bits on every run), thousands of threads with one L2 round trip each.  Its
+// blocks run beside this kernel: a CTA counts itself in for a row tile (control word, release) once its slot is
+// stored and the tensor scale written, a finalize block starts when its tile's count is complete, and the
+// GEMM that follows runs its 4-bit stages beside whatever is left of it (gemm_pair.cu, lr_late).  Measured in round 2 and
 // dropped (profiles/r02_experiments.md, B2): the sums inside this kernel -- by the CTA whose arrival completes
 // a row tile (36 finalizers, each a chain of L2 round trips: 6-11 us of tail at C2), or by every CTA behind a
 // grid barrier (imbalance + drain + fence + poll + sum: 6-8 us of tail that nothing can overlap); fp32
@@ -64,6 +66,8 @@ struct QFParams {
   int64_t rows, cols;
   const float* amax_in;         // streaming: tensor amax (device)
   uint32_t* ctl;                // control words of the workspace (WS_CTL_*), or null (amax given, no projection)
+  uint32_t* tile_cnt;           // per-row-tile arrival counters (WS_CTL_TILE_CNT), or null: k_finalize_h waits for the grid
+  uint32_t* tile_done;          // per-row-tile count of finished finalize blocks
   float* slots;                 // [(grid + row tiles) x 128 x r_t] fp32 partial H tiles (not zeroed)
   uint8_t* codes;
   uint8_t* sf;
@@ -109,7 +113,7 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
   // 1024-byte alignment for the 128-byte swizzle atoms
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   __shared__ uint64_t full_x[QF_MAX_NX], empty_x[QF_MAX_NX], full_d[QF_MAX_ND], empty_d[QF_MAX_ND];
-  __shared__ uint64_t acc_full[2], acc_free[2];
+  __shared__ uint64_t acc_full[2], acc_free[2], gdec_bar;
   __shared__ float enc_tab[128];
   __shared__ uint32_t tmem_base_s, s_red[QF_QWARPS], s_amax;
 
@@ -137,6 +141,7 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       mbar_init(&acc_full[a], 1);   // tcgen05.commit of a segment's last MMA
       mbar_init(&acc_free[a], 4);   // the four drain warps
     }
+    mbar_init(&gdec_bar, 1);        // this CTA has written the tensor scale (the drain warps publish their slots after it)
     fence_mbar_init();
   }
   if (R_T > 0 && warp == QF_W_ISSUER) {
@@ -280,6 +285,16 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
     // Warp w may read TMEM lanes 32 (w % 4) .. + 31 = rows of the tile.
     if constexpr (R_T > 0) {
       const int dq = warp & 3;
+      // the slot of segment seg is complete in memory and the tensor scale written: count this CTA in for row tile
+      // t0 + seg (release; k_finalize_h acquires the count)
+      auto publish = [&](int seg) {
+        asm volatile("bar.sync 2, 128;" ::: "memory");   // the four drain warps have stored their parts
+        if (warp == QF_W_DRAIN && lane == 0) {
+          mbar_wait(&gdec_bar, 0);
+          __threadfence();
+          asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p.tile_cnt + t0 + seg) : "memory");
+        }
+      };
       for (int seg = 0; seg < nseg; ++seg) {
         const int a = seg & 1;
         mbar_wait(&acc_full[a], (uint32_t)(seg >> 1) & 1);
@@ -299,8 +314,13 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(&acc_free[a]);   // the accumulator may be overwritten
+        if (!SINGLE && p.tile_cnt != nullptr) publish(seg);
       }
-      // the partial H tiles are in their slots; k_finalize_h (next launch) sums them
+      // the partial H tiles are in their slots; k_finalize_h (next launch) sums a row tile as soon as all its slots
+      // are published.  Single pass: the tensor scale is known only behind the grid barrier, the segments (at most
+      // three) are published then.
+      if (SINGLE && p.tile_cnt != nullptr)
+        for (int seg = 0; seg < nseg; ++seg) publish(seg);
     }
   } else {
     // =========================================================== quantizer warps: two groups of eight, group g
@@ -383,7 +403,10 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
     if constexpr (!SINGLE) {
       // ---- streaming mode (amax known)
       ts = tensor_scale(__ldcg(p.amax_in));
-      if (blockIdx.x == 0 && tid == 0) *p.g_dec_out = ts.g_dec;
+      if (tid == 0) {   // every CTA writes the (same) tensor scale: whoever sees this CTA's slots published sees it too
+        *p.g_dec_out = ts.g_dec;
+        mbar_arrive(&gdec_bar);
+      }
       if (tid < 128) enc_tab[tid] = enc_of_sf8((uint32_t)tid, ts.g_dec);
       qsync();
       if (grp == 1) advance_out();
@@ -431,7 +454,10 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
       QF_STAMP(3);
       qsync();
       ts = tensor_scale(__uint_as_float(s_amax));
-      if (blockIdx.x == 0 && tid == 0) *p.g_dec_out = ts.g_dec;
+      if (tid == 0) {
+        *p.g_dec_out = ts.g_dec;
+        mbar_arrive(&gdec_bar);
+      }
       if (tid < 128) enc_tab[tid] = enc_of_sf8((uint32_t)tid, ts.g_dec);
       qsync();
       // ---- phase 2: quantize from shared memory
@@ -476,8 +502,12 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
 template <int R_T>
 __global__ void __launch_bounds__(1024) k_finalize_h(const QFParams p, int G, const SumJob job) {
   constexpr int SLOT_F4 = QF_ROWS * R_T / 4;
-  __shared__ float4 s_part[8][QF_ROWS];
-  pdl_wait();      // the slots and g_dec come from the quantize kernel before us
+  extern __shared__ float4 s_part[];   // [P][QF_ROWS], P > 1 only
+  const bool flags = p.tile_cnt != nullptr;
+  // flags: this kernel's blocks may run BESIDE the quantize kernel and start a row tile's sum as soon as all its
+  // slots are published; they wait for that kernel as a whole only before they exit (completion stays transitive:
+  // the GEMM behind us needs its codes and scales).  No flags: wait for it here.
+  if (!flags) pdl_wait();
   pdl_trigger();
   if (job.n_slots > 0) {   // side job (ft_linear_bwd: the M slices of dB^T, written two kernels ago): slot order
     const int64_t nthr = (int64_t)gridDim.x * gridDim.y * blockDim.x * blockDim.y;
@@ -494,8 +524,6 @@ __global__ void __launch_bounds__(1024) k_finalize_h(const QFParams p, int G, co
       job.out[i] = a;
     }
   }
-  float inv_alpha = 1.0f;   // Hs = bf16(H * (1 / alpha)), alpha = g_dec(this) * g_dec(other)
-  if (p.hs_out != nullptr) inv_alpha = __fdiv_rn(1.0f, __fmul_rn(__ldcg(p.g_dec_out), __ldg(p.other_dec_scale)));
   const int C = p.chunks_per_tile;
   const int64_t TC = p.total_chunks;
   const int r = threadIdx.x, part = threadIdx.y, P = blockDim.y;
@@ -505,6 +533,19 @@ __global__ void __launch_bounds__(1024) k_finalize_h(const QFParams p, int G, co
   // the CTAs whose ranges meet row tile t: owner(c) = floor(((c + 1) * G - 1) / TC)
   const int i_lo = (int)(((t * C + 1) * G - 1) / TC);
   const int i_hi = (int)((((t + 1) * C) * G - 1) / TC);
+  if (flags) {
+    if (r == 0 && part == 0) {
+      const uint32_t want = (uint32_t)(i_hi - i_lo + 1);
+      const uint64_t t_start = globaltimer_ns();
+      while (ld_acquire_u32(p.tile_cnt + t) < want) {
+        __nanosleep(64);
+        if (globaltimer_ns() - t_start > 2000000000ull) __trap();   // fail, do not hang
+      }
+    }
+    __syncthreads();
+  }
+  float inv_alpha = 1.0f;   // Hs = bf16(H * (1 / alpha)), alpha = g_dec(this) * g_dec(other)
+  if (p.hs_out != nullptr) inv_alpha = __fdiv_rn(1.0f, __fmul_rn(__ldcg(p.g_dec_out), __ldg(p.other_dec_scale)));
   const float4* src = reinterpret_cast<const float4*>(p.slots) + (i_lo + t) * SLOT_F4 + q * QF_ROWS + r;
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
   constexpr int BATCH = 8;   // loads in flight per thread
@@ -522,24 +563,36 @@ __global__ void __launch_bounds__(1024) k_finalize_h(const QFParams p, int G, co
     }
   }
   if (P > 1) {
-    s_part[part][r] = acc;
+    s_part[part * QF_ROWS + r] = acc;
     __syncthreads();
-    if (part != 0) return;
-    for (int k = 1; k < P; ++k) {
-      const float4 o = s_part[k][r];
-      acc.x += o.x;
-      acc.y += o.y;
-      acc.z += o.z;
-      acc.w += o.w;
-    }
+    if (part == 0)
+      for (int k = 1; k < P; ++k) {
+        const float4 o = s_part[k * QF_ROWS + r];
+        acc.x += o.x;
+        acc.y += o.y;
+        acc.z += o.z;
+        acc.w += o.w;
+      }
   }
-  if (gr >= p.rows) return;
-  if (p.h_out != nullptr)
-    *reinterpret_cast<uint2*>(p.h_out + gr * R_T + q * 4) = make_uint2(pack_bf16x2(acc.x, acc.y), pack_bf16x2(acc.z, acc.w));
-  if (p.hs_out != nullptr)
-    *reinterpret_cast<uint2*>(p.hs_out + gr * R_T + q * 4) =
-        make_uint2(pack_bf16x2(__fmul_rn(acc.x, inv_alpha), __fmul_rn(acc.y, inv_alpha)),
-                   pack_bf16x2(__fmul_rn(acc.z, inv_alpha), __fmul_rn(acc.w, inv_alpha)));
+  if (part == 0 && gr < p.rows) {
+    if (p.h_out != nullptr)
+      *reinterpret_cast<uint2*>(p.h_out + gr * R_T + q * 4) = make_uint2(pack_bf16x2(acc.x, acc.y), pack_bf16x2(acc.z, acc.w));
+    if (p.hs_out != nullptr)
+      *reinterpret_cast<uint2*>(p.hs_out + gr * R_T + q * 4) =
+          make_uint2(pack_bf16x2(__fmul_rn(acc.x, inv_alpha), __fmul_rn(acc.y, inv_alpha)),
+                     pack_bf16x2(__fmul_rn(acc.z, inv_alpha), __fmul_rn(acc.w, inv_alpha)));
+  }
+  if (flags) {
+    __syncthreads();   // every thread of the block has read its slots
+    if (r == 0 && part == 0) {
+      // the last block of this row tile puts its two counters back to zero for the next call
+      if (atomicAdd(p.tile_done + t, 1u) == gridDim.x - 1) {
+        p.tile_cnt[t] = 0u;
+        p.tile_done[t] = 0u;
+      }
+    }
+    pdl_wait();   // "this grid complete" implies "the quantize kernel complete"
+  }
 }
 
 int launch_amax(const void* x_bf16, int64_t n, float* amax_out, cudaStream_t st, bool zero_first, bool pdl);
@@ -625,7 +678,8 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3((unsigned)(R_T / 4), (unsigned)tiles, 1);
       cfg.blockDim = dim3(QF_ROWS, (unsigned)parts, 1);
-      cfg.stream = st;
+      cfg.dynamicSmemBytes = parts > 1 ? (size_t)parts * QF_ROWS * sizeof(float4) : 0;   // none on the large shapes: the
+      cfg.stream = st;                                                                    // blocks fit beside the quantize CTAs
       cudaLaunchAttribute attr[1];
       attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
       attr[0].val.programmaticStreamSerializationAllowed = 1;
@@ -710,6 +764,9 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
   p.cols = cols;
   p.amax_in = amax_t;
   p.ctl = reinterpret_cast<uint32_t*>(ws);
+  const bool tile_flags = ws != nullptr && r_t > 0 && ceil_div(rows, QF_ROWS) <= WS_CTL_MAX_TILES;
+  p.tile_cnt = tile_flags ? reinterpret_cast<uint32_t*>(ws + WS_CTL_TILE_CNT) : nullptr;
+  p.tile_done = tile_flags ? reinterpret_cast<uint32_t*>(ws + WS_CTL_TILE_DONE) : nullptr;
   p.slots = ws ? reinterpret_cast<float*>(ws + ws_layout(rows, r_t).slots_off) : nullptr;
   p.codes = out->codes;
   p.sf = out->sf;
