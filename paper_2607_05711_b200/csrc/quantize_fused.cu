@@ -81,6 +81,7 @@ struct QFParams {
   int64_t total_chunks;         // TC = row tiles * C
 #ifdef FT_TRACE
   unsigned long long* trace;    // development builds only: 8 globaltimer stamps per CTA
+  int dbg;                      // 1 = no D-slice loads, 2 = no MMAs, 4 = no slot stores (timing only)
 #endif
 };
 
@@ -189,8 +190,19 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
         uint32_t phx = 0;
         for (int it = 0; it < n; ++it) {
           if (it >= NX) mbar_wait(&empty_x[sx], phx ^ 1);
+#ifdef FT_TRACE
+          if (p.dbg & 1) {
+            mbar_expect_tx(&full_x[sx], QF_X_BYTES);
+            tma_load_2d_hint(smem + sx * QF_X_BYTES, &map_x, &full_x[sx], kc * QF_KC, t * QF_ROWS, pol_stream);
+          } else
+#endif
+          {
           mbar_expect_tx(&full_x[sx], QF_X_BYTES + (R_T > 0 ? D_BYTES : 0));
           tma_load_2d_hint(smem + sx * QF_X_BYTES, &map_x, &full_x[sx], kc * QF_KC, t * QF_ROWS, pol_stream);
+          }
+#ifdef FT_TRACE
+          if (!(p.dbg & 1))
+#endif
           if constexpr (R_T > 0) {
 #pragma unroll
             for (int g = 0; g < NG; ++g)
@@ -256,6 +268,9 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
           if (first && seg >= 2) mbar_wait(&acc_free[seg & 1], (uint32_t)((seg >> 1) - 1) & 1);
           tc_fence_after();
           if constexpr (!SINGLE) {
+#ifdef FT_TRACE
+            if (!(p.dbg & 2))
+#endif
             issue_mma(xs_u + sx * QF_X_BYTES, ds_u + sx * D_BYTES, tmem_base_s + (seg & 1) * ACC_COLS, first);
             tc_commit(&empty_x[sx]);                      // slot free once the MMAs have read it
           } else {
@@ -307,6 +322,9 @@ k_quantize_fused(const __grid_constant__ CUtensorMap map_x, const __grid_constan
           uint32_t v[16];
           tmem_ld16(tmem_base_s + ((uint32_t)(dq * 32) << 16) + a * ACC_COLS + c0, v);
           tmem_ld_wait();
+#ifdef FT_TRACE
+          if (!(p.dbg & 4))
+#endif
 #pragma unroll
           for (int j = 0; j < 16; j += 4)
             *reinterpret_cast<uint4*>(dst + (c0 + j) / 4 * (QF_ROWS * 4)) = make_uint4(v[j], v[j + 1], v[j + 2], v[j + 3]);
@@ -779,6 +797,7 @@ int launch_quantize_fused(const void* x, int64_t rows, int64_t cols, const float
   p.total_chunks = ceil_div(rows, QF_ROWS) * (cols / QF_KC);
 #ifdef FT_TRACE
   p.trace = g_qf_trace;
+  p.dbg = getenv("FT_QF_DBG") ? atoi(getenv("FT_QF_DBG")) : 0;
 #endif
   switch (r_t) {
     case 0: return launch_qf<0>(mx, md, p, x, amax_t, after_kernel, finalize_last, job, st);
