@@ -704,7 +704,10 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
       cfg.attrs = attr;
       cfg.numAttrs = pdl_enabled() ? 1 : 0;
       FT_CUDA_TRY(cudaLaunchKernelEx(&cfg, k_finalize_h<(R_T > 0 ? R_T : 16)>, p, grid, job));
-      if (finalize_last != nullptr) *finalize_last = true;   // the caller's GEMM may start beside it (gemm_pair.cu)
+      // The caller's GEMM may start beside k_finalize_h (gemm_pair.cu, lr_late) only if every finalize block has waited
+      // for the quantize grid BEFORE it lets its dependents go, i.e. without the tile counters: with them the blocks
+      // trigger at once and wait at their end, and a GEMM that skipped its own wait could read codes still being written.
+      if (finalize_last != nullptr) *finalize_last = p.tile_cnt == nullptr;
     }
     return FT_OK;
   };
@@ -731,6 +734,14 @@ static int launch_qf(const CUtensorMap& mx, const CUtensorMap& md, QFParams p, c
     after_kernel = true;
   }
   p.amax_in = amax_t;
+  // Streaming: nearly every row tile is completed by a CTA whose range ENDS in it, so the sums cannot start before
+  // the kernel's end whatever the protocol.  A caller that chains a GEMM (finalize_last != NULL) is better served by
+  // the grid-wide wait + lr_late (the GEMM's 4-bit stages run beside the sums); a stand-alone call by the counters
+  // (the finalize blocks are resident and start the moment the last slot lands).
+  if (finalize_last != nullptr) {
+    p.tile_cnt = nullptr;
+    p.tile_done = nullptr;
+  }
   const int stage = QF_X_BYTES + (R_T == 0 ? 0 : D_BYTES);
   int nxs = (QF_SMEM_MAX - 1024) / stage;          // as deep as shared memory allows: 9 x 24 KB, 7 x 32 KB, 12 x 16 KB
   if (nxs > QF_MAX_NX) nxs = QF_MAX_NX;
