@@ -32,8 +32,8 @@ FP4_NOMINAL_TFLOPS = 9000.0   # dense NVFP4, B200 (B200_PROFILING.md): the peak 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch (bytes) from the ncu --set full capture of the C2 step
 # summarised in profiles/r02_full_summary.md (ncu flushes the caches before every launch: cold-cache figures; the
 # quantize entries include their k_finalize_h launch)
-NCU_DRAM_TRAFFIC = {"gemm_fwd": 61.67e6, "gemm_dgrad": 45.28e6, "quantize_X": 34.67e6, "quantize_G": 102.86e6,
-                    "wgrad_dBt": 89.21e6, "wgrad_dA": 29.32e6}
+NCU_DRAM_TRAFFIC = {"gemm_fwd": 62.30e6, "gemm_dgrad": 45.00e6, "quantize_X": 34.67e6, "quantize_G": 102.86e6,
+                    "wgrad_dBt": 89.46e6, "wgrad_dA": 29.31e6}
 PROBE_SRC = os.path.join(ROOT, "bench_fp4_probe.cu")
 PROBE_BIN = os.path.join(ROOT, "build", "bench_fp4_probe")
 
