@@ -232,7 +232,10 @@ def test_weight_quantize_16x16_and_pack(B, N, K):
 
 @pytest.mark.parametrize("rows,cols,r_t,kind", [(128, 512, 16, "x"), (200, 1024, 64, "x"), (256, 3072, 48, "x"),
                                                 (384, 2048, 96, "g"), (130, 4096, 128, "g"), (1, 64, 32, "x"),
-                                                (2000, 128, 64, "x"), (4608, 3072, 64, "x"), (2304, 3072, 128, "g")] +
+                                                (2000, 128, 64, "x"), (4608, 3072, 64, "x"), (2304, 3072, 128, "g"),
+                                                # 481 row tiles: more than the workspace has per-tile counters for
+                                                # (480): k_finalize_h falls back to the grid-wide wait
+                                                (61500, 64, 16, "g")] +
                          [(rows, cols, 32, "x") for rows, cols in synth.C4_SHAPES])
 def test_fused_projection(B, qmode, rows, cols, r_t, kind):
     rng = synth.make_rng(rows + cols + r_t)
