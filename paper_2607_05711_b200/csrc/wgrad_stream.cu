@@ -16,6 +16,8 @@
 //   * dA: the last kernel of the call has nobody behind it to add slots; its slices meet by red.global.add.v4.f32
 //     in a buffer that the dB^T launch cleared on its way (order of the additions not fixed: DESIGN.md O-17).
 // ft_lora_wgrad (the standalone call, no workspace) keeps wgrad.cu's cluster kernel.
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace ft {
@@ -41,6 +43,9 @@ struct WgsParams {
                                 //    wait for it at the END (completion stays transitive for the next launch)
   float4* zero_fill;            // non-null: buffer this launch clears for a LATER launch (zero_fill_n4 float4s)
   int64_t zero_fill_n4;
+#ifdef FT_TRACE
+  int dbg;                      // development builds: 1 = no MMAs, 2 = no amax fold, 4 = no L2 hint
+#endif
 };
 
 __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float c, float d) {
@@ -94,7 +99,11 @@ k_wgrad_s(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CU
   if (warp == 0) {
     if (elect_one()) {   // ---- TMA producer
       // the pass that also finds max |G| is followed by the quantize pass over the same G: ask L2 to keep it
+#ifdef FT_TRACE
+      const bool keep = p.amax_bits != nullptr && !(p.dbg & 4);
+#else
       const bool keep = p.amax_bits != nullptr;
+#endif
       const uint64_t pol = l2_policy_evict_last();
       for (int it = 0; it < n_chunks; ++it) {
         const int s = it % WS_STAGES;
@@ -123,6 +132,9 @@ k_wgrad_s(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CU
         tc_fence_after();
         const uint32_t in_u = smem_u32(smem + s * STAGE_BYTES);
         const uint32_t l_u = in_u + WS_IN_BYTES;
+#ifdef FT_TRACE
+        if (!(p.dbg & 1))
+#endif
 #pragma unroll
         for (int k = 0; k < 4; ++k)   // 16 rows of m per MMA = two 8-row swizzle groups = 2048 bytes
           mma_bf16(tmem_base, make_smem_desc(in_u + k * 2048, 1024, WS_MC * 128, 2),
@@ -140,6 +152,9 @@ k_wgrad_s(const __grid_constant__ CUtensorMap map_in, const __grid_constant__ CU
       const int s = it % WS_STAGES;
       mbar_wait(&full_bar[s], (it / WS_STAGES) & 1);
       const uint4* src = reinterpret_cast<const uint4*>(smem + s * STAGE_BYTES);
+#ifdef FT_TRACE
+      if (!(p.dbg & 2))
+#endif
 #pragma unroll 4
       for (int j = 0; j < WS_IN_BYTES / 16 / 64; ++j) {
         const uint4 v = src[t64 + j * 64];
@@ -250,6 +265,9 @@ int launch_wgrad_stream(const void* in, const void* l, int64_t M, int64_t F, int
   p.amax_bits = amax_in;
   p.zero_fill = reinterpret_cast<float4*>(zero_fill);
   p.zero_fill_n4 = zero_fill_n / 4;   // F' * r, r % 16 == 0
+#ifdef FT_TRACE
+  p.dbg = getenv("FT_WG_DBG") ? atoi(getenv("FT_WG_DBG")) : 0;
+#endif
   const bool pdl = after_kernel;
   p.late_wait = (beside_prev && pdl && zero_fill == nullptr) ? 1 : 0;
   const dim3 grid((unsigned)f_tiles, sl, 1);
