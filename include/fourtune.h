@@ -178,9 +178,9 @@ int ft_pack_weight(const ft_qtensor* r_kmajor, ft_qtensor* r_kmajor_tiled,
  * ([N x K/2 bytes]) -- the 4-bit elements transposed, nothing re-quantized; the same bytes ft_pack_weight writes to
  * r_nmajor->codes.  A caller that keeps ONE copy of the codes per layer points every layer's r_nmajor.codes at one
  * scratch buffer of max_layers(N K / 2) bytes and calls this before that layer's backward (same stream); the two
- * scale layouts (1/8 of the codes) stay per layer.  The tensor core takes 4-bit operands K-major only, and moving
- * the transposition into the dgrad main loop would cost more shared-memory traffic than the loop has to spare
- * (DESIGN.md section 5): a separate HBM-bound pass it is.  N % 64 == 0, K % 64 == 0; both pointers 16-byte aligned. */
+ * scale layouts (1/8 of the codes) stay per layer.  The tensor core takes 4-bit operands K-major only, and a
+ * transposition inside the dgrad main loop would put ordinary warps and one more hand-off per stage on a chain that
+ * runs at the tensor core's rate: a separate HBM-bound pass it is.  N % 64 == 0, K % 64 == 0; both pointers 16-byte aligned. */
 int ft_weight_transpose_codes(const ft_qtensor* r_kmajor, uint8_t* codes_t, void* stream);
 
 /* ---- a0+a1+a2: forward.  x_bf16 [M x K] -> y_bf16 [M x N].
