@@ -489,8 +489,10 @@ static int choose_pair_bn(int64_t M, int64_t N, int64_t K, int r_t, int ntile_av
 // the tile-cut scale layout worth packing for a weight that will meet M tokens: 224, 240, or 0 (256-wide tiles win)
 int best_pair_ntile(int64_t M, int64_t N, int64_t K, int r_t) {
   const int64_t pairs = sm_count() / 2;
-  const double c224 = pair_cost(224, M, N, K, r_t, pairs), c240 = pair_cost(240, M, N, K, r_t, pairs),
-               c256 = pair_cost(256, M, N, K, r_t, pairs);
+  const double c256 = pair_cost(256, M, N, K, r_t, pairs);
+  // a width that would leave a 16-column last tile is not run (launch_gemm4_pair): never worth packing for
+  const double c224 = N % 224 == 16 ? 2.0 * c256 : pair_cost(224, M, N, K, r_t, pairs);
+  const double c240 = N % 240 == 16 ? 2.0 * c256 : pair_cost(240, M, N, K, r_t, pairs);
   if (c256 <= c224 && c256 <= c240) return 0;
   return c240 < c224 ? 240 : 224;
 }
@@ -561,6 +563,9 @@ int launch_gemm4_pair(const ft_qtensor* a, const ft_qtensor* b, int64_t M, int64
   const int avail = (b->sf_ntile != nullptr) ? b->ntile : 0;
   int bn = choose_pair_bn(M, N, K, r_t, avail);
   if (bn != 256 && bn != avail) bn = 256;   // no scale layout for that width: the 256-wide kernel takes the standard one
+  // a last column tile of 16 columns would be an MMA of N = 16 across the pair (8 rows of B per CTA): below what the
+  // instruction takes with M = 256.  256-wide tiles leave multiples of 64.
+  if (bn != 256 && N % bn == 16) bn = 256;
   if (bn == 224) return launch_pair_bn<224>(a, b, M, N, K, lr_a, lr_b, r_t, out, lr_late, st);
   if (bn == 240) return launch_pair_bn<240>(a, b, M, N, K, lr_a, lr_b, r_t, out, lr_late, st);
   return launch_pair_bn<256>(a, b, M, N, K, lr_a, lr_b, r_t, out, lr_late, st);

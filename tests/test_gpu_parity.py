@@ -367,7 +367,8 @@ LAYER_CASES = [  # seed, M, K, N, r_s, r, tile_n (fourtune_debug.h: 0 auto, 128/
     (21, 129, 2048, 640, 0, 16, 1224), (22, 200, 1024, 768, 32, 64, 1224), (23, 260, 448, 1024, 16, 96, 1224),
     (24, 300, 576, 448, 32, 32, 1256), (25, 200, 1024, 768, 32, 64, 1256),
     (26, 1, 64, 64, 0, 0, 1240), (27, 130, 320, 192, 16, 16, 1240), (28, 300, 576, 448, 32, 32, 1240),
-    (29, 129, 2048, 640, 0, 16, 1240), (30, 260, 448, 1024, 16, 96, 1240), (31, 200, 1024, 960, 32, 64, 1240)]
+    (29, 129, 2048, 640, 0, 16, 1240), (30, 260, 448, 1024, 16, 96, 1240), (31, 200, 1024, 960, 32, 64, 1240),
+    (32, 140, 256, 256, 16, 16, 1240)]   # N = 240 + 16: the launcher must not run a 16-column tile (falls back to 256)
 
 
 @pytest.mark.parametrize("seed,M,K,N,r_s,r,bn", LAYER_CASES)
